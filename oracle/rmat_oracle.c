@@ -1,0 +1,96 @@
+/*
+ * oracle/rmat_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * A plain, slow, obviously-correct CPU evaluation of the R-matrix of
+ * PSTGF (arxiv 1909.07321), eq. 4, PAPER.md:108:
+ *
+ *     R_nm(E) = 1/(2 r0) * sum_{k=1..M} w_nk w_mk / (E_k - E)
+ *
+ * with r0 == a the R-matrix radius (record RA), w_nk the
+ * surface amplitudes (record WMAT; n over channels, k over the
+ * Hamiltonian size) and E_k the R-matrix poles (record
+ * VALUE).
+ *
+ * The method reaches exactly this result (up to rounding order), so the
+ * oracle is the definition written out: every one of the n_chan^2 entries of
+ * every energy is an independent k-ascending sum in FP64, each term
+ * (w_nk*w_mk)/(E_k-E), added with Neumaier's compensated summation
+ * (north_star: "plain, slow CPU triple loop in FP64 with compensated (Kahan)
+ * summation").  No blocking, no symmetry shortcut, no reordering.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may call this.  It shares no code with
+ * paper_1909_07321_b200/csrc and neither side includes the other.
+ *
+ * Pins (tests/test_oracle_pins.py): exact rational brute force, the hand
+ * example of tests/golden/eq4_hand_example.txt, the single-pole closed form,
+ * symmetry, definiteness, the resolvent identity, exact scalings, block
+ * structure, additivity, degenerate poles vs. a library SYRK.  Nothing in
+ * this file is "parity unpinned".
+ *
+ * Build: gcc -O2 -std=c11 -fno-fast-math -ffp-contract=off -fopenmp -fPIC -shared
+ * (-ffp-contract=off keeps the compensation from being fused away).
+ */
+#include <math.h>
+#include <stddef.h>
+
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+/* One entry of eq. 4 at one energy: k ascending, Neumaier-compensated. */
+static double eq4_entry(const double *w_n, const double *w_m, const double *E_k,
+                        int n_poles, double E, double a)
+{
+    double s = 0.0, c = 0.0;
+    for (int k = 0; k < n_poles; ++k) {
+        double t = (w_n[k] * w_m[k]) / (E_k[k] - E);
+        double u = s + t;
+        if (fabs(s) >= fabs(t))
+            c += (s - u) + t;
+        else
+            c += (t - u) + s;
+        s = u;
+    }
+    return (s + c) / (2.0 * a);
+}
+
+/*
+ * R_out[e][n][m] for e in [0,n_E), n,m in [0,n_chan): dense, row-major.
+ * W is row-major [n_chan][ldw] with k contiguous (reading R6).
+ * threads <= 1 runs serially; threads > 1 splits the energy loop only
+ * (the arithmetic of each entry is unchanged).  Returns 0, or 1 on bad
+ * arguments.
+ */
+int oracle_rmat_form(const double *W, long long ldw, const double *E_k,
+                     const double *energies, int n_chan, int n_poles, int n_E,
+                     double a, double *R_out, int threads)
+{
+    if (n_chan < 0 || n_poles < 0 || n_E < 0 || ldw < n_poles) return 1;
+    if (n_chan == 0 || n_E == 0) return 0;
+    if (!W && n_poles > 0) return 1;
+    if (!energies || !R_out) return 1;
+    (void)threads;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(dynamic, 1) num_threads(threads > 1 ? threads : 1)
+#endif
+    for (int e = 0; e < n_E; ++e) {
+        double E = energies[e];
+        double *R = R_out + (size_t)e * (size_t)n_chan * (size_t)n_chan;
+        for (int n = 0; n < n_chan; ++n)
+            for (int m = 0; m < n_chan; ++m)
+                R[(size_t)n * n_chan + m] =
+                    eq4_entry(W + (size_t)n * ldw, W + (size_t)m * ldw, E_k, n_poles, E, a);
+    }
+    return 0;
+}
+
+/* Threads the OpenMP runtime would use by default (for reporting "cores"). */
+int oracle_max_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}

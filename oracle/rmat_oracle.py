@@ -1,0 +1,80 @@
+"""ctypes wrapper around oracle/rmat_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+The oracle evaluates eq. 4 of arxiv 1909.07321 entry by entry
+in FP64 with Neumaier summation; see the header of ``rmat_oracle.c``.  Only
+``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s cpu_baseline /
+``--impl reference`` legs may import this module.  It imports nothing from
+``paper_1909_07321_b200`` and the product never imports it.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "rmat_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle_rmat.so")
+_CFLAGS = ["-O2", "-std=c11", "-fno-fast-math", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared"]
+
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the C oracle in-tree (gcc); returns the library path."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".tmp{os.getpid()}"
+        subprocess.run(["gcc", *_CFLAGS, _SRC, "-o", tmp, "-lm"], check=True)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        dp = ctypes.POINTER(ctypes.c_double)
+        lib.oracle_rmat_form.argtypes = [dp, ctypes.c_longlong, dp, dp, ctypes.c_int, ctypes.c_int,
+                                         ctypes.c_int, ctypes.c_double, dp, ctypes.c_int]
+        lib.oracle_rmat_form.restype = ctypes.c_int
+        lib.oracle_max_threads.argtypes = []
+        lib.oracle_max_threads.restype = ctypes.c_int
+        _lib = lib
+    return _lib
+
+
+def max_threads() -> int:
+    return int(_load().oracle_max_threads())
+
+
+def _dptr(a: np.ndarray):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def rmat_form(W, E_k, energies, a: float, threads: int = 1) -> np.ndarray:
+    """R[e, n, m] of eq. 4 for one partial wave.
+
+    W [n_chan, n_poles] (row-major, any ld via a strided view's base is NOT
+    supported: the array is made contiguous), E_k [n_poles], energies [n_E].
+    """
+    W = np.ascontiguousarray(W, dtype=np.float64)
+    E_k = np.ascontiguousarray(E_k, dtype=np.float64)
+    energies = np.ascontiguousarray(energies, dtype=np.float64)
+    if W.ndim != 2 or E_k.ndim != 1 or energies.ndim != 1 or W.shape[1] != E_k.shape[0]:
+        raise ValueError("shape mismatch: W [n_chan, n_poles], E_k [n_poles], energies [n_E]")
+    n_chan, n_poles = W.shape
+    n_E = energies.shape[0]
+    R = np.zeros((n_E, n_chan, n_chan), dtype=np.float64)
+    # ld >= 1 keeps ctypes happy for n_poles == 0
+    rc = _load().oracle_rmat_form(_dptr(W), max(n_poles, 0), _dptr(E_k), _dptr(energies),
+                                  n_chan, n_poles, n_E, float(a), _dptr(R), int(threads))
+    if rc != 0:
+        raise ValueError(f"oracle_rmat_form rejected its arguments (rc={rc})")
+    return R
+
+
+def rmat_form_batch(waves, threads: int = 1) -> list[np.ndarray]:
+    """Eq. 4 for each partial wave of a ragged batch (objects with W, E_k, energies, a)."""
+    return [rmat_form(w.W, w.E_k, w.energies, w.a, threads=threads) for w in waves]
