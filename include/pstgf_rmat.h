@@ -1,0 +1,159 @@
+/*
+ * pstgf_rmat.h -- C ABI of libpstgf_rmat.so: R-matrix formation on one B200 (sm_100a).
+ *
+ * The operation is eq. 4 of arxiv 1909.07321 (section 3):
+ *
+ *     R_nm(E) = 1/(2 r0) * sum_{k=1..M} w_nk w_mk / (E_k - E)
+ *
+ * evaluated for every energy E of a mesh and every partial wave, i.e. the
+ * batched energy-scaled symmetric contraction
+ * R(E) = (1/2a) W diag(1/(E_k - E)) W^T (PSTGF's subroutine RINIT,
+ * PAPER.md:168).  a == r0 is the R-matrix radius (record RA),
+ * W the surface amplitudes w_nk (record WMAT), E_k the R-matrix
+ * poles (record VALUE), one (W, E_k) pair per partial wave with
+ * its own NCHAN and MNP2.
+ *
+ * All arithmetic is IEEE FP64.  There is no CPU fallback and no other device
+ * path: every call either enqueues sm_100a kernels or returns an error.
+ *
+ * Conventions for every call
+ *  - Pointers named in "DEVICE" lists are device pointers owned by the caller
+ *    (allocate them with any CUDA allocator, e.g. PyTorch).  The library
+ *    allocates no device memory in the DEVICE-pointer calls; the batch call
+ *    keeps its tables in the caller's workspace.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default
+ *    stream).  DEVICE-pointer calls enqueue work and return without
+ *    synchronising; buffers must stay alive until the stream reaches the end
+ *    of the enqueued work.  Host structs (pstgf_wave_t arrays) are consumed
+ *    before the call returns.
+ *  - Layout: W is row-major [n_chan][ldw], element (n,k) at W[n*ldw + k],
+ *    ldw >= n_poles (k contiguous).  R_out is dense row-major
+ *    [n_E][n_chan][n_chan]; BOTH triangles are written and R_out[e][n][m] ==
+ *    R_out[e][m][n] bitwise.  R_out must not overlap any input or another
+ *    wave's R_out.  Inputs may be shared between waves.
+ *  - Sizes: n_E == 0, n_chan == 0 or n_waves == 0 -> PSTGF_OK, nothing
+ *    written.  n_poles == 0 -> R_out is zero-filled (empty sum).
+ *  - An energy equal to a pole is not detected (data lives on the device):
+ *    IEEE semantics apply (inf/NaN in that energy's R).  The paper is silent;
+ *    callers keep a clearance (the synthetic workloads use 1e-3 Ryd).
+ *  - Alignment: every pointer must be 8-byte aligned (else
+ *    PSTGF_ERR_ALIGNMENT).  W 16-byte aligned with even ldw selects the TMA
+ *    staging path; otherwise a slower load path inside the same kernel is
+ *    used.  Any n_chan (odd included) is supported.
+ *  - Results are deterministic: each R element is produced by exactly one
+ *    thread with a fixed k order, whatever CTA picked the work item up.
+ *  - Errors are returned as pstgf_status_t; nothing is thrown or printed.
+ *    Argument errors are detected before anything is enqueued.
+ */
+#ifndef PSTGF_RMAT_H
+#define PSTGF_RMAT_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PSTGF_RMAT_VERSION 100 /* major*100 + minor */
+
+typedef enum {
+  PSTGF_OK = 0,
+  PSTGF_ERR_INVALID_VALUE = 1,      /* NULL where data is required, negative size, ldw < n_poles, a not finite or <= 0 */
+  PSTGF_ERR_ALIGNMENT = 2,          /* a pointer is not 8-byte aligned */
+  PSTGF_ERR_WORKSPACE = 3,          /* workspace NULL, not 256-byte aligned, or smaller than the query says */
+  PSTGF_ERR_UNSUPPORTED_DEVICE = 4, /* no CUDA device, or the current device is not compute capability 10.x */
+  PSTGF_ERR_CUDA = 5                /* a CUDA runtime/driver call failed; see pstgf_last_cuda_error() */
+} pstgf_status_t;
+
+/*
+ * One partial wave of a ragged batch: a HOST struct holding DEVICE pointers
+ * (or HOST pointers for pstgf_rmat_form_batch_host).  Field meanings as in
+ * pstgf_rmat_form.
+ */
+typedef struct {
+  int n_chan;             /* NCHAN */
+  int n_poles;            /* MNP2, */
+  int n_E;                /* energies of this wave's mesh */
+  long long ldw;          /* leading dimension of W in elements, >= n_poles */
+  double a;               /* RA, a.u., > 0 */
+  const double *W;        /* [n_chan][ldw] */
+  const double *E_k;      /* [n_poles] */
+  const double *energies; /* [n_E] */
+  double *R_out;          /* [n_E][n_chan][n_chan] */
+} pstgf_wave_t;
+
+/*
+ * Eq. 4 for one partial wave at n_E energies.
+ * DEVICE: W, E_k, energies, R_out.
+ *   W        [n_chan][ldw]   surface amplitudes w_nk
+ *   E_k      [n_poles]       poles, Ryd, any order
+ *   energies [n_E]           energies, same units and origin as E_k
+ *   a                        R-matrix radius r0 in a.u., finite and > 0
+ *   R_out    [n_E][n_chan][n_chan]
+ * One persistent kernel launch (plus a zero-fill when n_poles == 0); work
+ * items (energy block, upper-triangle tile) are assigned to CTAs round-robin.
+ */
+pstgf_status_t pstgf_rmat_form(const double *W, long long ldw, const double *E_k,
+                               const double *energies, int n_chan, int n_poles, int n_E,
+                               double a, double *R_out, void *stream);
+
+/*
+ * Bytes of device workspace pstgf_rmat_form_batch needs for these waves
+ * (only n_waves matters today; the waves are passed for future layouts).
+ * Returns 0 for n_waves <= 0.
+ */
+size_t pstgf_rmat_batch_workspace_bytes(const pstgf_wave_t *waves, int n_waves);
+
+/*
+ * Eq. 4 for every wave of a ragged batch in ONE persistent kernel launch.
+ * `waves` is a HOST array of n_waves structs with DEVICE pointers.
+ * `workspace` is DEVICE memory, 256-byte aligned, at least
+ * pstgf_rmat_batch_workspace_bytes() long; it holds the wave table (with one
+ * TMA descriptor per wave), the item-range table and the work counter, and
+ * may be reused by the next call on the same stream.  Work items (wave,
+ * energy block, tile), waves ordered by decreasing cost, are handed to CTAs
+ * through an atomic counter: the counterpart of the paper's energy-permuting
+ * distribution over MPI ranks (Fig. 1).
+ */
+pstgf_status_t pstgf_rmat_form_batch(const pstgf_wave_t *waves, int n_waves, void *workspace,
+                                     size_t workspace_bytes, void *stream);
+
+/*
+ * The same result as pstgf_rmat_form from a one-thread-per-element kernel
+ * that follows eq. 4 term by term ((w_n*w_m)/(E_k-E), k ascending,
+ * compensated sum).  Slow; provided so that callers and tests can check every
+ * energy of a large run against an independent device evaluation.
+ * DEVICE: W, E_k, energies, R_out.
+ */
+pstgf_status_t pstgf_rmat_form_naive(const double *W, long long ldw, const double *E_k,
+                                     const double *energies, int n_chan, int n_poles, int n_E,
+                                     double a, double *R_out, void *stream);
+
+/*
+ * End-to-end convenience over HOST buffers: `waves` holds HOST pointers
+ * (pinned memory recommended).  Inputs are copied to the device, R is formed
+ * in chunks of energies and copied back into the host R_out while the next
+ * chunk is computed.  Allocates device memory from the stream-ordered pool of
+ * the current device for the duration of the call and SYNCHRONISES before
+ * returning.  `max_chunk_bytes` bounds the device R staging per chunk
+ * (0 = default 256 MiB; two chunks are in flight).
+ */
+pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves,
+                                          size_t max_chunk_bytes, void *stream);
+
+/* Kernel launches enqueued by this thread's last successful call (for accounting). */
+int pstgf_last_launch_count(void);
+
+/* Static description of a status code (never NULL). */
+const char *pstgf_status_string(pstgf_status_t status);
+
+/* cudaError_t (as int) behind this thread's last PSTGF_ERR_CUDA, else 0. */
+int pstgf_last_cuda_error(void);
+
+/* PSTGF_RMAT_VERSION of the loaded library. */
+int pstgf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PSTGF_RMAT_H */

@@ -1,0 +1,428 @@
+// pstgf_rmat.cu -- C ABI of libpstgf_rmat.so (include/pstgf_rmat.h): argument checks, the host
+// planner (tile / item tables, TMA descriptors) and the launches of the sm_100a kernel in
+// rmat_kernel.cuh.  Eq. 4 of arxiv 1909.07321.
+#include <cuda_runtime.h>
+#include <cuda.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <mutex>
+#include <numeric>
+#include <vector>
+
+#include "../../include/pstgf_rmat.h"
+#include "rmat_kernel.cuh"
+
+namespace {
+
+using pstgf::DevWave;
+
+thread_local int tl_cuda_error = 0;
+thread_local int tl_launches = 0;
+
+pstgf_status_t cuda_fail(cudaError_t e) {
+  tl_cuda_error = (int)e;
+  (void)cudaGetLastError();
+  return PSTGF_ERR_CUDA;
+}
+#define PSTGF_CUDA(expr)                                  \
+  do {                                                    \
+    cudaError_t e_ = (expr);                              \
+    if (e_ != cudaSuccess) return cuda_fail(e_);          \
+  } while (0)
+
+// ---- device / driver state -----------------------------------------------------------------
+typedef CUresult (*encode_tiled_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                    const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+struct DeviceState {
+  int device = -1;
+  int sm_count = 0;
+  bool ok = false;
+};
+
+encode_tiled_fn g_encode = nullptr;
+std::once_flag g_encode_once;
+std::mutex g_attr_mutex;
+bool g_attr_set[64] = {false};
+
+pstgf_status_t device_state(DeviceState &ds) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) {
+    tl_cuda_error = (int)e;
+    (void)cudaGetLastError();
+    return PSTGF_ERR_UNSUPPORTED_DEVICE;
+  }
+  int major = 0, sms = 0;
+  PSTGF_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+  PSTGF_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  if (major != 10) return PSTGF_ERR_UNSUPPORTED_DEVICE;
+  std::call_once(g_encode_once, [] {
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      g_encode = reinterpret_cast<encode_tiled_fn>(fn);
+  });
+  if (!g_encode) return PSTGF_ERR_UNSUPPORTED_DEVICE;
+  {
+    std::lock_guard<std::mutex> lock(g_attr_mutex);
+    if (dev < 64 && !g_attr_set[dev]) {
+      PSTGF_CUDA(cudaFuncSetAttribute(pstgf::rmat_persistent_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      pstgf::SMEM_BYTES));
+      PSTGF_CUDA(cudaFuncSetAttribute(pstgf::rmat_persistent_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      pstgf::SMEM_BYTES));
+      g_attr_set[dev] = true;
+    }
+  }
+  ds.device = dev;
+  ds.sm_count = sms;
+  ds.ok = true;
+  return PSTGF_OK;
+}
+
+// ---- argument checks -----------------------------------------------------------------------
+bool aligned8(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 7u) == 0; }
+
+pstgf_status_t check_wave(const pstgf_wave_t &w) {
+  if (w.n_chan < 0 || w.n_poles < 0 || w.n_E < 0) return PSTGF_ERR_INVALID_VALUE;
+  if (!(w.a > 0.0) || !std::isfinite(w.a)) return PSTGF_ERR_INVALID_VALUE;
+  if (w.n_chan == 0 || w.n_E == 0) return PSTGF_OK;       // nothing to read or write
+  if (!w.energies || !w.R_out) return PSTGF_ERR_INVALID_VALUE;
+  if (w.n_poles > 0 && (!w.W || !w.E_k || w.ldw < w.n_poles)) return PSTGF_ERR_INVALID_VALUE;
+  if (!aligned8(w.W) || !aligned8(w.E_k) || !aligned8(w.energies) || !aligned8(w.R_out)) return PSTGF_ERR_ALIGNMENT;
+  return PSTGF_OK;
+}
+
+// ---- planner -------------------------------------------------------------------------------
+// Fills everything of DevWave except the tensor map.
+void plan_wave(const pstgf_wave_t &w, DevWave &d) {
+  std::memset(&d, 0, sizeof(d));
+  d.W = w.W;
+  d.E_k = w.E_k;
+  d.energies = w.energies;
+  d.R_out = w.R_out;
+  d.ldw = w.ldw;
+  d.inv2a = 1.0 / (2.0 * w.a);
+  d.n_chan = w.n_chan;
+  d.n_poles = w.n_poles;
+  d.n_E = w.n_E;
+  d.n_kt = (w.n_poles + pstgf::KT - 1) / pstgf::KT;
+  d.n_i = (w.n_chan + pstgf::TM - 1) / pstgf::TM;
+  d.n_j = (w.n_chan + pstgf::TN - 1) / pstgf::TN;
+  d.n_eb = (w.n_E + pstgf::EB - 1) / pstgf::EB;
+  int tiles = d.n_i;
+  for (int i = 0; i < d.n_i; ++i) tiles += pstgf::off_tiles_in_row(d.n_j, i);
+  d.n_tiles = tiles;
+  d.use_tma = ((reinterpret_cast<uintptr_t>(w.W) & 15u) == 0 && (w.ldw % 2) == 0 && w.ldw * 8 < (1LL << 40)) ? 1 : 0;
+}
+
+long long wave_items(const DevWave &d) { return (long long)d.n_tiles * d.n_eb; }
+
+// Relative cost of a wave's items, for the largest-first order of the batch.
+double wave_item_cost(const pstgf_wave_t &w) { return (double)std::min(w.n_chan, pstgf::TM) * w.n_poles; }
+
+pstgf_status_t encode_map(DevWave &d) {
+  if (!d.use_tma) return PSTGF_OK;
+  cuuint64_t dims[2] = {(cuuint64_t)d.n_poles, (cuuint64_t)d.n_chan};
+  cuuint64_t strides[1] = {(cuuint64_t)d.ldw * 8};
+  cuuint32_t box[2] = {(cuuint32_t)pstgf::KT, (cuuint32_t)pstgf::TN};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = g_encode(&d.map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double *>(d.W), dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    d.use_tma = 0;   // shapes the encoder refuses fall back to the plain staging path
+  }
+  return PSTGF_OK;
+}
+
+// A wave with work for the contraction kernel (n_poles == 0 is a zero-fill instead).
+bool wave_has_items(const pstgf_wave_t &w) { return w.n_chan > 0 && w.n_E > 0 && w.n_poles > 0; }
+
+pstgf_status_t zero_fill(const pstgf_wave_t &w, cudaStream_t s) {
+  if (w.n_chan > 0 && w.n_E > 0 && w.n_poles == 0) {
+    PSTGF_CUDA(cudaMemsetAsync(w.R_out, 0, sizeof(double) * (size_t)w.n_E * w.n_chan * w.n_chan, s));
+    ++tl_launches;
+  }
+  return PSTGF_OK;
+}
+
+// workspace layout of the batch call
+constexpr size_t WS_COUNTER_BYTES = 256;
+size_t ws_item_begin_bytes(int n_waves) { return (((size_t)n_waves + 1) * sizeof(long long) + 255) & ~(size_t)255; }
+size_t ws_bytes(int n_waves) { return WS_COUNTER_BYTES + ws_item_begin_bytes(n_waves) + (size_t)n_waves * sizeof(DevWave); }
+
+}  // namespace
+
+extern "C" {
+
+pstgf_status_t pstgf_rmat_form(const double *W, long long ldw, const double *E_k, const double *energies, int n_chan,
+                               int n_poles, int n_E, double a, double *R_out, void *stream) {
+  tl_launches = 0;
+  pstgf_wave_t w{n_chan, n_poles, n_E, ldw, a, W, E_k, energies, R_out};
+  pstgf_status_t st = check_wave(w);
+  if (st != PSTGF_OK) return st;
+  if (n_chan == 0 || n_E == 0) return PSTGF_OK;
+  DeviceState ds;
+  st = device_state(ds);
+  if (st != PSTGF_OK) return st;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  if (n_poles == 0) return zero_fill(w, s);
+  DevWave d;
+  plan_wave(w, d);
+  st = encode_map(d);
+  if (st != PSTGF_OK) return st;
+  const long long n_items = wave_items(d);
+  const int grid = (int)std::min<long long>(ds.sm_count, n_items);
+  pstgf::rmat_persistent_kernel<false><<<grid, pstgf::NUM_THREADS, pstgf::SMEM_BYTES, s>>>(d, nullptr, nullptr, 1,
+                                                                                         n_items, nullptr);
+  PSTGF_CUDA(cudaGetLastError());
+  tl_launches = 1;
+  return PSTGF_OK;
+}
+
+size_t pstgf_rmat_batch_workspace_bytes(const pstgf_wave_t *waves, int n_waves) {
+  (void)waves;
+  return n_waves > 0 ? ws_bytes(n_waves) : 0;
+}
+
+pstgf_status_t pstgf_rmat_form_batch(const pstgf_wave_t *waves, int n_waves, void *workspace, size_t workspace_bytes,
+                                     void *stream) {
+  tl_launches = 0;
+  if (n_waves < 0) return PSTGF_ERR_INVALID_VALUE;
+  if (n_waves == 0) return PSTGF_OK;
+  if (!waves) return PSTGF_ERR_INVALID_VALUE;
+  for (int p = 0; p < n_waves; ++p) {
+    pstgf_status_t st = check_wave(waves[p]);
+    if (st != PSTGF_OK) return st;
+  }
+  if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) != 0 || workspace_bytes < ws_bytes(n_waves))
+    return PSTGF_ERR_WORKSPACE;
+  DeviceState ds;
+  pstgf_status_t st = device_state(ds);
+  if (st != PSTGF_OK) return st;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  int launches = 0;
+  // waves with work, most expensive items first (largest-first list scheduling)
+  std::vector<int> order;
+  for (int p = 0; p < n_waves; ++p) {
+    if (wave_has_items(waves[p])) order.push_back(p);
+    else {
+      st = zero_fill(waves[p], s);
+      if (st != PSTGF_OK) return st;
+    }
+  }
+  launches = tl_launches;
+  if (order.empty()) return PSTGF_OK;
+  std::stable_sort(order.begin(), order.end(),
+                   [&](int x, int y) { return wave_item_cost(waves[x]) > wave_item_cost(waves[y]); });
+  const int nw = (int)order.size();
+  // host image of the workspace: [counter | item_begin[nw+1] | DevWave[nw]]
+  const size_t off_begin = WS_COUNTER_BYTES, off_waves = WS_COUNTER_BYTES + ws_item_begin_bytes(n_waves);
+  std::vector<unsigned char> img(off_waves + (size_t)nw * sizeof(DevWave), 0);
+  long long *item_begin = reinterpret_cast<long long *>(img.data() + off_begin);
+  long long total = 0;
+  for (int q = 0; q < nw; ++q) {
+    DevWave d;
+    plan_wave(waves[order[q]], d);
+    st = encode_map(d);
+    if (st != PSTGF_OK) return st;
+    std::memcpy(img.data() + off_waves + (size_t)q * sizeof(DevWave), &d, sizeof(DevWave));
+    item_begin[q] = total;
+    total += wave_items(d);
+  }
+  item_begin[nw] = total;
+  unsigned char *ws = static_cast<unsigned char *>(workspace);
+  PSTGF_CUDA(cudaMemcpyAsync(ws, img.data(), img.size(), cudaMemcpyHostToDevice, s));
+  const int grid = (int)std::min<long long>(ds.sm_count, total);
+  DevWave dummy;
+  std::memset(&dummy, 0, sizeof(dummy));
+  pstgf::rmat_persistent_kernel<true><<<grid, pstgf::NUM_THREADS, pstgf::SMEM_BYTES, s>>>(
+      dummy, reinterpret_cast<const DevWave *>(ws + off_waves), reinterpret_cast<const long long *>(ws + off_begin), nw,
+      total, reinterpret_cast<unsigned long long *>(ws));
+  PSTGF_CUDA(cudaGetLastError());
+  tl_launches = launches + 1;
+  return PSTGF_OK;
+}
+
+pstgf_status_t pstgf_rmat_form_naive(const double *W, long long ldw, const double *E_k, const double *energies,
+                                     int n_chan, int n_poles, int n_E, double a, double *R_out, void *stream) {
+  tl_launches = 0;
+  pstgf_wave_t w{n_chan, n_poles, n_E, ldw, a, W, E_k, energies, R_out};
+  pstgf_status_t st = check_wave(w);
+  if (st != PSTGF_OK) return st;
+  if (n_chan == 0 || n_E == 0) return PSTGF_OK;
+  DeviceState ds;
+  st = device_state(ds);
+  if (st != PSTGF_OK) return st;
+  const long long n_elems = (long long)n_E * n_chan * n_chan;
+  const int threads = 128;
+  const long long blocks = (n_elems + threads - 1) / threads;
+  if (blocks > 0x7fffffffLL) return PSTGF_ERR_INVALID_VALUE;
+  pstgf::rmat_naive_kernel<<<(unsigned)blocks, threads, 0, static_cast<cudaStream_t>(stream)>>>(
+      W, ldw, E_k, energies, n_chan, n_poles, n_elems, a, R_out);
+  PSTGF_CUDA(cudaGetLastError());
+  tl_launches = 1;
+  return PSTGF_OK;
+}
+
+// ---- end-to-end call over HOST buffers ---------------------------------------------------------
+namespace {
+struct HostCallResources {
+  cudaStream_t s = nullptr, copy = nullptr;
+  cudaEvent_t computed[2] = {nullptr, nullptr}, copied[2] = {nullptr, nullptr};
+  std::vector<void *> allocs;
+  ~HostCallResources() {
+    if (copy) cudaStreamSynchronize(copy);
+    cudaStreamSynchronize(s);
+    for (void *p : allocs) cudaFreeAsync(p, s);
+    cudaStreamSynchronize(s);
+    for (int b = 0; b < 2; ++b) {
+      if (computed[b]) cudaEventDestroy(computed[b]);
+      if (copied[b]) cudaEventDestroy(copied[b]);
+    }
+    if (copy) cudaStreamDestroy(copy);
+  }
+};
+struct Segment { int wave, e0, ne; size_t off; };
+}  // namespace
+
+pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves, size_t max_chunk_bytes, void *stream) {
+  tl_launches = 0;
+  if (n_waves < 0) return PSTGF_ERR_INVALID_VALUE;
+  if (n_waves == 0) return PSTGF_OK;
+  if (!waves) return PSTGF_ERR_INVALID_VALUE;
+  for (int p = 0; p < n_waves; ++p) {
+    pstgf_status_t st = check_wave(waves[p]);
+    if (st != PSTGF_OK) return st;
+  }
+  DeviceState ds;
+  pstgf_status_t st = device_state(ds);
+  if (st != PSTGF_OK) return st;
+  const size_t cap = max_chunk_bytes ? max_chunk_bytes : ((size_t)256 << 20);
+  HostCallResources res;
+  res.s = static_cast<cudaStream_t>(stream);
+  PSTGF_CUDA(cudaStreamCreateWithFlags(&res.copy, cudaStreamNonBlocking));
+  for (int b = 0; b < 2; ++b) {
+    PSTGF_CUDA(cudaEventCreateWithFlags(&res.computed[b], cudaEventDisableTiming));
+    PSTGF_CUDA(cudaEventCreateWithFlags(&res.copied[b], cudaEventDisableTiming));
+  }
+  auto dev_alloc = [&](size_t bytes, void **out) -> cudaError_t {
+    cudaError_t e = cudaMallocAsync(out, bytes ? bytes : 8, res.s);
+    if (e == cudaSuccess) res.allocs.push_back(*out);
+    return e;
+  };
+  // inputs: W re-pitched to an even leading dimension so that the TMA staging path applies
+  std::vector<pstgf_wave_t> dev(waves, waves + n_waves);
+  for (int p = 0; p < n_waves; ++p) {
+    const pstgf_wave_t &w = waves[p];
+    if (w.n_chan == 0 || w.n_E == 0) continue;
+    if (w.n_poles == 0) {
+      std::memset(w.R_out, 0, sizeof(double) * (size_t)w.n_E * w.n_chan * w.n_chan);
+      continue;
+    }
+    const long long pitch = ((long long)w.n_poles + 1) & ~1LL;
+    void *dW, *dEk, *dEn;
+    PSTGF_CUDA(dev_alloc(sizeof(double) * (size_t)pitch * w.n_chan, &dW));
+    PSTGF_CUDA(dev_alloc(sizeof(double) * (size_t)w.n_poles, &dEk));
+    PSTGF_CUDA(dev_alloc(sizeof(double) * (size_t)w.n_E, &dEn));
+    PSTGF_CUDA(cudaMemcpy2DAsync(dW, pitch * 8, w.W, w.ldw * 8, (size_t)w.n_poles * 8, w.n_chan, cudaMemcpyHostToDevice, res.s));
+    PSTGF_CUDA(cudaMemcpyAsync(dEk, w.E_k, sizeof(double) * (size_t)w.n_poles, cudaMemcpyHostToDevice, res.s));
+    PSTGF_CUDA(cudaMemcpyAsync(dEn, w.energies, sizeof(double) * (size_t)w.n_E, cudaMemcpyHostToDevice, res.s));
+    dev[p].W = static_cast<double *>(dW);
+    dev[p].ldw = pitch;
+    dev[p].E_k = static_cast<double *>(dEk);
+    dev[p].energies = static_cast<double *>(dEn);
+  }
+  // chunks of (wave, energy range) segments, each at most `cap` bytes of R (at least one energy block)
+  std::vector<std::vector<Segment>> chunks;
+  size_t max_chunk = 0, cur = 0;
+  size_t max_segs = 1;
+  chunks.emplace_back();
+  for (int p = 0; p < n_waves; ++p) {
+    const pstgf_wave_t &w = waves[p];
+    if (!wave_has_items(w)) continue;
+    const size_t per_e = sizeof(double) * (size_t)w.n_chan * w.n_chan;
+    int e0 = 0;
+    while (e0 < w.n_E) {
+      size_t room = cap > cur ? cap - cur : 0;
+      int ne = (int)std::min<size_t>((size_t)(w.n_E - e0), room / per_e);
+      if (ne < w.n_E - e0) ne -= ne % pstgf::EB;      // split only at energy-block boundaries
+      if (ne <= 0) {
+        if (cur > 0) {                               // close the chunk and retry in an empty one
+          chunks.emplace_back();
+          cur = 0;
+          continue;
+        }
+        ne = std::min(pstgf::EB, w.n_E - e0);          // one block does not fit the cap: take it anyway
+      }
+      chunks.back().push_back(Segment{p, e0, ne, cur});
+      cur += per_e * (size_t)ne;
+      max_chunk = std::max(max_chunk, cur);
+      max_segs = std::max(max_segs, chunks.back().size());
+      e0 += ne;
+    }
+  }
+  if (chunks.back().empty()) chunks.pop_back();
+  if (chunks.empty()) return PSTGF_OK;
+  void *rbuf[2], *wsbuf[2];
+  const size_t wsb = ws_bytes((int)max_segs);
+  for (int b = 0; b < 2; ++b) {
+    PSTGF_CUDA(dev_alloc(max_chunk, &rbuf[b]));
+    PSTGF_CUDA(dev_alloc(wsb, &wsbuf[b]));
+  }
+  int launches = 0;
+  std::vector<pstgf_wave_t> sub;
+  for (size_t c = 0; c < chunks.size(); ++c) {
+    const int b = (int)(c & 1);
+    if (c >= 2) PSTGF_CUDA(cudaStreamWaitEvent(res.s, res.copied[b], 0));
+    sub.clear();
+    for (const Segment &g : chunks[c]) {
+      pstgf_wave_t w = dev[g.wave];
+      w.energies = dev[g.wave].energies + g.e0;
+      w.n_E = g.ne;
+      w.R_out = reinterpret_cast<double *>(static_cast<unsigned char *>(rbuf[b]) + g.off);
+      sub.push_back(w);
+    }
+    st = pstgf_rmat_form_batch(sub.data(), (int)sub.size(), wsbuf[b], wsb, res.s);
+    if (st != PSTGF_OK) return st;
+    launches += tl_launches;
+    PSTGF_CUDA(cudaEventRecord(res.computed[b], res.s));
+    PSTGF_CUDA(cudaStreamWaitEvent(res.copy, res.computed[b], 0));
+    for (const Segment &g : chunks[c]) {
+      const pstgf_wave_t &w = waves[g.wave];
+      const size_t per_e = sizeof(double) * (size_t)w.n_chan * w.n_chan;
+      PSTGF_CUDA(cudaMemcpyAsync(w.R_out + (size_t)g.e0 * w.n_chan * w.n_chan, static_cast<unsigned char *>(rbuf[b]) + g.off,
+                                 per_e * (size_t)g.ne, cudaMemcpyDeviceToHost, res.copy));
+    }
+    PSTGF_CUDA(cudaEventRecord(res.copied[b], res.copy));
+  }
+  PSTGF_CUDA(cudaStreamSynchronize(res.copy));
+  PSTGF_CUDA(cudaStreamSynchronize(res.s));
+  tl_launches = launches;
+  return PSTGF_OK;
+}
+
+int pstgf_last_launch_count(void) { return tl_launches; }
+
+const char *pstgf_status_string(pstgf_status_t status) {
+  switch (status) {
+    case PSTGF_OK: return "PSTGF_OK";
+    case PSTGF_ERR_INVALID_VALUE: return "PSTGF_ERR_INVALID_VALUE: null pointer, negative size, ldw < n_poles, or a not finite and > 0";
+    case PSTGF_ERR_ALIGNMENT: return "PSTGF_ERR_ALIGNMENT: a pointer is not 8-byte aligned";
+    case PSTGF_ERR_WORKSPACE: return "PSTGF_ERR_WORKSPACE: workspace null, not 256-byte aligned, or too small";
+    case PSTGF_ERR_UNSUPPORTED_DEVICE: return "PSTGF_ERR_UNSUPPORTED_DEVICE: needs a CUDA device of compute capability 10.x";
+    case PSTGF_ERR_CUDA: return "PSTGF_ERR_CUDA: a CUDA call failed, see pstgf_last_cuda_error()";
+  }
+  return "unknown pstgf_status_t";
+}
+
+int pstgf_last_cuda_error(void) { return tl_cuda_error; }
+
+int pstgf_version(void) { return PSTGF_RMAT_VERSION; }
+
+}  // extern "C"

@@ -1,0 +1,64 @@
+// rmat_common.h -- tile constants and the device-visible tables shared by the host planner
+// and the sm_100a kernel of libpstgf_rmat.so.  (Not shared with oracle/: that is a separate
+// C translation unit with no includes from here.)
+//
+// Work decomposition of eq. 4 for one partial wave with C = n_chan,
+// K = n_poles, N = n_E:
+//   tile kinds   DIAG(i)    rows/cols [64 i, 64 i + 64): upper triangle of 8x8 DMMA blocks
+//                OFF(i, j)  rows [64 i, 64 i + 64) x cols [32 j, 32 j + 32), j >= 2 i + 2
+//   energy block EB = 8 consecutive energies, one per consumer warp
+//   item         (wave, tile, energy block); item index inside a wave = tile * n_eb + eb
+//                (energy-fastest: CTAs running side by side share one W tile in L2)
+// Only tiles on or above the diagonal exist ("half of the symmetric R-matrix"),
+// the mirror is written by the epilogue ("symmetrised").
+#pragma once
+#include <cuda.h>
+#include <stdint.h>
+
+namespace pstgf {
+
+constexpr int TM = 64;      // tile rows: I panel
+constexpr int TN = 32;      // OFF tile columns: J panel; also the TMA box height
+constexpr int KT = 20;      // poles per pipeline stage; row pitch 20 doubles == 4 (mod 16) -> conflict-free LDS.64
+constexpr int EB = 8;       // energies per item == consumer warps per CTA
+constexpr int STAGES = 8;   // smem ring depth
+constexpr int NUM_THREADS = (EB + 4) * 32;           // 8 consumer warps + the producer warpgroup (1 of its 4 warps works)
+constexpr int PRODUCER_REGS = 56;                    // setmaxnreg targets: 8*224 + 4*56 = 12*168, the launch allocation
+constexpr int CONSUMER_REGS = 224;
+constexpr int BOX_BYTES = TN * KT * 8;               // one TMA box: 32 rows x 20 poles
+constexpr int WI_BYTES = TM * KT * 8;                // two boxes
+constexpr int WJ_BYTES = TN * KT * 8;
+constexpr int D_BYTES = EB * KT * 8;                 // d_e[k] = 1/(E_k - E_e) for the stage
+constexpr int STAGE_BYTES = WI_BYTES + WJ_BYTES + D_BYTES;   // 16640
+constexpr int SMEM_BARRIER_OFFSET = STAGES * STAGE_BYTES;
+constexpr int SMEM_ITEM_OFFSET = SMEM_BARRIER_OFFSET + (2 * STAGES + 4) * 8;
+constexpr int SMEM_BYTES = SMEM_ITEM_OFFSET + 2 * 64 + 128;  // + alignment slack
+
+// One partial wave as the kernel sees it.  Built on the host, lives in kernel parameter
+// space (single-wave call) or in the caller's workspace (batch call).
+struct alignas(128) DevWave {
+  CUtensorMap map;         // W viewed as [n_chan][n_poles] (row stride ldw*8), box [TN][KT], no swizzle
+  const double *W;
+  const double *E_k;
+  const double *energies;
+  double *R_out;
+  long long ldw;
+  double inv2a;            // 1/(2a), PAPER.md:108 prefactor
+  int n_chan, n_poles, n_E;
+  int n_kt;                // ceil(n_poles / KT)
+  int n_i;                 // ceil(n_chan / TM): DIAG tiles
+  int n_j;                 // ceil(n_chan / TN)
+  int n_eb;                // ceil(n_E / EB)
+  int n_tiles;             // n_i + number of OFF tiles
+  int use_tma;             // W 16-byte aligned and ldw even
+  int pad_;
+};
+static_assert(sizeof(DevWave) == 256, "DevWave layout");
+
+// Host-side tile arithmetic (also used by the kernel's decoder).
+__host__ __device__ inline int off_tiles_in_row(int n_j, int i) {
+  int c = n_j - (2 * i + 2);
+  return c > 0 ? c : 0;
+}
+
+}  // namespace pstgf

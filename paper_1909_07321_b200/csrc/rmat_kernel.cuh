@@ -1,0 +1,420 @@
+// rmat_kernel.cuh -- the persistent sm_100a kernel behind pstgf_rmat_form / pstgf_rmat_form_batch.
+//
+// One CTA per SM, 12 warps.  Warps 8..11 are the producer warpgroup: they hand most of their
+// registers to the consumers (setmaxnreg) and only warp 8 works: it takes work items (atomic counter in the
+// batch call, round-robin in the single-wave call), issues the TMA loads of the W panels and
+// builds the pole scaling d_e[k] = 1/(E_k - E_e) of the stage in shared memory (SURVEY 8a-S1,
+// S2; the denominator of eq. 4).  Warps 0..7 are consumers, one energy of the
+// item's block each: they contract acc[n][m] += W[n][k] * (W[m][k] * d_e[k]) on the FP64 tensor
+// pipe (mma.sync m8n8k4 -> DMMA.8x8x4) over upper-triangle tiles only (S3) and
+// write R and its mirror scaled by 1/(2a) (S4).  Producer and consumers are
+// coupled by an mbarrier full/empty ring that runs on across item boundaries, so the next
+// item's first stages land while the epilogue of the current one is being stored.
+#pragma once
+#include "rmat_common.h"
+
+namespace pstgf {
+
+struct ItemInfo {        // handed from the producer to the consumers through smem
+  double *R;             // R_out of the block's first energy
+  double inv2a;
+  int n_chan;
+  int n_valid_e;         // energies in this block (1..EB)
+  int row0, col0;
+  int kind;              // 0 DIAG, 1 OFF, -1 stop
+  int nblk;              // DIAG: valid 8x8 block rows/cols; OFF: valid 8-wide column blocks
+  int n_kt;
+  int pad_;
+};
+static_assert(sizeof(ItemInfo) <= 64, "ItemInfo slot");
+
+// ---- PTX wrappers ------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) {
+  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "MBAR_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra MBAR_DONE;\n"
+      "bra MBAR_WAIT;\n"
+      "MBAR_DONE:\n"
+      "}\n" ::"r"(bar),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map, int c0, int c1, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+      ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(bar)
+      : "memory");
+}
+// D(8x8) += A(8x4) * B(4x8), FP64.  Lane l holds A[l/4][l%4], B[l%4][l/4], D[l/4][2*(l%4)+{0,1}].
+__device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+               : "+d"(c0), "+d"(c1)
+               : "d"(a), "d"(b));
+}
+
+struct PipeState {
+  uint32_t stage = 0, phase = 0;
+  __device__ __forceinline__ void advance() {
+    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+  }
+};
+
+// ---- consumers ---------------------------------------------------------------------------
+// Warps whose energy slot lies beyond n_E only keep the ring moving.
+__device__ __forceinline__ void consume_idle(int n_kt, PipeState &ps, uint32_t full0, uint32_t empty0, int lane) {
+  for (int kt = 0; kt < n_kt; ++kt) {
+    mbar_wait(full0 + 8 * ps.stage, ps.phase);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(empty0 + 8 * ps.stage);
+    ps.advance();
+  }
+}
+
+// OFF tile: 64 x 32 block strictly above the diagonal; 8 x 4 DMMA blocks, all needed
+// (column blocks >= nblk lie beyond n_chan and are skipped).
+__device__ __forceinline__ void consume_off(const ItemInfo &it, const unsigned char *smem, PipeState &ps,
+                                            uint32_t full0, uint32_t empty0, int warp, int lane) {
+  double acc[8][4][2];
+#pragma unroll
+  for (int bi = 0; bi < 8; ++bi)
+#pragma unroll
+    for (int bj = 0; bj < 4; ++bj) acc[bi][bj][0] = acc[bi][bj][1] = 0.0;
+  const int g = lane >> 2, q = lane & 3;
+  const int ncb = it.nblk;
+  for (int kt = 0; kt < it.n_kt; ++kt) {
+    mbar_wait(full0 + 8 * ps.stage, ps.phase);
+    const double *wi = reinterpret_cast<const double *>(smem + ps.stage * STAGE_BYTES) + g * KT + q;
+    const double *wj = wi + TM * KT;
+    const double *dd = reinterpret_cast<const double *>(smem + ps.stage * STAGE_BYTES + WI_BYTES + WJ_BYTES) +
+                       warp * KT + q;
+#pragma unroll
+    for (int ks = 0; ks < KT / 4; ++ks) {
+      const double dv = dd[ks * 4];
+      double a[8];
+#pragma unroll
+      for (int bi = 0; bi < 8; ++bi) a[bi] = wi[bi * 8 * KT + ks * 4];
+#pragma unroll
+      for (int bj = 0; bj < 4; ++bj) {
+        if (bj < ncb) {
+          const double b = wj[bj * 8 * KT + ks * 4] * dv;   // pole scaling folded into the B fragment
+#pragma unroll
+          for (int bi = 0; bi < 8; ++bi) dmma884(acc[bi][bj][0], acc[bi][bj][1], a[bi], b);
+        }
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(empty0 + 8 * ps.stage);
+    ps.advance();
+  }
+  // epilogue: R[r][c] and the mirror R[c][r]; rows are always inside the matrix for OFF tiles
+  const int C = it.n_chan;
+  double *R = it.R + (size_t)warp * C * C;
+  const double s = it.inv2a;
+#pragma unroll
+  for (int bj = 0; bj < 4; ++bj) {
+    if (bj < ncb) {
+      const int c = it.col0 + bj * 8 + 2 * q;
+#pragma unroll
+      for (int bi = 0; bi < 8; ++bi) {
+        const int r = it.row0 + bi * 8 + g;
+        const double v0 = acc[bi][bj][0] * s, v1 = acc[bi][bj][1] * s;
+        if (c < C) { __stcs(R + (size_t)r * C + c, v0); __stcs(R + (size_t)c * C + r, v0); }
+        if (c + 1 < C) { __stcs(R + (size_t)r * C + c + 1, v1); __stcs(R + (size_t)(c + 1) * C + r, v1); }
+      }
+    }
+  }
+}
+
+// DIAG tile: 64 x 64 block on the diagonal; only 8x8 blocks (bi <= bj) are computed, and in
+// blocks on the diagonal only elements c >= r are stored (with their mirror), so that
+// R[n][m] == R[m][n] bitwise.
+__device__ __forceinline__ void consume_diag(const ItemInfo &it, const unsigned char *smem, PipeState &ps,
+                                             uint32_t full0, uint32_t empty0, int warp, int lane) {
+  double acc[36][2];
+#pragma unroll
+  for (int t = 0; t < 36; ++t) acc[t][0] = acc[t][1] = 0.0;
+  const int g = lane >> 2, q = lane & 3;
+  const int nb = it.nblk;
+  for (int kt = 0; kt < it.n_kt; ++kt) {
+    mbar_wait(full0 + 8 * ps.stage, ps.phase);
+    const double *wi = reinterpret_cast<const double *>(smem + ps.stage * STAGE_BYTES) + g * KT + q;
+    const double *dd = reinterpret_cast<const double *>(smem + ps.stage * STAGE_BYTES + WI_BYTES + WJ_BYTES) +
+                       warp * KT + q;
+#pragma unroll
+    for (int ks = 0; ks < KT / 4; ++ks) {
+      const double dv = dd[ks * 4];
+      double a[8];
+#pragma unroll
+      for (int bi = 0; bi < 8; ++bi) a[bi] = wi[bi * 8 * KT + ks * 4];
+#pragma unroll
+      for (int bj = 0; bj < 8; ++bj) {
+        if (bj < nb) {
+          const double b = a[bj] * dv;
+#pragma unroll
+          for (int bi = 0; bi <= bj; ++bi) dmma884(acc[bj * (bj + 1) / 2 + bi][0], acc[bj * (bj + 1) / 2 + bi][1], a[bi], b);
+        }
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(empty0 + 8 * ps.stage);
+    ps.advance();
+  }
+  const int C = it.n_chan;
+  double *R = it.R + (size_t)warp * C * C;
+  const double s = it.inv2a;
+#pragma unroll
+  for (int bj = 0; bj < 8; ++bj) {
+    if (bj < nb) {
+      const int c = it.row0 + bj * 8 + 2 * q;
+#pragma unroll
+      for (int bi = 0; bi <= bj; ++bi) {
+        const int r = it.row0 + bi * 8 + g;
+        const double v0 = acc[bj * (bj + 1) / 2 + bi][0] * s, v1 = acc[bj * (bj + 1) / 2 + bi][1] * s;
+        if (r < C) {
+          if (c < C && c >= r) {
+            __stcs(R + (size_t)r * C + c, v0);
+            if (c > r) __stcs(R + (size_t)c * C + r, v0);
+          }
+          if (c + 1 < C && c + 1 >= r) {
+            __stcs(R + (size_t)r * C + c + 1, v1);
+            if (c + 1 > r) __stcs(R + (size_t)(c + 1) * C + r, v1);
+          }
+        }
+      }
+    }
+  }
+}
+
+// ---- producer ----------------------------------------------------------------------------
+// Tile index inside a wave -> (kind, row0, col0, nblk).  DIAG tiles first (they are the most
+// expensive: 36 DMMA per k-step against 32), then OFF tiles row by row.
+__device__ __forceinline__ void decode_tile(const DevWave &w, int tile, int &kind, int &row0, int &col0, int &nblk) {
+  if (tile < w.n_i) {
+    kind = 0;
+    row0 = col0 = tile * TM;
+    const int left = w.n_chan - row0;
+    nblk = left >= TM ? TM / 8 : (left + 7) / 8;
+  } else {
+    kind = 1;
+    int t = tile - w.n_i, i = 0;
+    for (;; ++i) {
+      const int cnt = off_tiles_in_row(w.n_j, i);
+      if (t < cnt) break;
+      t -= cnt;
+    }
+    row0 = i * TM;
+    col0 = (2 * i + 2 + t) * TN;
+    const int left = w.n_chan - col0;
+    nblk = left >= TN ? TN / 8 : (left + 7) / 8;
+  }
+}
+
+// Staging without TMA (W not 16-byte aligned or ldw odd): the producer warp copies the panels
+// with plain loads, zero-filling rows >= n_chan and poles >= n_poles like the TMA path does.
+__device__ __forceinline__ void stage_panel_plain(double *dst, const DevWave &w, int row0, int rows, int k0, int lane) {
+  for (int idx = lane; idx < rows * KT; idx += 32) {
+    const int r = idx / KT, kk = idx - r * KT;
+    const int row = row0 + r, k = k0 + kk;
+    dst[idx] = (row < w.n_chan && k < w.n_poles) ? __ldg(w.W + (size_t)row * w.ldw + k) : 0.0;
+  }
+}
+
+template <bool BATCH>
+__global__ void __launch_bounds__(NUM_THREADS, 1)
+rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__restrict__ waves,
+                       const long long *__restrict__ item_begin, int n_waves, long long n_items,
+                       unsigned long long *counter) {
+  extern __shared__ unsigned char smem_raw[];
+  unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
+  const uint32_t bar0 = smem_u32(smem + SMEM_BARRIER_OFFSET);
+  const uint32_t full0 = bar0, empty0 = bar0 + 8 * STAGES;
+  const uint32_t item_full0 = bar0 + 16 * STAGES, item_empty0 = item_full0 + 16;
+  ItemInfo *ring = reinterpret_cast<ItemInfo *>(smem + SMEM_ITEM_OFFSET);   // 2 slots of 64 B
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < STAGES; ++s) {
+      mbar_init(full0 + 8 * s, 33);    // 32 producer lanes (d written) + 1 (TMA expect_tx / plain staging done)
+      mbar_init(empty0 + 8 * s, EB);   // one arrival per consumer warp
+    }
+    for (int s = 0; s < 2; ++s) {
+      mbar_init(item_full0 + 8 * s, 1);
+      mbar_init(item_empty0 + 8 * s, EB);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  if (warp >= EB) {
+    // ================= producer warpgroup: give registers away, warp EB does the work =================
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(PRODUCER_REGS));
+    if (warp != EB) return;
+    PipeState ps;
+    uint32_t iq = 0, iphase = 0;
+    long long next_static = blockIdx.x;
+    for (;;) {
+      long long item;
+      if (BATCH) {
+        unsigned long long got = 0;
+        if (lane == 0) got = atomicAdd(counter, 1ULL);
+        item = (long long)__shfl_sync(0xffffffffu, got, 0);
+      } else {
+        item = next_static;
+        next_static += gridDim.x;
+      }
+      const bool stop = item >= n_items;
+      // locate the wave (batch: binary search in the item-range table)
+      int p = 0;
+      if (BATCH && !stop) {
+        int lo = 0, hi = n_waves;            // item_begin[lo] <= item < item_begin[hi]
+        while (hi - lo > 1) {
+          const int mid = (lo + hi) >> 1;
+          if (__ldg(item_begin + mid) <= item) lo = mid; else hi = mid;
+        }
+        p = lo;
+        item -= __ldg(item_begin + p);
+      }
+      const DevWave &w = BATCH ? waves[p] : single;
+      int kind = -1, row0 = 0, col0 = 0, nblk = 0, eb = 0, n_valid = 0, n_kt = 0;
+      if (!stop) {
+        const int tile = (int)(item / w.n_eb);
+        eb = (int)(item - (long long)tile * w.n_eb);
+        decode_tile(w, tile, kind, row0, col0, nblk);
+        n_valid = min(EB, w.n_E - eb * EB);
+        n_kt = w.n_kt;
+      }
+      mbar_wait(item_empty0 + 8 * iq, iphase ^ 1u);
+      if (lane == 0) {
+        ItemInfo &ii = ring[iq];
+        ii.kind = kind;
+        if (!stop) {
+          ii.R = w.R_out + (size_t)eb * EB * w.n_chan * w.n_chan;
+          ii.inv2a = w.inv2a;
+          ii.n_chan = w.n_chan;
+          ii.n_valid_e = n_valid;
+          ii.row0 = row0;
+          ii.col0 = col0;
+          ii.nblk = nblk;
+          ii.n_kt = n_kt;
+        }
+        mbar_arrive(item_full0 + 8 * iq);   // release: the stores above are visible to waiters
+      }
+      iq ^= 1u;
+      if (iq == 0) iphase ^= 1u;
+      if (stop) break;
+
+      // per-item constants of the pole-scaling stage: lane handles entries idx = lane + 32 t of d[EB][KT]
+      constexpr int DT = EB * KT / 32;
+      static_assert(EB * KT % 32 == 0, "d tile must split evenly over the producer warp");
+      double en[DT];
+      int kk[DT];
+      bool ev[DT];
+#pragma unroll
+      for (int t = 0; t < DT; ++t) {
+        const int idx = lane + 32 * t;
+        const int e = idx / KT;
+        kk[t] = idx - e * KT;
+        ev[t] = e < n_valid;
+        en[t] = ev[t] ? __ldg(w.energies + (size_t)eb * EB + e) : 0.0;
+      }
+      double ek[DT];
+#pragma unroll
+      for (int t = 0; t < DT; ++t) ek[t] = (ev[t] && kk[t] < w.n_poles) ? __ldg(w.E_k + kk[t]) : 0.0;
+      const CUtensorMap *map = &w.map;
+      const uint32_t tx_bytes = (kind == 0 ? 2 : 3) * BOX_BYTES;
+      for (int kt = 0; kt < n_kt; ++kt) {
+        const int k0 = kt * KT;
+        // prefetch the next stage's poles before blocking on the ring
+        double ek_next[DT];
+#pragma unroll
+        for (int t = 0; t < DT; ++t) {
+          const int k = k0 + KT + kk[t];
+          ek_next[t] = (ev[t] && k < w.n_poles) ? __ldg(w.E_k + k) : 0.0;
+        }
+        mbar_wait(empty0 + 8 * ps.stage, ps.phase ^ 1u);
+        unsigned char *st = smem + ps.stage * STAGE_BYTES;
+        const uint32_t full = full0 + 8 * ps.stage;
+        if (w.use_tma) {
+          if (lane == 0) {
+            mbar_arrive_expect_tx(full, tx_bytes);
+            const uint32_t dst = smem_u32(st);
+            tma_load_2d(dst, map, k0, row0, full);
+            tma_load_2d(dst + BOX_BYTES, map, k0, row0 + TN, full);
+            if (kind != 0) tma_load_2d(dst + WI_BYTES, map, k0, col0, full);
+          }
+        } else {
+          stage_panel_plain(reinterpret_cast<double *>(st), w, row0, TM, k0, lane);
+          if (kind != 0) stage_panel_plain(reinterpret_cast<double *>(st + WI_BYTES), w, col0, TN, k0, lane);
+          __syncwarp();
+          if (lane == 0) mbar_arrive(full);
+        }
+        // S1: d_e[k] = 1/(E_k - E_e); 0 beyond n_poles / n_E so that zero-filled W columns stay zero
+        double *dsm = reinterpret_cast<double *>(st + WI_BYTES + WJ_BYTES);
+#pragma unroll
+        for (int t = 0; t < DT; ++t) {
+          const bool ok = ev[t] && (k0 + kk[t] < w.n_poles);
+          dsm[lane + 32 * t] = ok ? 1.0 / (ek[t] - en[t]) : 0.0;
+          ek[t] = ek_next[t];
+        }
+        mbar_arrive(full);
+        ps.advance();
+      }
+    }
+  } else {
+    // ================= consumer warps: one energy of the block each =================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(CONSUMER_REGS));
+    PipeState ps;
+    uint32_t iq = 0, iphase = 0;
+    for (;;) {
+      mbar_wait(item_full0 + 8 * iq, iphase);
+      const ItemInfo it = ring[iq];
+      if (it.kind < 0) break;
+      if (warp >= it.n_valid_e) consume_idle(it.n_kt, ps, full0, empty0, lane);
+      else if (it.kind == 0) consume_diag(it, smem, ps, full0, empty0, warp, lane);
+      else consume_off(it, smem, ps, full0, empty0, warp, lane);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(item_empty0 + 8 * iq);
+      iq ^= 1u;
+      if (iq == 0) iphase ^= 1u;
+    }
+  }
+}
+
+// ---- verification kernel: eq. 4 term by term, one thread per R element ----------------------
+__global__ void rmat_naive_kernel(const double *__restrict__ W, long long ldw, const double *__restrict__ E_k,
+                                  const double *__restrict__ energies, int n_chan, int n_poles, long long n_elems,
+                                  double a, double *__restrict__ R_out) {
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= n_elems) return;
+  const long long cc = (long long)n_chan * n_chan;
+  const long long e = idx / cc;
+  const int rem = (int)(idx - e * cc);
+  const int n = rem / n_chan, m = rem - n * n_chan;
+  const double E = energies[e];
+  const double *wn = W + (size_t)n * ldw, *wm = W + (size_t)m * ldw;
+  double s = 0.0, c = 0.0;
+  for (int k = 0; k < n_poles; ++k) {
+    const double t = __ddiv_rn(__dmul_rn(wn[k], wm[k]), __dsub_rn(E_k[k], E));
+    const double u = __dadd_rn(s, t);
+    c = __dadd_rn(c, fabs(s) >= fabs(t) ? __dadd_rn(__dsub_rn(s, u), t) : __dadd_rn(__dsub_rn(t, u), s));
+    s = u;
+  }
+  R_out[idx] = __ddiv_rn(__dadd_rn(s, c), __dmul_rn(2.0, a));
+}
+
+}  // namespace pstgf

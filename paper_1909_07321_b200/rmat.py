@@ -1,0 +1,192 @@
+"""Thin ctypes binding over libpstgf_rmat.so (include/pstgf_rmat.h): argument marshalling only.
+
+Every step of eq. 4 runs in the library's sm_100a kernels.  PyTorch is used for
+device memory and streams.  There is no CPU fallback: a missing library or a failing call raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Sequence
+
+import torch
+
+from . import build as _build
+
+PSTGF_OK = 0
+_STATUS_NAMES = {0: "PSTGF_OK", 1: "PSTGF_ERR_INVALID_VALUE", 2: "PSTGF_ERR_ALIGNMENT", 3: "PSTGF_ERR_WORKSPACE",
+                 4: "PSTGF_ERR_UNSUPPORTED_DEVICE", 5: "PSTGF_ERR_CUDA"}
+
+EXPORTS = ["pstgf_rmat_form", "pstgf_rmat_batch_workspace_bytes", "pstgf_rmat_form_batch", "pstgf_rmat_form_naive",
+           "pstgf_rmat_form_batch_host", "pstgf_last_launch_count", "pstgf_status_string", "pstgf_last_cuda_error",
+           "pstgf_version"]
+
+
+class PstgfError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(message)
+        self.status = status
+
+
+class pstgf_wave_t(ctypes.Structure):
+    _fields_ = [("n_chan", ctypes.c_int), ("n_poles", ctypes.c_int), ("n_E", ctypes.c_int),
+                ("ldw", ctypes.c_longlong), ("a", ctypes.c_double),
+                ("W", ctypes.c_void_p), ("E_k", ctypes.c_void_p), ("energies", ctypes.c_void_p),
+                ("R_out", ctypes.c_void_p)]
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def load(build_if_missing: bool = False):
+    """Load libpstgf_rmat.so (built in-tree).  Raises if it is not there: no fallback exists."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = library_path()
+    if not os.path.exists(path):
+        if build_if_missing:
+            _build.build()
+        else:
+            raise PstgfError(-1, f"{path} is missing: run `python -m paper_1909_07321_b200.build` "
+                                 "(or __graft_entry__.build()); there is no CPU fallback")
+    lib = ctypes.CDLL(path)
+    vp, ll, i, d, sz = ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+    lib.pstgf_rmat_form.argtypes = [vp, ll, vp, vp, i, i, i, d, vp, vp]
+    lib.pstgf_rmat_form.restype = i
+    lib.pstgf_rmat_form_naive.argtypes = [vp, ll, vp, vp, i, i, i, d, vp, vp]
+    lib.pstgf_rmat_form_naive.restype = i
+    lib.pstgf_rmat_batch_workspace_bytes.argtypes = [ctypes.POINTER(pstgf_wave_t), i]
+    lib.pstgf_rmat_batch_workspace_bytes.restype = sz
+    lib.pstgf_rmat_form_batch.argtypes = [ctypes.POINTER(pstgf_wave_t), i, vp, sz, vp]
+    lib.pstgf_rmat_form_batch.restype = i
+    lib.pstgf_rmat_form_batch_host.argtypes = [ctypes.POINTER(pstgf_wave_t), i, sz, vp]
+    lib.pstgf_rmat_form_batch_host.restype = i
+    lib.pstgf_last_launch_count.restype = i
+    lib.pstgf_status_string.argtypes = [i]
+    lib.pstgf_status_string.restype = ctypes.c_char_p
+    lib.pstgf_last_cuda_error.restype = i
+    lib.pstgf_version.restype = i
+    _lib = lib
+    return lib
+
+
+def _check(status: int):
+    if status != PSTGF_OK:
+        lib = load()
+        msg = lib.pstgf_status_string(status).decode()
+        if status == 5:
+            msg += f" (cudaError_t {lib.pstgf_last_cuda_error()})"
+        raise PstgfError(status, msg)
+
+
+def _stream_ptr(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream) if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def _dev_f64(t: torch.Tensor, name: str):
+    if not isinstance(t, torch.Tensor) or t.dtype != torch.float64 or not t.is_cuda:
+        raise TypeError(f"{name} must be a CUDA float64 torch.Tensor")
+    return t
+
+
+def _wave_struct(W, E_k, energies, a, R_out) -> pstgf_wave_t:
+    _dev_f64(W, "W"); _dev_f64(E_k, "E_k"); _dev_f64(energies, "energies"); _dev_f64(R_out, "R_out")
+    if W.dim() != 2 or W.stride(1) != 1 and W.shape[1] > 1:
+        raise ValueError("W must be [n_chan, n_poles] with unit stride along poles")
+    n_chan, n_poles = int(W.shape[0]), int(W.shape[1])
+    ldw = int(W.stride(0)) if n_chan > 1 else max(n_poles, int(W.stride(0)))
+    n_E = int(energies.shape[0])
+    if E_k.dim() != 1 or int(E_k.shape[0]) != n_poles or not E_k.is_contiguous():
+        raise ValueError("E_k must be contiguous [n_poles]")
+    if energies.dim() != 1 or not energies.is_contiguous():
+        raise ValueError("energies must be contiguous [n_E]")
+    if tuple(R_out.shape) != (n_E, n_chan, n_chan) or not R_out.is_contiguous():
+        raise ValueError("R_out must be contiguous [n_E, n_chan, n_chan]")
+    return pstgf_wave_t(n_chan, n_poles, n_E, ldw, float(a), W.data_ptr(), E_k.data_ptr(), energies.data_ptr(),
+                        R_out.data_ptr())
+
+
+def pstgf_rmat_form(W, E_k, energies, a: float, R_out=None, stream=None) -> torch.Tensor:
+    """R[e] = (1/2a) W diag(1/(E_k - E_e)) W^T for one partial wave (eq. 4).
+
+    W [n_chan, n_poles] (row stride = ldw), E_k [n_poles], energies [n_E]: CUDA float64 tensors.
+    Returns R_out [n_E, n_chan, n_chan] (allocated if not given).  Asynchronous on ``stream``.
+    """
+    lib = load()
+    if R_out is None:
+        R_out = torch.empty((energies.shape[0], W.shape[0], W.shape[0]), dtype=torch.float64, device=W.device)
+    w = _wave_struct(W, E_k, energies, a, R_out)
+    with torch.cuda.device(W.device):
+        _check(lib.pstgf_rmat_form(w.W, w.ldw, w.E_k, w.energies, w.n_chan, w.n_poles, w.n_E, w.a, w.R_out,
+                                   _stream_ptr(stream)))
+    return R_out
+
+
+def pstgf_rmat_form_naive(W, E_k, energies, a: float, R_out=None, stream=None) -> torch.Tensor:
+    """Same result from the library's term-by-term verification kernel (slow)."""
+    lib = load()
+    if R_out is None:
+        R_out = torch.empty((energies.shape[0], W.shape[0], W.shape[0]), dtype=torch.float64, device=W.device)
+    w = _wave_struct(W, E_k, energies, a, R_out)
+    with torch.cuda.device(W.device):
+        _check(lib.pstgf_rmat_form_naive(w.W, w.ldw, w.E_k, w.energies, w.n_chan, w.n_poles, w.n_E, w.a, w.R_out,
+                                         _stream_ptr(stream)))
+    return R_out
+
+
+def make_wave_array(waves: Sequence[tuple]) -> "ctypes.Array[pstgf_wave_t]":
+    """waves: sequence of (W, E_k, energies, a, R_out) tuples of CUDA tensors."""
+    arr = (pstgf_wave_t * len(waves))()
+    for p, (W, E_k, energies, a, R_out) in enumerate(waves):
+        arr[p] = _wave_struct(W, E_k, energies, a, R_out)
+    return arr
+
+
+def pstgf_rmat_batch_workspace_bytes(wave_array, n_waves: int | None = None) -> int:
+    lib = load()
+    n = len(wave_array) if n_waves is None else n_waves
+    return int(lib.pstgf_rmat_batch_workspace_bytes(wave_array, n))
+
+
+def pstgf_rmat_form_batch(wave_array, workspace: torch.Tensor, stream=None, n_waves: int | None = None) -> None:
+    """Ragged batch over partial waves in one persistent launch.  ``wave_array`` from make_wave_array;
+    ``workspace`` a CUDA uint8 tensor of at least pstgf_rmat_batch_workspace_bytes bytes (256-byte aligned)."""
+    lib = load()
+    n = len(wave_array) if n_waves is None else n_waves
+    with torch.cuda.device(workspace.device):
+        _check(lib.pstgf_rmat_form_batch(wave_array, n, workspace.data_ptr(), workspace.numel() * workspace.element_size(),
+                                         _stream_ptr(stream)))
+
+
+def pstgf_rmat_form_batch_host(host_waves: Sequence[tuple], max_chunk_bytes: int = 0, stream=None) -> None:
+    """End-to-end call over HOST tensors (pinned recommended): (W, E_k, energies, a, R_out) per wave, all CPU
+    float64 contiguous tensors; R_out is filled on return (the call synchronises)."""
+    lib = load()
+    arr = (pstgf_wave_t * len(host_waves))()
+    for p, (W, E_k, energies, a, R_out) in enumerate(host_waves):
+        for t, nm in ((W, "W"), (E_k, "E_k"), (energies, "energies"), (R_out, "R_out")):
+            if t.dtype != torch.float64 or t.is_cuda or not t.is_contiguous():
+                raise TypeError(f"{nm} must be a contiguous CPU float64 tensor")
+        n_chan, n_poles = int(W.shape[0]), int(W.shape[1])
+        arr[p] = pstgf_wave_t(n_chan, n_poles, int(energies.shape[0]), max(n_poles, 1) if n_chan <= 1 else int(W.stride(0)),
+                              float(a), W.data_ptr(), E_k.data_ptr(), energies.data_ptr(), R_out.data_ptr())
+    _check(lib.pstgf_rmat_form_batch_host(arr, len(host_waves), int(max_chunk_bytes), _stream_ptr(stream)))
+
+
+def pstgf_last_launch_count() -> int:
+    return int(load().pstgf_last_launch_count())
+
+
+def pstgf_version() -> int:
+    return int(load().pstgf_version())
+
+
+def pstgf_status_string(status: int) -> str:
+    return load().pstgf_status_string(int(status)).decode()
