@@ -1,0 +1,377 @@
+#!/usr/bin/env python
+"""bench.py -- R-matrix formation throughput on B200 (eq. 4 of arxiv 1909.07321).
+
+A "step" is one pass of the whole hot path (pole scaling, TMA staging, DMMA SYRK, mirrored
+store, scheduler: SURVEY.md 8a S1-S5) over one synthetic workload, through the C ABI of
+libpstgf_rmat.so.  Default workload: BASELINE.json configs[4], the "large single partial wave"
+the north_star's >= 70 % target is quoted on (n_chan 512, n_poles 10240, n_E 256); --config 1..5
+selects another (2-5 are parity-test sizes as well).
+
+    python bench.py --gpus 1 --steps 10 --warmup 3            # this repo's CUDA path
+    python bench.py --impl reference --steps 3 --warmup 1     # the CPU oracle as it stands
+
+One JSON line on stdout (rank 0).  See DESIGN.md "Measurement" for every key.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "R-matrix energies/s"
+UNIT = "energies/s"
+# FP64 nominal ratio used when the DMMA probe is not run: FP64 tensor 45 TFLOP/s per B200
+# (/opt/skills/guides/blackwell_cuda_programming.md:52) over bf16 dense 2250 TFLOP/s (B200_PROFILING.md:36).
+FP64_OVER_BF16_NOMINAL = 45.0 / 2250.0
+FALLBACK_BF16_TFLOPS = 1590.0      # B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
+FALLBACK_HBM_GBS = 6650.0
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return dict(source="measured", hbm_gbs=float(p["hbm_gbs"]), bf16=float(p["bf16_tflops"]),
+                    bf16_sustained=float(p.get("bf16_tflops_sustained", p["bf16_tflops"])),
+                    sm_max_mhz=float(p.get("sm_max_mhz", 1965.0)))
+    return dict(source="fallback", hbm_gbs=FALLBACK_HBM_GBS, bf16=FALLBACK_BF16_TFLOPS, bf16_sustained=1400.0,
+                sm_max_mhz=1965.0)
+
+
+# ---- clocks ----------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi -lms sampling of SM clock and throttle reasons during the timed region."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.file = None
+
+    def start(self):
+        try:
+            self.file = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits",
+                                          "-lms", "50", "-i", str(self.index)], stdout=self.file, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.file.flush()
+        self.file.seek(0)
+        clocks, reasons, power, cmax = [], set(), [], None
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.file.read().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                clocks.append(float(parts[0]))
+                cmax = float(parts[1])
+                power.append(float(parts[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        self.file.close()
+        try:
+            os.unlink(self.file.name)
+        except OSError:
+            pass
+        if clocks:
+            clocks.sort()
+            out.update(sm_mhz=clocks[len(clocks) // 2], sm_max_mhz=cmax, reasons=sorted(reasons), samples=len(clocks),
+                       power_w_max=max(power) if power else None)
+        return out
+
+
+# ---- workload --------------------------------------------------------------------------------
+def workload_description(cfg: int, wl) -> dict:
+    names = {1: "configs[0] single wave 8x160, n_E 1000", 2: "configs[1] single wave 64x1280, n_E 4096",
+             3: "configs[2] 8 waves 256x5120, n_E 2048 shared", 4: "configs[3] ragged 32 waves n_chan U[16,400], n_E 512",
+             5: "configs[4] large single wave 512x10240, n_E 256"}
+    return {"workload": names[cfg], "config_index": cfg - 1, "seed": wl.seed, "n_waves": len(wl.waves),
+            "n_chan": [w.n_chan for w in wl.waves] if len(wl.waves) <= 8 else
+            {"min": min(w.n_chan for w in wl.waves), "max": max(w.n_chan for w in wl.waves)},
+            "n_energies_per_step": wl.n_energies(), "counted_flop_per_step": wl.counted_flop(),
+            "r_bytes_per_step": wl.r_bytes(), "parallelism": "replica per GPU (waves/energies are independent)"}
+
+
+# ---- CPU oracle legs (the only places bench.py touches oracle/) ---------------------------------
+def oracle_sample_run(wl, energies_per_wave: int, threads: int):
+    """Time the oracle, as it stands, on the first `energies_per_wave` energies of every wave."""
+    from oracle import rmat_oracle
+    t0 = time.perf_counter()
+    n = 0
+    for w in wl.waves:
+        k = min(energies_per_wave, w.n_E)
+        rmat_oracle.rmat_form(w.W, w.E_k, w.energies[:k], w.a, threads=threads)
+        n += k
+    return n, time.perf_counter() - t0
+
+
+def oracle_cores():
+    from oracle import rmat_oracle
+    rmat_oracle.build()
+    return max(1, min(rmat_oracle.max_threads(), os.cpu_count() or 1))
+
+
+def est_oracle_seconds_per_energy(wl) -> float:
+    # ~2.6 ns per compensated term (SURVEY.md 8d probe), C(C+1)/2 * K terms... the oracle fills all C^2 entries
+    return sum(2.6e-9 * w.n_chan * w.n_chan * w.n_poles for w in wl.waves) / max(1, len(wl.waves))
+
+
+def cpu_baseline(wl, target_seconds: float) -> dict:
+    cores = oracle_cores()
+    per_e = est_oracle_seconds_per_energy(wl)                   # one thread, one energy of an average wave
+    # energies per wave so that the wall time is ~target_seconds with `cores` threads over energies
+    k = int(max(1, min(min(w.n_E for w in wl.waves), round(target_seconds * cores / (per_e * len(wl.waves))))))
+    if k >= cores:
+        k -= k % cores
+    n, dt = oracle_sample_run(wl, k, cores)
+    return {"value": n / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"first {k} energies of each of {len(wl.waves)} wave(s), {n} energies, {dt:.2f} s wall, "
+                      f"OpenMP over energies; every energy of a wave costs the same, so energies/s extrapolates",
+            "counted_gflops": n and sum(min(k, w.n_E) * w.n_chan ** 2 * w.n_poles for w in wl.waves) / dt / 1e9}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores; each step a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_1909_07321_b200 import inputs
+    wl = inputs.make_config(args.config)
+    cores = oracle_cores()
+    per_e = est_oracle_seconds_per_energy(wl)
+    budget = 120.0 / max(1, args.steps + args.warmup)            # whole run within a few minutes
+    k = int(max(1, min(min(w.n_E for w in wl.waves), round(min(budget, 20.0) * cores / (per_e * len(wl.waves))))))
+    if k >= cores:
+        k -= k % cores
+    for _ in range(args.warmup):
+        oracle_sample_run(wl, k, cores)
+    total_n, total_t = 0, 0.0
+    for _ in range(args.steps):
+        n, dt = oracle_sample_run(wl, k, cores)
+        total_n += n
+        total_t += dt
+    value = total_n / total_t
+    sample = f"each step: first {k} energies of each of {len(wl.waves)} wave(s) ({total_n // max(1, args.steps)} energies)"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 0, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * total_t / max(1, args.steps), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_description(args.config, wl),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ---- CUDA arm ----------------------------------------------------------------------------------
+def run_cuda(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_1909_07321_b200 import inputs, rmat
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: there is no CPU fallback for the product path")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    rmat.load()          # raises if libpstgf_rmat.so is missing
+    peaks = measured_peaks()
+
+    # Every rank forms the whole workload on its own GPU (replicas: waves and energies are independent,
+    # no data-path collective -- DESIGN.md "Multi-GPU").
+    wl = inputs.make_config(args.config)
+    dev_waves, shared = [], {}
+    for w in wl.waves:
+        key = id(w.energies)
+        if key not in shared:
+            shared[key] = torch.from_numpy(w.energies).cuda()
+        R = torch.empty((w.n_E, w.n_chan, w.n_chan), dtype=torch.float64, device="cuda")
+        dev_waves.append((torch.from_numpy(w.W).cuda(), torch.from_numpy(w.E_k).cuda(), shared[key], w.a, R))
+    single = len(dev_waves) == 1
+    if not single:
+        arr = rmat.make_wave_array(dev_waves)
+        ws = torch.empty(rmat.pstgf_rmat_batch_workspace_bytes(arr), dtype=torch.uint8, device="cuda")
+    flush_buf = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+
+    def step():
+        if single:
+            W, E_k, en, a, R = dev_waves[0]
+            rmat.pstgf_rmat_form(W, E_k, en, a, R_out=R)
+        else:
+            rmat.pstgf_rmat_form_batch(arr, ws)
+        return rmat.pstgf_last_launch_count()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(3, args.warmup)):
+        flush_buf.zero_()
+        step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.15)
+    starts = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    ends = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    launches = 0
+    barrier()
+    wall0 = time.perf_counter()
+    for i in range(args.steps):
+        flush_buf.zero_()                 # L2 flush between timed iterations (outside the event pair)
+        starts[i].record()
+        launches += step()
+        ends[i].record()
+    barrier()
+    wall = time.perf_counter() - wall0
+    step_ms = [s.elapsed_time(e) for s, e in zip(starts, ends)]
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = float(sum(step_ms))
+    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms_max = float(t.item())
+    ms_per_step = total_ms_max / args.steps
+    n_e = wl.n_energies()
+    value = world * n_e * args.steps / (total_ms_max * 1e-3)
+    flop = wl.counted_flop()
+
+    # ---- dominant kernel: the persistent DMMA SYRK kernel is the only launch of a step ----
+    kern_ms = total_ms / args.steps                      # this rank's average launch duration (CUDA events, launch stream)
+    achieved_tflops = flop / (kern_ms * 1e-3) / 1e12
+    # FP64 peak: probe the DMMA pipe (the instruction the kernel issues) right here, burst, best of 5
+    probe = None
+    if rank == 0:
+        sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
+        sink = torch.empty(sms * 4 * 256, dtype=torch.float64, device="cuda")
+        probe = {}
+        for kind, name in ((0, "dmma"), (1, "dfma"), (2, "dmma+dfma")):
+            best = 0.0
+            for _ in range(5):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                fl = rmat.pstgf_fp64_probe(kind, 4000, sms * 4, 256, sink)
+                e1.record()
+                torch.cuda.synchronize()
+                best = max(best, fl / (e0.elapsed_time(e1) * 1e-3) / 1e12)
+            probe[name] = best
+    peak_rule = peaks["bf16"] * FP64_OVER_BF16_NOMINAL       # the other dtype's measured burst peak x nominal ratio
+    t_fp64 = flop / (peak_rule * 1e12)
+    t_hbm = wl.r_bytes() / (peaks["hbm_gbs"] * 1e9)
+    roofline = {"bound": "tensor", "achieved": achieved_tflops, "peak": peak_rule, "unit": "TFLOP/s",
+                "frac": achieved_tflops / peak_rule, "traffic": None,
+                "peak_source": f"{peaks['source']} bf16 burst {peaks['bf16']} TFLOP/s x nominal FP64/bf16 ratio 45/2250",
+                "kernel": "rmat_persistent_kernel", "flop_per_launch": flop,
+                "t_roof_ms": 1e3 * max(t_fp64, t_hbm), "hbm_write_gbs": wl.r_bytes() / (kern_ms * 1e-3) / 1e9,
+                "hbm_peak_gbs": peaks["hbm_gbs"]}
+    if probe:
+        roofline["fp64_probe_tflops"] = probe
+        roofline["frac_of_dmma_probe"] = achieved_tflops / probe["dmma"] if probe["dmma"] > 0 else None
+    traffic_file = os.path.join(ROOT, "profiles", f"traffic_config{args.config}.json")
+    if os.path.exists(traffic_file):
+        with open(traffic_file) as f:
+            roofline["traffic"] = json.load(f).get("dram_bytes_per_launch")
+
+    # ---- end to end: HOST buffers through the C ABI, copies inside the timed region ----
+    e2e = None
+    if not args.no_e2e:
+        host = []
+        for w in wl.waves:
+            hW = torch.from_numpy(w.W).pin_memory()
+            hEk = torch.from_numpy(w.E_k).pin_memory()
+            hEn = torch.from_numpy(w.energies).pin_memory()
+            hR = torch.empty((w.n_E, w.n_chan, w.n_chan), dtype=torch.float64).pin_memory()
+            host.append((hW, hEk, hEn, w.a, hR))
+        h2d = sum(8 * (a[0].numel() + a[1].numel() + a[2].numel()) for a in host)
+        d2h = sum(8 * a[4].numel() for a in host)
+        e2e_steps = max(1, min(args.steps, 5))
+        rmat.pstgf_rmat_form_batch_host(host)        # warm-up (allocator pool, pinned pages)
+        barrier()
+        t0 = time.perf_counter()
+        e2e_launches = 0
+        for _ in range(e2e_steps):
+            rmat.pstgf_rmat_form_batch_host(host)    # synchronises before returning
+            e2e_launches += rmat.pstgf_last_launch_count()
+        torch.cuda.synchronize()
+        dt = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(dt, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * n_e * e2e_steps / float(dt.item()), "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "steps": e2e_steps, "ms_per_step": 1e3 * float(dt.item()) / e2e_steps,
+               "api": "pstgf_rmat_form_batch_host (pinned host buffers; whole R copied back)"}
+        del host
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_baseline(wl, args.cpu_seconds)
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": dict(workload_description(args.config, wl), l2="flushed between timed steps (512 MiB write)",
+                               sha256=wl.sha256()[:16]),
+                "tflops_counted": world * flop * args.steps / (total_ms_max * 1e-3) / 1e12,
+                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,
+                "clocks": clocks, "wall_s_timed_region": wall, "step_ms_min_max": [min(step_ms), max(step_ms)]}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -8,7 +8,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libpstgf_rmat.so")
-SOURCES = [os.path.join(CSRC, "pstgf_rmat.cu")]
+SOURCES = [os.path.join(CSRC, "pstgf_rmat.cu"), os.path.join(CSRC, "fp64_probe.cu")]
 HEADERS = [os.path.join(CSRC, "rmat_common.h"), os.path.join(CSRC, "rmat_kernel.cuh"),
            os.path.join(os.path.dirname(_HERE), "include", "pstgf_rmat.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
