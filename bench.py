@@ -296,7 +296,7 @@ def run_cuda(args):
             for _ in range(5):
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 e0.record()
-                fl = rmat.pstgf_fp64_probe(kind, 4000, sms * 4, 256, sink)
+                fl = rmat.pstgf_fp64_probe(kind, 2000, sms * 2, 256, sink)
                 e1.record()
                 torch.cuda.synchronize()
                 best = max(best, fl / (e0.elapsed_time(e1) * 1e-3) / 1e12)

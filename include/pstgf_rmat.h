@@ -145,8 +145,9 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
  * Measurement utility (not on the hot path): a register-resident FP64
  * throughput probe that fixes the roofline denominator of the contraction
  * (MEASURED_PEAKS.json has no FP64 entry).  kind 0 = DMMA.8x8x4 (the
- * instruction the SYRK kernel issues), 1 = DFMA, 2 = both interleaved.
- * Launches `blocks` CTAs of `threads` threads (multiple of 32, <= 1024) that
+ * instruction the SYRK kernel issues, in its register-tile pattern), 1 = DFMA,
+ * 2 = DMMA on even warps and DFMA on odd warps.
+ * Launches `blocks` CTAs of `threads` threads (multiple of 32, <= 256) that
  * each run `iters` iterations; DEVICE `sink` receives blocks*threads doubles.
  * HOST `flop_out` (may be NULL) receives the FLOPs the launch performs
  * (2 per FMA).  Asynchronous on `stream`; time it with events.

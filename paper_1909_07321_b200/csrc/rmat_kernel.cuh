@@ -87,15 +87,15 @@ __device__ __forceinline__ void consume_idle(int n_kt, PipeState &ps, uint32_t f
 
 // OFF tile: 64 x 32 block strictly above the diagonal; 8 x 4 DMMA blocks, all needed
 // (column blocks >= nblk lie beyond n_chan and are skipped).
+template <int NCB>
 __device__ __forceinline__ void consume_off(const ItemInfo &it, const unsigned char *smem, PipeState &ps,
                                             uint32_t full0, uint32_t empty0, int warp, int lane) {
-  double acc[8][4][2];
+  double acc[8][NCB][2];
 #pragma unroll
   for (int bi = 0; bi < 8; ++bi)
 #pragma unroll
-    for (int bj = 0; bj < 4; ++bj) acc[bi][bj][0] = acc[bi][bj][1] = 0.0;
+    for (int bj = 0; bj < NCB; ++bj) acc[bi][bj][0] = acc[bi][bj][1] = 0.0;
   const int g = lane >> 2, q = lane & 3;
-  const int ncb = it.nblk;
   for (int kt = 0; kt < it.n_kt; ++kt) {
     mbar_wait(full0 + 8 * ps.stage, ps.phase);
     const double *wi = reinterpret_cast<const double *>(smem + ps.stage * STAGE_BYTES) + g * KT + q;
@@ -109,12 +109,10 @@ __device__ __forceinline__ void consume_off(const ItemInfo &it, const unsigned c
 #pragma unroll
       for (int bi = 0; bi < 8; ++bi) a[bi] = wi[bi * 8 * KT + ks * 4];
 #pragma unroll
-      for (int bj = 0; bj < 4; ++bj) {
-        if (bj < ncb) {
-          const double b = wj[bj * 8 * KT + ks * 4] * dv;   // pole scaling folded into the B fragment
+      for (int bj = 0; bj < NCB; ++bj) {
+        const double b = wj[bj * 8 * KT + ks * 4] * dv;   // pole scaling folded into the B fragment
 #pragma unroll
-          for (int bi = 0; bi < 8; ++bi) dmma884(acc[bi][bj][0], acc[bi][bj][1], a[bi], b);
-        }
+        for (int bi = 0; bi < 8; ++bi) dmma884(acc[bi][bj][0], acc[bi][bj][1], a[bi], b);
       }
     }
     __syncwarp();
@@ -126,16 +124,14 @@ __device__ __forceinline__ void consume_off(const ItemInfo &it, const unsigned c
   double *R = it.R + (size_t)warp * C * C;
   const double s = it.inv2a;
 #pragma unroll
-  for (int bj = 0; bj < 4; ++bj) {
-    if (bj < ncb) {
-      const int c = it.col0 + bj * 8 + 2 * q;
+  for (int bj = 0; bj < NCB; ++bj) {
+    const int c = it.col0 + bj * 8 + 2 * q;
 #pragma unroll
-      for (int bi = 0; bi < 8; ++bi) {
-        const int r = it.row0 + bi * 8 + g;
-        const double v0 = acc[bi][bj][0] * s, v1 = acc[bi][bj][1] * s;
-        if (c < C) { __stcs(R + (size_t)r * C + c, v0); __stcs(R + (size_t)c * C + r, v0); }
-        if (c + 1 < C) { __stcs(R + (size_t)r * C + c + 1, v1); __stcs(R + (size_t)(c + 1) * C + r, v1); }
-      }
+    for (int bi = 0; bi < 8; ++bi) {
+      const int r = it.row0 + bi * 8 + g;
+      const double v0 = acc[bi][bj][0] * s, v1 = acc[bi][bj][1] * s;
+      if (c < C) { __stcs(R + (size_t)r * C + c, v0); __stcs(R + (size_t)c * C + r, v0); }
+      if (c + 1 < C) { __stcs(R + (size_t)r * C + c + 1, v1); __stcs(R + (size_t)(c + 1) * C + r, v1); }
     }
   }
 }
@@ -143,13 +139,13 @@ __device__ __forceinline__ void consume_off(const ItemInfo &it, const unsigned c
 // DIAG tile: 64 x 64 block on the diagonal; only 8x8 blocks (bi <= bj) are computed, and in
 // blocks on the diagonal only elements c >= r are stored (with their mirror), so that
 // R[n][m] == R[m][n] bitwise.
+template <int NB>
 __device__ __forceinline__ void consume_diag(const ItemInfo &it, const unsigned char *smem, PipeState &ps,
                                              uint32_t full0, uint32_t empty0, int warp, int lane) {
-  double acc[36][2];
+  double acc[NB * (NB + 1) / 2][2];
 #pragma unroll
-  for (int t = 0; t < 36; ++t) acc[t][0] = acc[t][1] = 0.0;
+  for (int t = 0; t < NB * (NB + 1) / 2; ++t) acc[t][0] = acc[t][1] = 0.0;
   const int g = lane >> 2, q = lane & 3;
-  const int nb = it.nblk;
   for (int kt = 0; kt < it.n_kt; ++kt) {
     mbar_wait(full0 + 8 * ps.stage, ps.phase);
     const double *wi = reinterpret_cast<const double *>(smem + ps.stage * STAGE_BYTES) + g * KT + q;
@@ -158,16 +154,14 @@ __device__ __forceinline__ void consume_diag(const ItemInfo &it, const unsigned 
 #pragma unroll
     for (int ks = 0; ks < KT / 4; ++ks) {
       const double dv = dd[ks * 4];
-      double a[8];
+      double a[NB];
 #pragma unroll
-      for (int bi = 0; bi < 8; ++bi) a[bi] = wi[bi * 8 * KT + ks * 4];
+      for (int bi = 0; bi < NB; ++bi) a[bi] = wi[bi * 8 * KT + ks * 4];
 #pragma unroll
-      for (int bj = 0; bj < 8; ++bj) {
-        if (bj < nb) {
-          const double b = a[bj] * dv;
+      for (int bj = 0; bj < NB; ++bj) {
+        const double b = a[bj] * dv;
 #pragma unroll
-          for (int bi = 0; bi <= bj; ++bi) dmma884(acc[bj * (bj + 1) / 2 + bi][0], acc[bj * (bj + 1) / 2 + bi][1], a[bi], b);
-        }
+        for (int bi = 0; bi <= bj; ++bi) dmma884(acc[bj * (bj + 1) / 2 + bi][0], acc[bj * (bj + 1) / 2 + bi][1], a[bi], b);
       }
     }
     __syncwarp();
@@ -178,24 +172,47 @@ __device__ __forceinline__ void consume_diag(const ItemInfo &it, const unsigned 
   double *R = it.R + (size_t)warp * C * C;
   const double s = it.inv2a;
 #pragma unroll
-  for (int bj = 0; bj < 8; ++bj) {
-    if (bj < nb) {
-      const int c = it.row0 + bj * 8 + 2 * q;
+  for (int bj = 0; bj < NB; ++bj) {
+    const int c = it.row0 + bj * 8 + 2 * q;
 #pragma unroll
-      for (int bi = 0; bi <= bj; ++bi) {
-        const int r = it.row0 + bi * 8 + g;
-        const double v0 = acc[bj * (bj + 1) / 2 + bi][0] * s, v1 = acc[bj * (bj + 1) / 2 + bi][1] * s;
-        if (r < C) {
-          if (c < C && c >= r) {
-            __stcs(R + (size_t)r * C + c, v0);
-            if (c > r) __stcs(R + (size_t)c * C + r, v0);
-          }
-          if (c + 1 < C && c + 1 >= r) {
-            __stcs(R + (size_t)r * C + c + 1, v1);
-            if (c + 1 > r) __stcs(R + (size_t)(c + 1) * C + r, v1);
-          }
+    for (int bi = 0; bi <= bj; ++bi) {
+      const int r = it.row0 + bi * 8 + g;
+      const double v0 = acc[bj * (bj + 1) / 2 + bi][0] * s, v1 = acc[bj * (bj + 1) / 2 + bi][1] * s;
+      if (r < C) {
+        if (c < C && c >= r) {
+          __stcs(R + (size_t)r * C + c, v0);
+          if (c > r) __stcs(R + (size_t)c * C + r, v0);
+        }
+        if (c + 1 < C && c + 1 >= r) {
+          __stcs(R + (size_t)r * C + c + 1, v1);
+          if (c + 1 > r) __stcs(R + (size_t)(c + 1) * C + r, v1);
         }
       }
+    }
+  }
+}
+
+// The tile shapes are compile-time variants (no predicates inside the DMMA loop); ragged edges of
+// a wave pick the variant with fewer 8-wide blocks.
+__device__ __forceinline__ void consume_item(const ItemInfo &it, const unsigned char *smem, PipeState &ps,
+                                             uint32_t full0, uint32_t empty0, int warp, int lane) {
+  if (it.kind == 0) {
+    switch (it.nblk) {
+      case 8: consume_diag<8>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 7: consume_diag<7>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 6: consume_diag<6>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 5: consume_diag<5>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 4: consume_diag<4>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 3: consume_diag<3>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 2: consume_diag<2>(it, smem, ps, full0, empty0, warp, lane); break;
+      default: consume_diag<1>(it, smem, ps, full0, empty0, warp, lane); break;
+    }
+  } else {
+    switch (it.nblk) {
+      case 4: consume_off<4>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 3: consume_off<3>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 2: consume_off<2>(it, smem, ps, full0, empty0, warp, lane); break;
+      default: consume_off<1>(it, smem, ps, full0, empty0, warp, lane); break;
     }
   }
 }
@@ -239,8 +256,7 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
 rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__restrict__ waves,
                        const long long *__restrict__ item_begin, int n_waves, long long n_items,
                        unsigned long long *counter) {
-  extern __shared__ unsigned char smem_raw[];
-  unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
+  extern __shared__ __align__(128) unsigned char smem[];   // used directly: the shared address space is kept (LDS/STS)
   const uint32_t bar0 = smem_u32(smem + SMEM_BARRIER_OFFSET);
   const uint32_t full0 = bar0, empty0 = bar0 + 8 * STAGES;
   const uint32_t item_full0 = bar0 + 16 * STAGES, item_empty0 = item_full0 + 16;
@@ -385,8 +401,7 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
       const ItemInfo it = ring[iq];
       if (it.kind < 0) break;
       if (warp >= it.n_valid_e) consume_idle(it.n_kt, ps, full0, empty0, lane);
-      else if (it.kind == 0) consume_diag(it, smem, ps, full0, empty0, warp, lane);
-      else consume_off(it, smem, ps, full0, empty0, warp, lane);
+      else consume_item(it, smem, ps, full0, empty0, warp, lane);
       __syncwarp();
       if (lane == 0) mbar_arrive(item_empty0 + 8 * iq);
       iq ^= 1u;
