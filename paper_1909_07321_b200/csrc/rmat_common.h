@@ -22,7 +22,8 @@ constexpr int TN = 32;      // OFF tile columns: J panel; also the TMA box heigh
 constexpr int KT = 20;      // poles per pipeline stage; row pitch 20 doubles == 4 (mod 16) -> conflict-free LDS.64
 constexpr int EB = 8;       // energies per item == consumer warps per CTA
 constexpr int STAGES = 8;   // smem ring depth
-constexpr int NUM_THREADS = (EB + 4) * 32;           // 8 consumer warps + the producer warpgroup (1 of its 4 warps works)
+constexpr int PRODUCER_WARPS = 4;                    // one warpgroup: 1 load warp + 3 pole-scaling warps
+constexpr int NUM_THREADS = (EB + PRODUCER_WARPS) * 32;   // 8 consumer warps + the producer warpgroup
 constexpr int PRODUCER_REGS = 56;                    // setmaxnreg targets: 8*224 + 4*56 = 12*168, the launch allocation
 constexpr int CONSUMER_REGS = 224;
 constexpr int BOX_BYTES = TN * KT * 8;               // one TMA box: 32 rows x 20 poles

@@ -1,10 +1,10 @@
 // rmat_kernel.cuh -- the persistent sm_100a kernel behind pstgf_rmat_form / pstgf_rmat_form_batch.
 //
 // One CTA per SM, 12 warps.  Warps 8..11 are the producer warpgroup: they hand most of their
-// registers to the consumers (setmaxnreg) and only warp 8 works: it takes work items (atomic counter in the
-// batch call, round-robin in the single-wave call), issues the TMA loads of the W panels and
-// builds the pole scaling d_e[k] = 1/(E_k - E_e) of the stage in shared memory (SURVEY 8a-S1,
-// S2; the denominator of eq. 4).  Warps 0..7 are consumers, one energy of the
+// registers to the consumers (setmaxnreg).  Warp 8 takes work items (atomic counter in the batch
+// call, round-robin in the single-wave call), publishes them and issues the TMA loads of the W
+// panels; warps 9..11 build the pole scaling d_e[k] = 1/(E_k - E_e) of every
+// stage in shared memory (S1; the denominator of eq. 4).  Warps 0..7 are consumers, one energy of the
 // item's block each: they contract acc[n][m] += W[n][k] * (W[m][k] * d_e[k]) on the FP64 tensor
 // pipe (mma.sync m8n8k4 -> DMMA.8x8x4) over upper-triangle tiles only (S3) and
 // write R and its mirror scaled by 1/(2a) (S4).  Producer and consumers are
@@ -15,16 +15,18 @@
 
 namespace pstgf {
 
-struct ItemInfo {        // handed from the producer to the consumers through smem
+struct ItemInfo {        // handed from the load warp to the pole-scaling and consumer warps through smem
   double *R;             // R_out of the block's first energy
+  const double *E_k;     // the wave's poles
+  const double *energies;// the block's first energy
   double inv2a;
   int n_chan;
+  int n_poles;
   int n_valid_e;         // energies in this block (1..EB)
   int row0, col0;
   int kind;              // 0 DIAG, 1 OFF, -1 stop
   int nblk;              // DIAG: valid 8x8 block rows/cols; OFF: valid 8-wide column blocks
   int n_kt;
-  int pad_;
 };
 static_assert(sizeof(ItemInfo) <= 64, "ItemInfo slot");
 
@@ -265,130 +267,156 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < STAGES; ++s) {
-      mbar_init(full0 + 8 * s, 33);    // 32 producer lanes (d written) + 1 (TMA expect_tx / plain staging done)
+      mbar_init(full0 + 8 * s, PRODUCER_WARPS);   // load warp (TMA expect_tx / plain staging done) + 3 pole-scaling warps
       mbar_init(empty0 + 8 * s, EB);   // one arrival per consumer warp
     }
     for (int s = 0; s < 2; ++s) {
       mbar_init(item_full0 + 8 * s, 1);
-      mbar_init(item_empty0 + 8 * s, EB);
+      mbar_init(item_empty0 + 8 * s, EB + PRODUCER_WARPS - 1);   // consumers + pole-scaling warps
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
 
   if (warp >= EB) {
-    // ================= producer warpgroup: give registers away, warp EB does the work =================
+    // ================= producer warpgroup: give registers away =================
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(PRODUCER_REGS));
-    if (warp != EB) return;
-    PipeState ps;
-    uint32_t iq = 0, iphase = 0;
-    long long next_static = blockIdx.x;
-    for (;;) {
-      long long item;
-      if (BATCH) {
-        unsigned long long got = 0;
-        if (lane == 0) got = atomicAdd(counter, 1ULL);
-        item = (long long)__shfl_sync(0xffffffffu, got, 0);
-      } else {
-        item = next_static;
-        next_static += gridDim.x;
-      }
-      const bool stop = item >= n_items;
-      // locate the wave (batch: binary search in the item-range table)
-      int p = 0;
-      if (BATCH && !stop) {
-        int lo = 0, hi = n_waves;            // item_begin[lo] <= item < item_begin[hi]
-        while (hi - lo > 1) {
-          const int mid = (lo + hi) >> 1;
-          if (__ldg(item_begin + mid) <= item) lo = mid; else hi = mid;
-        }
-        p = lo;
-        item -= __ldg(item_begin + p);
-      }
-      const DevWave &w = BATCH ? waves[p] : single;
-      int kind = -1, row0 = 0, col0 = 0, nblk = 0, eb = 0, n_valid = 0, n_kt = 0;
-      if (!stop) {
-        const int tile = (int)(item / w.n_eb);
-        eb = (int)(item - (long long)tile * w.n_eb);
-        decode_tile(w, tile, kind, row0, col0, nblk);
-        n_valid = min(EB, w.n_E - eb * EB);
-        n_kt = w.n_kt;
-      }
-      mbar_wait(item_empty0 + 8 * iq, iphase ^ 1u);
-      if (lane == 0) {
-        ItemInfo &ii = ring[iq];
-        ii.kind = kind;
-        if (!stop) {
-          ii.R = w.R_out + (size_t)eb * EB * w.n_chan * w.n_chan;
-          ii.inv2a = w.inv2a;
-          ii.n_chan = w.n_chan;
-          ii.n_valid_e = n_valid;
-          ii.row0 = row0;
-          ii.col0 = col0;
-          ii.nblk = nblk;
-          ii.n_kt = n_kt;
-        }
-        mbar_arrive(item_full0 + 8 * iq);   // release: the stores above are visible to waiters
-      }
-      iq ^= 1u;
-      if (iq == 0) iphase ^= 1u;
-      if (stop) break;
-
-      // per-item constants of the pole-scaling stage: lane handles entries idx = lane + 32 t of d[EB][KT]
-      constexpr int DT = EB * KT / 32;
-      static_assert(EB * KT % 32 == 0, "d tile must split evenly over the producer warp");
-      double en[DT];
-      int kk[DT];
-      bool ev[DT];
-#pragma unroll
-      for (int t = 0; t < DT; ++t) {
-        const int idx = lane + 32 * t;
-        const int e = idx / KT;
-        kk[t] = idx - e * KT;
-        ev[t] = e < n_valid;
-        en[t] = ev[t] ? __ldg(w.energies + (size_t)eb * EB + e) : 0.0;
-      }
-      double ek[DT];
-#pragma unroll
-      for (int t = 0; t < DT; ++t) ek[t] = (ev[t] && kk[t] < w.n_poles) ? __ldg(w.E_k + kk[t]) : 0.0;
-      const CUtensorMap *map = &w.map;
-      const uint32_t tx_bytes = (kind == 0 ? 2 : 3) * BOX_BYTES;
-      for (int kt = 0; kt < n_kt; ++kt) {
-        const int k0 = kt * KT;
-        // prefetch the next stage's poles before blocking on the ring
-        double ek_next[DT];
-#pragma unroll
-        for (int t = 0; t < DT; ++t) {
-          const int k = k0 + KT + kk[t];
-          ek_next[t] = (ev[t] && k < w.n_poles) ? __ldg(w.E_k + k) : 0.0;
-        }
-        mbar_wait(empty0 + 8 * ps.stage, ps.phase ^ 1u);
-        unsigned char *st = smem + ps.stage * STAGE_BYTES;
-        const uint32_t full = full0 + 8 * ps.stage;
-        if (w.use_tma) {
-          if (lane == 0) {
-            mbar_arrive_expect_tx(full, tx_bytes);
-            const uint32_t dst = smem_u32(st);
-            tma_load_2d(dst, map, k0, row0, full);
-            tma_load_2d(dst + BOX_BYTES, map, k0, row0 + TN, full);
-            if (kind != 0) tma_load_2d(dst + WI_BYTES, map, k0, col0, full);
-          }
+    if (warp == EB) {
+      // ---- load warp: takes work items, publishes them, stages the W panels (S2, S5) ----
+      PipeState ps;
+      uint32_t iq = 0, iphase = 0;
+      long long next_static = blockIdx.x;
+      for (;;) {
+        long long item;
+        if (BATCH) {
+          unsigned long long got = 0;
+          if (lane == 0) got = atomicAdd(counter, 1ULL);
+          item = (long long)__shfl_sync(0xffffffffu, got, 0);
         } else {
-          stage_panel_plain(reinterpret_cast<double *>(st), w, row0, TM, k0, lane);
-          if (kind != 0) stage_panel_plain(reinterpret_cast<double *>(st + WI_BYTES), w, col0, TN, k0, lane);
-          __syncwarp();
-          if (lane == 0) mbar_arrive(full);
+          item = next_static;
+          next_static += gridDim.x;
         }
-        // S1: d_e[k] = 1/(E_k - E_e); 0 beyond n_poles / n_E so that zero-filled W columns stay zero
-        double *dsm = reinterpret_cast<double *>(st + WI_BYTES + WJ_BYTES);
+        const bool stop = item >= n_items;
+        // locate the wave (batch: binary search in the item-range table)
+        int p = 0;
+        if (BATCH && !stop) {
+          int lo = 0, hi = n_waves;            // item_begin[lo] <= item < item_begin[hi]
+          while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (__ldg(item_begin + mid) <= item) lo = mid; else hi = mid;
+          }
+          p = lo;
+          item -= __ldg(item_begin + p);
+        }
+        const DevWave &w = BATCH ? waves[p] : single;
+        int kind = -1, row0 = 0, col0 = 0, nblk = 0, eb = 0, n_valid = 0, n_kt = 0;
+        if (!stop) {
+          const int tile = (int)(item / w.n_eb);
+          eb = (int)(item - (long long)tile * w.n_eb);
+          decode_tile(w, tile, kind, row0, col0, nblk);
+          n_valid = min(EB, w.n_E - eb * EB);
+          n_kt = w.n_kt;
+        }
+        mbar_wait(item_empty0 + 8 * iq, iphase ^ 1u);
+        if (lane == 0) {
+          ItemInfo &ii = ring[iq];
+          ii.kind = kind;
+          if (!stop) {
+            ii.R = w.R_out + (size_t)eb * EB * w.n_chan * w.n_chan;
+            ii.E_k = w.E_k;
+            ii.energies = w.energies + (size_t)eb * EB;
+            ii.inv2a = w.inv2a;
+            ii.n_chan = w.n_chan;
+            ii.n_poles = w.n_poles;
+            ii.n_valid_e = n_valid;
+            ii.row0 = row0;
+            ii.col0 = col0;
+            ii.nblk = nblk;
+            ii.n_kt = n_kt;
+          }
+          mbar_arrive(item_full0 + 8 * iq);   // release: the stores above are visible to waiters
+        }
+        iq ^= 1u;
+        if (iq == 0) iphase ^= 1u;
+        if (stop) break;
+
+        const CUtensorMap *map = &w.map;
+        const uint32_t tx_bytes = (kind == 0 ? 2 : 3) * BOX_BYTES;
+        for (int kt = 0; kt < n_kt; ++kt) {
+          const int k0 = kt * KT;
+          mbar_wait(empty0 + 8 * ps.stage, ps.phase ^ 1u);
+          unsigned char *st = smem + ps.stage * STAGE_BYTES;
+          const uint32_t full = full0 + 8 * ps.stage;
+          if (w.use_tma) {
+            if (lane == 0) {
+              mbar_arrive_expect_tx(full, tx_bytes);
+              const uint32_t dst = smem_u32(st);
+              tma_load_2d(dst, map, k0, row0, full);
+              tma_load_2d(dst + BOX_BYTES, map, k0, row0 + TN, full);
+              if (kind != 0) tma_load_2d(dst + WI_BYTES, map, k0, col0, full);
+            }
+          } else {
+            stage_panel_plain(reinterpret_cast<double *>(st), w, row0, TM, k0, lane);
+            if (kind != 0) stage_panel_plain(reinterpret_cast<double *>(st + WI_BYTES), w, col0, TN, k0, lane);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(full);
+          }
+          ps.advance();
+        }
+      }
+    } else {
+      // ---- pole-scaling warps (S1): d_e[k] = 1/(E_k - E_e) of every stage, built in shared memory.
+      // Three warps on three different SM sub-partitions share the EB x KT entries of a stage: the FP64
+      // pipe they need is saturated by the consumers' DMMAs, and one warp alone cannot get enough issue
+      // slots to keep up with the ring.
+      constexpr int DW = PRODUCER_WARPS - 1;                 // 3 warps, 96 lanes
+      constexpr int DT = (EB * KT + DW * 32 - 1) / (DW * 32);
+      const int dl = (warp - EB - 1) * 32 + lane;
+      PipeState ps;
+      uint32_t iq = 0, iphase = 0;
+      for (;;) {
+        mbar_wait(item_full0 + 8 * iq, iphase);
+        const ItemInfo it = ring[iq];
+        __syncwarp();
+        if (lane == 0) mbar_arrive(item_empty0 + 8 * iq);
+        iq ^= 1u;
+        if (iq == 0) iphase ^= 1u;
+        if (it.kind < 0) break;
+        double en[DT], ek[DT];
+        int kk[DT], slot[DT];
+        bool ev[DT];
 #pragma unroll
         for (int t = 0; t < DT; ++t) {
-          const bool ok = ev[t] && (k0 + kk[t] < w.n_poles);
-          dsm[lane + 32 * t] = ok ? 1.0 / (ek[t] - en[t]) : 0.0;
-          ek[t] = ek_next[t];
+          const int idx = dl + DW * 32 * t;
+          const int e = idx / KT;
+          slot[t] = idx < EB * KT ? idx : -1;
+          kk[t] = idx - e * KT;
+          ev[t] = slot[t] >= 0 && e < it.n_valid_e;
+          en[t] = ev[t] ? __ldg(it.energies + e) : 0.0;
+          ek[t] = (ev[t] && kk[t] < it.n_poles) ? __ldg(it.E_k + kk[t]) : 0.0;
         }
-        mbar_arrive(full);
-        ps.advance();
+        for (int kt = 0; kt < it.n_kt; ++kt) {
+          const int k0 = kt * KT;
+          // prefetch the next stage's poles before blocking on the ring
+          double ek_next[DT];
+#pragma unroll
+          for (int t = 0; t < DT; ++t) {
+            const int k = k0 + KT + kk[t];
+            ek_next[t] = (ev[t] && k < it.n_poles) ? __ldg(it.E_k + k) : 0.0;
+          }
+          mbar_wait(empty0 + 8 * ps.stage, ps.phase ^ 1u);
+          double *dsm = reinterpret_cast<double *>(smem + ps.stage * STAGE_BYTES + WI_BYTES + WJ_BYTES);
+#pragma unroll
+          for (int t = 0; t < DT; ++t) {
+            // 0 beyond n_poles / n_E so that zero-filled W columns stay zero
+            const bool ok = ev[t] && (k0 + kk[t] < it.n_poles);
+            if (slot[t] >= 0) dsm[slot[t]] = ok ? 1.0 / (ek[t] - en[t]) : 0.0;
+            ek[t] = ek_next[t];
+          }
+          __syncwarp();
+          if (lane == 0) mbar_arrive(full0 + 8 * ps.stage);
+          ps.advance();
+        }
       }
     }
   } else {
