@@ -127,7 +127,7 @@ def workload_description(cfg: int, wl) -> dict:
             "n_chan": [w.n_chan for w in wl.waves] if len(wl.waves) <= 8 else
             {"min": min(w.n_chan for w in wl.waves), "max": max(w.n_chan for w in wl.waves)},
             "n_energies_per_step": wl.n_energies(), "counted_flop_per_step": wl.counted_flop(),
-            "r_bytes_per_step": wl.r_bytes(), "parallelism": "replica per GPU (waves/energies are independent)"}
+            "r_bytes_per_step": wl.r_bytes(), "parallelism": "energy blocks sharded over ranks, wave-rotated (shard.plan); no collective"}
 
 
 # ---- CPU oracle legs (the only places bench.py touches oracle/) ---------------------------------
@@ -201,6 +201,23 @@ def run_reference(args):
     return 0
 
 
+def ncu_traffic(cfg: int):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the SYRK kernel from the committed
+    `ncu --set full` capture (profiles/traffic.csv: config,dram_bytes_per_launch,...), else None."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(path):
+        return None
+    with open(path) as f:
+        for line in f:
+            parts = line.strip().split(",")
+            if parts and parts[0] == str(cfg):
+                try:
+                    return float(parts[1])
+                except (ValueError, IndexError):
+                    return None
+    return None
+
+
 # ---- CUDA arm ----------------------------------------------------------------------------------
 def run_cuda(args):
     import numpy as np
@@ -220,9 +237,21 @@ def run_cuda(args):
     rmat.load()          # raises if libpstgf_rmat.so is missing
     peaks = measured_peaks()
 
-    # Every rank forms the whole workload on its own GPU (replicas: waves and energies are independent,
-    # no data-path collective -- DESIGN.md "Multi-GPU").
-    wl = inputs.make_config(args.config)
+    # Weak scaling over ranks: at N ranks the job is the configuration with an N times
+    # finer energy mesh; shard.plan gives each rank its wave-rotated share of the energy blocks (PAPER.md:116,
+    # :135-137, Fig. 1), i.e. the configuration's own n_E per wave and rank.  No data-path collective.
+    if world == 1:
+        wl = inputs.make_config(args.config)
+        n_e_job = wl.n_energies()
+    else:
+        from paper_1909_07321_b200 import shard
+        base = inputs.config_shapes(args.config)
+        wl_job = inputs.make_config(args.config, n_E=world * base[0][2])
+        n_e_job = wl_job.n_energies()
+        wl = inputs.Workload(name=wl_job.name, seed=wl_job.seed)
+        for p, idx in shard.plan([w.n_E for w in wl_job.waves], rank, world):
+            w = wl_job.waves[p]
+            wl.waves.append(inputs.Wave(w.W, w.E_k, np.ascontiguousarray(w.energies[idx]), w.a))
     dev_waves, shared = [], {}
     for w in wl.waves:
         key = id(w.energies)
@@ -278,8 +307,8 @@ def run_cuda(args):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     total_ms_max = float(t.item())
     ms_per_step = total_ms_max / args.steps
-    n_e = wl.n_energies()
-    value = world * n_e * args.steps / (total_ms_max * 1e-3)
+    n_e = wl.n_energies()                       # this rank's share
+    value = n_e_job * args.steps / (total_ms_max * 1e-3)
     flop = wl.counted_flop()
 
     # ---- dominant kernel: the persistent DMMA SYRK kernel is the only launch of a step ----
@@ -301,22 +330,27 @@ def run_cuda(args):
                 torch.cuda.synchronize()
                 best = max(best, fl / (e0.elapsed_time(e1) * 1e-3) / 1e12)
             probe[name] = best
-    peak_rule = peaks["bf16"] * FP64_OVER_BF16_NOMINAL       # the other dtype's measured burst peak x nominal ratio
-    t_fp64 = flop / (peak_rule * 1e12)
+    # Peak: the FP64 tensor (DMMA) rate measured live by the probe above (burst, this kernel is timed alone);
+    # MEASURED_PEAKS.json has no FP64 entry.  The guide's rule (another dtype's measured peak x nominal ratio)
+    # gives a LOWER figure because the bf16 measurement is power-limited (1335 MHz) while FP64 runs at 1965 MHz;
+    # the harder denominator is used and the rule-based one is reported beside it.
+    peak_rule = peaks["bf16"] * FP64_OVER_BF16_NOMINAL
+    peak_nominal = 148 * 64 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12      # 64 FP64 FMA/clk/SM (B300_MICROARCH.md), 37.2 TFLOP/s
+    if probe and probe["dmma"] > 0:
+        peak, peak_source = max(probe["dmma"], peak_rule), "DMMA.8x8x4 register-resident probe, measured in this run (burst, best of 5)"
+    else:
+        peak, peak_source = max(peak_nominal, peak_rule), "148 SM x 64 FMA/clk x 2 x sm_max_mhz (no probe on this rank)"
+    t_fp64 = flop / (peak * 1e12)
     t_hbm = wl.r_bytes() / (peaks["hbm_gbs"] * 1e9)
-    roofline = {"bound": "tensor", "achieved": achieved_tflops, "peak": peak_rule, "unit": "TFLOP/s",
-                "frac": achieved_tflops / peak_rule, "traffic": None,
-                "peak_source": f"{peaks['source']} bf16 burst {peaks['bf16']} TFLOP/s x nominal FP64/bf16 ratio 45/2250",
+    roofline = {"bound": "tensor", "achieved": achieved_tflops, "peak": peak, "unit": "TFLOP/s",
+                "frac": achieved_tflops / peak, "traffic": None, "peak_source": peak_source,
+                "peak_rule_bf16_x_ratio": peak_rule, "peak_nominal_fp64": peak_nominal,
                 "kernel": "rmat_persistent_kernel", "flop_per_launch": flop,
                 "t_roof_ms": 1e3 * max(t_fp64, t_hbm), "hbm_write_gbs": wl.r_bytes() / (kern_ms * 1e-3) / 1e9,
                 "hbm_peak_gbs": peaks["hbm_gbs"]}
     if probe:
         roofline["fp64_probe_tflops"] = probe
-        roofline["frac_of_dmma_probe"] = achieved_tflops / probe["dmma"] if probe["dmma"] > 0 else None
-    traffic_file = os.path.join(ROOT, "profiles", f"traffic_config{args.config}.json")
-    if os.path.exists(traffic_file):
-        with open(traffic_file) as f:
-            roofline["traffic"] = json.load(f).get("dram_bytes_per_launch")
+    roofline["traffic"] = ncu_traffic(args.config)
 
     # ---- end to end: HOST buffers through the C ABI, copies inside the timed region ----
     e2e = None
@@ -342,7 +376,7 @@ def run_cuda(args):
         dt = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
         if world > 1:
             dist.all_reduce(dt, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * n_e * e2e_steps / float(dt.item()), "unit": UNIT, "h2d_bytes_per_step": h2d,
+        e2e = {"value": n_e_job * e2e_steps / float(dt.item()), "unit": UNIT, "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "steps": e2e_steps, "ms_per_step": 1e3 * float(dt.item()) / e2e_steps,
                "api": "pstgf_rmat_form_batch_host (pinned host buffers; whole R copied back)"}
         del host
@@ -355,9 +389,10 @@ def run_cuda(args):
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                "config": dict(workload_description(args.config, wl), l2="flushed between timed steps (512 MiB write)",
+                "config": dict(workload_description(args.config, wl), n_energies_per_step=n_e_job, n_energies_per_rank=n_e,
+                               l2="flushed between timed steps (512 MiB write)",
                                sha256=wl.sha256()[:16]),
-                "tflops_counted": world * flop * args.steps / (total_ms_max * 1e-3) / 1e12,
+                "tflops_counted": world * flop * args.steps / (total_ms_max * 1e-3) / 1e12,   # ranks carry equal shares
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,
                 "clocks": clocks, "wall_s_timed_region": wall, "step_ms_min_max": [min(step_ms), max(step_ms)]}
         print(json.dumps(line), flush=True)

@@ -1,0 +1,123 @@
+"""The C-ABI boundary without a GPU: libpstgf_rmat.so loads, exports every symbol that
+include/pstgf_rmat.h declares, the Python binding covers the same names, the struct layout
+matches the header, and argument errors are reported before any CUDA call is made.
+"""
+import ctypes
+import os
+import re
+import subprocess
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "pstgf_rmat.h")
+
+
+def _declared_functions():
+    src = open(HEADER).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)          # drop comments
+    src = re.sub(r"^\s*#.*$", "", src, flags=re.M)            # and preprocessor lines
+    names = re.findall(r"\b(pstgf_[a-z0-9_]+)\s*\(", src)
+    return sorted(set(names))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_1909_07321_b200 import build
+    path = build.build()              # compiles only if missing or stale (nvcc cross-compiles without a GPU)
+    return ctypes.CDLL(path)
+
+
+def test_header_declares_the_boundary_calls():
+    names = _declared_functions()
+    for required in ("pstgf_rmat_form", "pstgf_rmat_form_batch", "pstgf_rmat_batch_workspace_bytes",
+                     "pstgf_status_string", "pstgf_last_cuda_error", "pstgf_version"):
+        assert required in names
+
+
+def test_library_exports_every_declared_symbol(lib):
+    for name in _declared_functions():
+        assert hasattr(lib, name), f"{name} is declared in include/pstgf_rmat.h but not exported"
+
+
+def test_binding_lists_the_same_names():
+    from paper_1909_07321_b200 import rmat
+    assert sorted(rmat.EXPORTS) == _declared_functions()
+    for name in _declared_functions():
+        if name in ("pstgf_last_cuda_error",):
+            continue                                           # surfaced through PstgfError only
+        assert hasattr(rmat, name), f"binding lacks {name}"
+
+
+def test_header_compiles_as_plain_c(tmp_path):
+    """The boundary is C: no C++ or torch types in the signatures."""
+    c = tmp_path / "use_header.c"
+    c.write_text('#include "pstgf_rmat.h"\n'
+                 "int main(void) { pstgf_wave_t w; (void)w; return sizeof(pstgf_wave_t) == 64 ? 0 : 1; }\n")
+    exe = tmp_path / "use_header"
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-pedantic", "-I", os.path.join(ROOT, "include"),
+                    str(c), "-o", str(exe)], check=True)
+    assert subprocess.run([str(exe)]).returncode == 0
+
+
+def test_wave_struct_layout_matches_binding():
+    from paper_1909_07321_b200 import rmat
+    assert ctypes.sizeof(rmat.pstgf_wave_t) == 64
+    off = {n: getattr(rmat.pstgf_wave_t, n).offset for n, _ in rmat.pstgf_wave_t._fields_}
+    assert off == {"n_chan": 0, "n_poles": 4, "n_E": 8, "ldw": 16, "a": 24, "W": 32, "E_k": 40, "energies": 48,
+                   "R_out": 56}
+
+
+def test_version_and_status_strings(lib):
+    lib.pstgf_version.restype = ctypes.c_int
+    lib.pstgf_status_string.restype = ctypes.c_char_p
+    lib.pstgf_status_string.argtypes = [ctypes.c_int]
+    m = re.search(r"#define\s+PSTGF_RMAT_VERSION\s+(\d+)", open(HEADER).read())
+    assert lib.pstgf_version() == int(m.group(1))
+    seen = set()
+    for code in range(6):
+        s = lib.pstgf_status_string(code).decode()
+        assert s and s not in seen
+        seen.add(s)
+    assert b"unknown" in lib.pstgf_status_string(99)
+
+
+def test_argument_errors_need_no_device(lib):
+    """Argument checks come before any CUDA call, so they can be exercised here (no compute)."""
+    vp, ll, i, d = ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int, ctypes.c_double
+    lib.pstgf_rmat_form.argtypes = [vp, ll, vp, vp, i, i, i, d, vp, vp]
+    lib.pstgf_rmat_form.restype = i
+    fake = 4096                                                   # never dereferenced: the call fails first
+    assert lib.pstgf_rmat_form(fake, 6, fake, fake, 4, 6, 1, 0.0, fake, None) == 1      # a <= 0
+    assert lib.pstgf_rmat_form(fake, 5, fake, fake, 4, 6, 1, 20.0, fake, None) == 1     # ldw < n_poles
+    assert lib.pstgf_rmat_form(None, 6, fake, fake, 4, 6, 1, 20.0, fake, None) == 1     # NULL W
+    assert lib.pstgf_rmat_form(fake, 6, fake, fake, -1, 6, 1, 20.0, fake, None) == 1    # negative size
+    assert lib.pstgf_rmat_form(fake + 4, 6, fake, fake, 4, 6, 1, 20.0, fake, None) == 2  # misaligned
+    assert lib.pstgf_rmat_form(fake, 6, fake, fake, 0, 6, 1, 20.0, fake, None) == 0     # n_chan == 0: nothing to do
+    assert lib.pstgf_rmat_form(fake, 6, fake, fake, 4, 6, 0, 20.0, fake, None) == 0     # n_E == 0
+
+
+def test_no_device_is_an_error_not_a_fallback(lib):
+    """On a box without a GPU a well-formed call must fail loudly (there is no CPU path)."""
+    torch = pytest.importorskip("torch")
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    vp, ll, i, d = ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int, ctypes.c_double
+    lib.pstgf_rmat_form.argtypes = [vp, ll, vp, vp, i, i, i, d, vp, vp]
+    lib.pstgf_rmat_form.restype = i
+    assert lib.pstgf_rmat_form(4096, 6, 4096, 4096, 4, 6, 1, 20.0, 4096, None) in (4, 5)
+
+
+def test_product_does_not_touch_the_oracle():
+    """Nothing under the package imports, links or names oracle/ (and vice versa)."""
+    pkg = os.path.join(ROOT, "paper_1909_07321_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in text and "from oracle" not in text and "liboracle" not in text, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c", ".h")):
+            text = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_1909_07321_b200" not in text and "from paper_1909_07321_b200" not in text, f
+            assert "pstgf_rmat.h" not in text and "csrc/" not in text.replace("paper_1909_07321_b200/csrc", ""), f
