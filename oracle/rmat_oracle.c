@@ -85,6 +85,36 @@ int oracle_rmat_form(const double *W, long long ldw, const double *E_k,
     return 0;
 }
 
+/*
+ * The same entries, one at a time: out[s] = R[e_idx[s]][n_idx[s]][m_idx[s]] of eq. 4
+ * for s in [0,n_samples).  For waves too large to evaluate densely
+ * (the paper's 7261 x 106 661 case: one dense energy is 2.8e12 terms)
+ * the parity tests check sampled outputs this way.  Same eq4_entry as above, so every
+ * pin of oracle_rmat_form pins this too (tests check the two agree bitwise).
+ * Returns 0, 1 on bad arguments, 2 on an index out of range.
+ */
+int oracle_rmat_entries(const double *W, long long ldw, const double *E_k,
+                        const double *energies, int n_chan, int n_poles, int n_E,
+                        double a, long long n_samples, const int *e_idx, const int *n_idx,
+                        const int *m_idx, double *out, int threads)
+{
+    if (n_chan < 0 || n_poles < 0 || n_E < 0 || ldw < n_poles || n_samples < 0) return 1;
+    if (n_samples == 0) return 0;
+    if ((!W && n_poles > 0) || !energies || !e_idx || !n_idx || !m_idx || !out) return 1;
+    for (long long s = 0; s < n_samples; ++s)
+        if (e_idx[s] < 0 || e_idx[s] >= n_E || n_idx[s] < 0 || n_idx[s] >= n_chan ||
+            m_idx[s] < 0 || m_idx[s] >= n_chan)
+            return 2;
+    (void)threads;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(dynamic, 16) num_threads(threads > 1 ? threads : 1)
+#endif
+    for (long long s = 0; s < n_samples; ++s)
+        out[s] = eq4_entry(W + (size_t)n_idx[s] * ldw, W + (size_t)m_idx[s] * ldw, E_k, n_poles,
+                           energies[e_idx[s]], a);
+    return 0;
+}
+
 /* Threads the OpenMP runtime would use by default (for reporting "cores"). */
 int oracle_max_threads(void)
 {

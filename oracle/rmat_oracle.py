@@ -39,6 +39,10 @@ def _load():
         lib.oracle_rmat_form.argtypes = [dp, ctypes.c_longlong, dp, dp, ctypes.c_int, ctypes.c_int,
                                          ctypes.c_int, ctypes.c_double, dp, ctypes.c_int]
         lib.oracle_rmat_form.restype = ctypes.c_int
+        ip = ctypes.POINTER(ctypes.c_int)
+        lib.oracle_rmat_entries.argtypes = [dp, ctypes.c_longlong, dp, dp, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                            ctypes.c_double, ctypes.c_longlong, ip, ip, ip, dp, ctypes.c_int]
+        lib.oracle_rmat_entries.restype = ctypes.c_int
         lib.oracle_max_threads.argtypes = []
         lib.oracle_max_threads.restype = ctypes.c_int
         _lib = lib
@@ -73,6 +77,32 @@ def rmat_form(W, E_k, energies, a: float, threads: int = 1) -> np.ndarray:
     if rc != 0:
         raise ValueError(f"oracle_rmat_form rejected its arguments (rc={rc})")
     return R
+
+
+def rmat_entries(W, E_k, energies, a: float, e_idx, n_idx, m_idx, threads: int = 1) -> np.ndarray:
+    """R[e_idx[s], n_idx[s], m_idx[s]] of eq. 4, entry by entry (for waves too large to form densely).
+
+    W must already be a C-contiguous float64 array: it is NOT copied (6.2 GB at the paper's scale).
+    """
+    if not (isinstance(W, np.ndarray) and W.dtype == np.float64 and W.flags.c_contiguous and W.ndim == 2):
+        raise ValueError("W must be a C-contiguous float64 [n_chan, n_poles] array")
+    E_k = np.ascontiguousarray(E_k, dtype=np.float64)
+    energies = np.ascontiguousarray(energies, dtype=np.float64)
+    if E_k.ndim != 1 or energies.ndim != 1 or W.shape[1] != E_k.shape[0]:
+        raise ValueError("shape mismatch: W [n_chan, n_poles], E_k [n_poles], energies [n_E]")
+    idx = [np.ascontiguousarray(x, dtype=np.int32) for x in (e_idx, n_idx, m_idx)]
+    if not (idx[0].ndim == 1 and idx[0].shape == idx[1].shape == idx[2].shape):
+        raise ValueError("e_idx, n_idx, m_idx must be 1-D and of equal length")
+    n_chan, n_poles = W.shape
+    out = np.zeros(idx[0].shape[0], dtype=np.float64)
+    ip = ctypes.POINTER(ctypes.c_int)
+    rc = _load().oracle_rmat_entries(_dptr(W), n_poles, _dptr(E_k), _dptr(energies), n_chan, n_poles,
+                                     energies.shape[0], float(a), out.shape[0],
+                                     idx[0].ctypes.data_as(ip), idx[1].ctypes.data_as(ip), idx[2].ctypes.data_as(ip),
+                                     _dptr(out), int(threads))
+    if rc != 0:
+        raise ValueError(f"oracle_rmat_entries rejected its arguments (rc={rc})")
+    return out
 
 
 def rmat_form_batch(waves, threads: int = 1) -> list[np.ndarray]:

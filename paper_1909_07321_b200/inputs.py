@@ -80,7 +80,7 @@ class Workload:
         h = hashlib.sha256()
         for w in self.waves:
             for arr in (w.W, w.E_k, w.energies):
-                h.update(np.ascontiguousarray(arr).tobytes())
+                h.update(memoryview(np.ascontiguousarray(arr)).cast("B"))   # no 6 GB copy at paper scale
             h.update(np.float64(w.a).tobytes())
         return h.hexdigest()
 
@@ -177,8 +177,17 @@ _CONFIGS = {
     3: dict(seed=2, P=8, C=256, N=2048, a=25.0, sigma=0.05, poles=(-20.0, 200.0), mesh=(0.05, 30.0), kind="linear"),
     4: dict(seed=3, P=32, C=None, N=512, a=25.0, sigma=0.05, poles=(-20.0, 300.0), mesh=(0.01, 50.0), kind="geometric"),
     5: dict(seed=4, P=1, C=512, N=256, a=30.0, sigma=0.03, poles=(-30.0, 400.0), mesh=(0.01, 60.0), kind="linear"),
+    # Not in BASELINE.json: the one workload the paper times for this path, "7261 channels and a
+    # Hamiltonian size of 106 661" (neutral Fe).  W is 6.2 GB, R 422 MB per energy.
+    6: dict(seed=5, P=1, C=7261, K=106661, N=16, a=30.0, sigma=0.03, poles=(-30.0, 2000.0), mesh=(0.01, 10.0),
+            kind="linear"),
 }
 POLES_PER_CHANNEL = 20
+PAPER_SCALE_CONFIG = 6
+
+
+def _n_poles(c: dict, n_chan: int) -> int:
+    return int(c["K"]) if "K" in c else POLES_PER_CHANNEL * n_chan
 
 
 def config_shapes(cfg: int, seed: int | None = None) -> list[tuple[int, int, int]]:
@@ -189,11 +198,11 @@ def config_shapes(cfg: int, seed: int | None = None) -> list[tuple[int, int, int
         chans = [int(x) for x in rng.integers(16, 401, size=c["P"])]
     else:
         chans = [c["C"]] * c["P"]
-    return [(n, POLES_PER_CHANNEL * n, c["N"]) for n in chans]
+    return [(n, _n_poles(c, n), c["N"]) for n in chans]
 
 
 def make_config(cfg: int, seed: int | None = None, n_E: int | None = None) -> Workload:
-    """Build BASELINE.json config ``cfg`` (1..5).
+    """Build BASELINE.json config ``cfg`` (1..5), or 6: the paper-scale wave of PAPER.md:168.
 
     Draw order (reading R12): config 4 first draws all n_chan; then per wave,
     in order, W (row-major fill) and then E_k.  ``n_E`` overrides the mesh
@@ -207,7 +216,7 @@ def make_config(cfg: int, seed: int | None = None, n_E: int | None = None) -> Wo
         chans = [int(x) for x in rng.integers(16, 401, size=c["P"])]
     else:
         chans = [c["C"]] * c["P"]
-    drawn = [_draw_wave(rng, n, POLES_PER_CHANNEL * n, c["sigma"], *c["poles"]) for n in chans]
+    drawn = [_draw_wave(rng, n, _n_poles(c, n), c["sigma"], *c["poles"]) for n in chans]
     mesh_fn = linear_mesh if c["kind"] == "linear" else geometric_mesh
     mesh = mesh_fn(c["mesh"][0], c["mesh"][1], N)
     wl = Workload(name=f"config{cfg}", seed=s)

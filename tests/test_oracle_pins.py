@@ -279,3 +279,24 @@ def test_compensation_is_live(oracle):
     for t in 1.0 / E_k:
         plain += t
     assert plain != float(exact)  # the pin would be vacuous otherwise
+
+
+def test_entries_agree_with_dense_and_exact(oracle):
+    """oracle_rmat_entries (sampled outputs of waves too large to form densely) is the dense routine's
+    eq4_entry: bitwise equal to it, and pinned on its own against the exact rational value."""
+    rng = np.random.default_rng(31)
+    C, K, N = 5, 7, 3
+    W = rng.normal(0, 0.1, (C, K))
+    E_k = np.sort(rng.uniform(-5, 50, K))
+    en = np.array([0.3, 4.4, 9.1])
+    R = oracle.rmat_form(W, E_k, en, 20.0)
+    e, n, m = np.meshgrid(np.arange(N), np.arange(C), np.arange(C), indexing="ij")
+    got = oracle.rmat_entries(W, E_k, en, 20.0, e.ravel(), n.ravel(), m.ravel(), threads=3)
+    assert np.array_equal(got.reshape(N, C, C), R)
+    exact = _exact_eq4(W, E_k, en, 20.0)
+    assert np.abs(got.reshape(N, C, C) - exact).max() <= 64 * np.finfo(float).eps * np.abs(exact).max()
+    with pytest.raises(ValueError):
+        oracle.rmat_entries(W, E_k, en, 20.0, [3], [0], [0])          # energy index out of range
+    with pytest.raises(ValueError):
+        oracle.rmat_entries(W, E_k, en, 20.0, [0], [0], [C])
+    assert oracle.rmat_entries(W, E_k, en, 20.0, [], [], []).shape == (0,)
