@@ -131,12 +131,16 @@ pstgf_status_t pstgf_rmat_form_naive(const double *W, long long ldw, const doubl
 
 /*
  * End-to-end convenience over HOST buffers: `waves` holds HOST pointers
- * (pinned memory recommended).  Inputs are copied to the device, R is formed
- * in chunks of energies and copied back into the host R_out while the next
- * chunk is computed.  Allocates device memory from the stream-ordered pool of
- * the current device for the duration of the call and SYNCHRONISES before
- * returning.  `max_chunk_bytes` bounds the device R staging per chunk
- * (0 = default 256 MiB; two chunks are in flight).
+ * (pinned memory recommended; pageable memory works but copies synchronously).
+ * Inputs are copied to the device on `stream`, R is formed in chunks of whole
+ * energy blocks on two streams of the library's own and copied back into the
+ * host R_out on a third while the next chunks are being formed (three staging
+ * buffers in flight).  Device memory comes from a stream-ordered pool the
+ * library owns (one per device, kept for the life of the process so that
+ * repeated calls do not re-grow it).  SYNCHRONISES before returning.
+ * `max_chunk_bytes` bounds the device R staging per chunk (0 = default: one
+ * eighth of all R, clamped to [16 MiB, 256 MiB]); a chunk always holds at
+ * least one energy block.
  */
 pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves,
                                           size_t max_chunk_bytes, void *stream);

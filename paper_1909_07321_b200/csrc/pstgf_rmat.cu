@@ -272,19 +272,53 @@ pstgf_status_t pstgf_rmat_form_naive(const double *W, long long ldw, const doubl
 
 // ---- end-to-end call over HOST buffers ---------------------------------------------------------
 namespace {
+constexpr int HOST_RING = 3;          // R staging buffers in flight
+constexpr int HOST_COMPUTE_STREAMS = 2;
+
+// Device memory of the host call comes from a pool the library owns (one per device, kept for the life of
+// the process, release threshold = never): the default pool hands its memory back at every synchronise,
+// and re-growing it costs tens of milliseconds per call.
+std::mutex g_pool_mutex;
+cudaMemPool_t g_pool[64] = {nullptr};
+
+cudaError_t host_call_pool(int dev, cudaMemPool_t *out) {
+  std::lock_guard<std::mutex> lock(g_pool_mutex);
+  if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+  if (!g_pool[dev]) {
+    cudaMemPoolProps props;
+    std::memset(&props, 0, sizeof(props));
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = dev;
+    cudaMemPool_t pool;
+    cudaError_t e = cudaMemPoolCreate(&pool, &props);
+    if (e != cudaSuccess) return e;
+    unsigned long long keep = ~0ULL;
+    e = cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    if (e != cudaSuccess) { cudaMemPoolDestroy(pool); return e; }
+    g_pool[dev] = pool;
+  }
+  *out = g_pool[dev];
+  return cudaSuccess;
+}
+
 struct HostCallResources {
-  cudaStream_t s = nullptr, copy = nullptr;
-  cudaEvent_t computed[2] = {nullptr, nullptr}, copied[2] = {nullptr, nullptr};
+  cudaStream_t s = nullptr, copy = nullptr, compute[HOST_COMPUTE_STREAMS] = {nullptr, nullptr};
+  cudaEvent_t inputs = nullptr, computed[HOST_RING] = {nullptr}, copied[HOST_RING] = {nullptr};
   std::vector<void *> allocs;
   ~HostCallResources() {
+    for (cudaStream_t c : compute) if (c) cudaStreamSynchronize(c);
     if (copy) cudaStreamSynchronize(copy);
     cudaStreamSynchronize(s);
     for (void *p : allocs) cudaFreeAsync(p, s);
     cudaStreamSynchronize(s);
-    for (int b = 0; b < 2; ++b) {
+    if (inputs) cudaEventDestroy(inputs);
+    for (int b = 0; b < HOST_RING; ++b) {
       if (computed[b]) cudaEventDestroy(computed[b]);
       if (copied[b]) cudaEventDestroy(copied[b]);
     }
+    for (cudaStream_t c : compute) if (c) cudaStreamDestroy(c);
     if (copy) cudaStreamDestroy(copy);
   }
 };
@@ -296,23 +330,32 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
   if (n_waves < 0) return PSTGF_ERR_INVALID_VALUE;
   if (n_waves == 0) return PSTGF_OK;
   if (!waves) return PSTGF_ERR_INVALID_VALUE;
+  size_t total_r = 0;
   for (int p = 0; p < n_waves; ++p) {
     pstgf_status_t st = check_wave(waves[p]);
     if (st != PSTGF_OK) return st;
+    if (wave_has_items(waves[p])) total_r += sizeof(double) * (size_t)waves[p].n_E * waves[p].n_chan * waves[p].n_chan;
   }
   DeviceState ds;
   pstgf_status_t st = device_state(ds);
   if (st != PSTGF_OK) return st;
-  const size_t cap = max_chunk_bytes ? max_chunk_bytes : ((size_t)256 << 20);
+  // chunk size: about eight chunks per call so that the copy-back of one hides behind the formation of the
+  // next ones, never below 16 MiB (launch and tail overheads) nor above 256 MiB (device footprint)
+  size_t cap = max_chunk_bytes;
+  if (!cap) cap = std::min<size_t>((size_t)256 << 20, std::max<size_t>((size_t)16 << 20, total_r / 8));
   HostCallResources res;
   res.s = static_cast<cudaStream_t>(stream);
+  cudaMemPool_t pool;
+  PSTGF_CUDA(host_call_pool(ds.device, &pool));
   PSTGF_CUDA(cudaStreamCreateWithFlags(&res.copy, cudaStreamNonBlocking));
-  for (int b = 0; b < 2; ++b) {
+  for (cudaStream_t &c : res.compute) PSTGF_CUDA(cudaStreamCreateWithFlags(&c, cudaStreamNonBlocking));
+  PSTGF_CUDA(cudaEventCreateWithFlags(&res.inputs, cudaEventDisableTiming));
+  for (int b = 0; b < HOST_RING; ++b) {
     PSTGF_CUDA(cudaEventCreateWithFlags(&res.computed[b], cudaEventDisableTiming));
     PSTGF_CUDA(cudaEventCreateWithFlags(&res.copied[b], cudaEventDisableTiming));
   }
   auto dev_alloc = [&](size_t bytes, void **out) -> cudaError_t {
-    cudaError_t e = cudaMallocAsync(out, bytes ? bytes : 8, res.s);
+    cudaError_t e = cudaMallocFromPoolAsync(out, bytes ? bytes : 8, pool, res.s);
     if (e == cudaSuccess) res.allocs.push_back(*out);
     return e;
   };
@@ -369,17 +412,23 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
   }
   if (chunks.back().empty()) chunks.pop_back();
   if (chunks.empty()) return PSTGF_OK;
-  void *rbuf[2], *wsbuf[2];
+  const int ring = (int)std::min<size_t>(HOST_RING, chunks.size());
+  void *rbuf[HOST_RING], *wsbuf[HOST_RING];
   const size_t wsb = ws_bytes((int)max_segs);
-  for (int b = 0; b < 2; ++b) {
+  for (int b = 0; b < ring; ++b) {
     PSTGF_CUDA(dev_alloc(max_chunk, &rbuf[b]));
     PSTGF_CUDA(dev_alloc(wsb, &wsbuf[b]));
   }
+  // the formation kernels run on two streams of the library's own, so that the first CTAs of chunk c+1 start on
+  // the SMs the tail of chunk c has left; both wait for the inputs (and the allocations) enqueued on `stream`
+  PSTGF_CUDA(cudaEventRecord(res.inputs, res.s));
+  for (cudaStream_t c : res.compute) PSTGF_CUDA(cudaStreamWaitEvent(c, res.inputs, 0));
   int launches = 0;
   std::vector<pstgf_wave_t> sub;
   for (size_t c = 0; c < chunks.size(); ++c) {
-    const int b = (int)(c & 1);
-    if (c >= 2) PSTGF_CUDA(cudaStreamWaitEvent(res.s, res.copied[b], 0));
+    const int b = (int)(c % ring);
+    cudaStream_t cs = res.compute[c % HOST_COMPUTE_STREAMS];
+    if (c >= (size_t)ring) PSTGF_CUDA(cudaStreamWaitEvent(cs, res.copied[b], 0));
     sub.clear();
     for (const Segment &g : chunks[c]) {
       pstgf_wave_t w = dev[g.wave];
@@ -388,10 +437,10 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
       w.R_out = reinterpret_cast<double *>(static_cast<unsigned char *>(rbuf[b]) + g.off);
       sub.push_back(w);
     }
-    st = pstgf_rmat_form_batch(sub.data(), (int)sub.size(), wsbuf[b], wsb, res.s);
+    st = pstgf_rmat_form_batch(sub.data(), (int)sub.size(), wsbuf[b], wsb, cs);
     if (st != PSTGF_OK) return st;
     launches += tl_launches;
-    PSTGF_CUDA(cudaEventRecord(res.computed[b], res.s));
+    PSTGF_CUDA(cudaEventRecord(res.computed[b], cs));
     PSTGF_CUDA(cudaStreamWaitEvent(res.copy, res.computed[b], 0));
     for (const Segment &g : chunks[c]) {
       const pstgf_wave_t &w = waves[g.wave];
@@ -402,6 +451,7 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
     PSTGF_CUDA(cudaEventRecord(res.copied[b], res.copy));
   }
   PSTGF_CUDA(cudaStreamSynchronize(res.copy));
+  for (cudaStream_t c : res.compute) PSTGF_CUDA(cudaStreamSynchronize(c));
   PSTGF_CUDA(cudaStreamSynchronize(res.s));
   tl_launches = launches;
   return PSTGF_OK;
