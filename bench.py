@@ -412,9 +412,11 @@ def run_cuda(args):
         rmat.pstgf_rmat_form_batch_host(host)        # warm-up (allocator pool, pinned pages)
         barrier()
         t0 = time.perf_counter()
-        e2e_launches = 0
+        e2e_launches, e2e_ms = 0, []
         for _ in range(e2e_steps):
+            t1 = time.perf_counter()
             rmat.pstgf_rmat_form_batch_host(host)    # synchronises before returning
+            e2e_ms.append(1e3 * (time.perf_counter() - t1))
             e2e_launches += rmat.pstgf_last_launch_count()
         torch.cuda.synchronize()
         dt = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
@@ -422,6 +424,7 @@ def run_cuda(args):
             dist.all_reduce(dt, op=dist.ReduceOp.MAX)
         e2e = {"value": n_e_job * e2e_steps / float(dt.item()), "unit": UNIT, "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "steps": e2e_steps, "ms_per_step": 1e3 * float(dt.item()) / e2e_steps,
+               "step_ms_min_max": [min(e2e_ms), max(e2e_ms)], "gpu_launches": e2e_launches,
                "api": "pstgf_rmat_form_batch_host (pinned host buffers; whole R copied back)"}
         del host
 

@@ -19,8 +19,9 @@
  * Conventions for every call
  *  - Pointers named in "DEVICE" lists are device pointers owned by the caller
  *    (allocate them with any CUDA allocator, e.g. PyTorch).  The library
- *    allocates no device memory in the DEVICE-pointer calls; the batch call
- *    keeps its tables in the caller's workspace.
+ *    allocates no device memory in the DEVICE-pointer calls (but for the 8 KiB
+ *    counter pool of pstgf_rmat_form, once per device); the batch call keeps
+ *    its tables in the caller's workspace.
  *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default
  *    stream).  DEVICE-pointer calls enqueue work and return without
  *    synchronising; buffers must stay alive until the stream reaches the end
@@ -54,7 +55,7 @@
 extern "C" {
 #endif
 
-#define PSTGF_RMAT_VERSION 100 /* major*100 + minor */
+#define PSTGF_RMAT_VERSION 101 /* major*100 + minor */
 
 typedef enum {
   PSTGF_OK = 0,
@@ -91,11 +92,32 @@ typedef struct {
  *   a                        R-matrix radius r0 in a.u., finite and > 0
  *   R_out    [n_E][n_chan][n_chan]
  * One persistent kernel launch (plus a zero-fill when n_poles == 0); work
- * items (energy block, upper-triangle tile) are assigned to CTAs round-robin.
+ * items (energy block, upper-triangle tile) are drawn by the CTAs from an
+ * atomic counter.  The counter lives in a pool of 64 slots (8 KiB of device
+ * memory per device, allocated by the library at the first call -- the only
+ * device allocation of the DEVICE-pointer calls); when 64 launches are in
+ * flight at once, or `stream` is being captured into a CUDA graph, items are
+ * assigned round-robin instead.  Results do not depend on the assignment.
  */
 pstgf_status_t pstgf_rmat_form(const double *W, long long ldw, const double *E_k,
                                const double *energies, int n_chan, int n_poles, int n_E,
                                double a, double *R_out, void *stream);
+
+/*
+ * Scheduling knob (process-wide; meant for tests and measurements).  Work
+ * items are handed to the persistent CTAs largest first; the END of that list
+ * -- about one round of the grid's worth of work -- is cut into finer tiles
+ * (32-row instead of 64-row) so that the CTAs run dry together, the device-
+ * side counterpart of the paper's concern that no processor be left waiting
+ * (Fig. 1).  PSTGF_TAIL_AUTO (default) sizes that tail
+ * itself, PSTGF_TAIL_NONE uses coarse tiles only, PSTGF_TAIL_ALL fine tiles
+ * only.  Every R element has the same operands and summation order under all
+ * three policies: results are bitwise identical.
+ */
+#define PSTGF_TAIL_AUTO 0
+#define PSTGF_TAIL_NONE 1
+#define PSTGF_TAIL_ALL 2
+pstgf_status_t pstgf_rmat_set_tail_policy(int policy);
 
 /*
  * Bytes of device workspace pstgf_rmat_form_batch needs for these waves

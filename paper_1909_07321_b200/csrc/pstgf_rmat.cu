@@ -5,6 +5,7 @@
 #include <cuda.h>
 
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstring>
 #include <mutex>
@@ -98,7 +99,9 @@ pstgf_status_t check_wave(const pstgf_wave_t &w) {
 }
 
 // ---- planner -------------------------------------------------------------------------------
-// Fills everything of DevWave except the tensor map.
+std::atomic<int> g_tail_policy{PSTGF_TAIL_AUTO};
+
+// Fills everything of DevWave except the tensor map; every energy block starts out coarse.
 void plan_wave(const pstgf_wave_t &w, DevWave &d) {
   std::memset(&d, 0, sizeof(d));
   d.W = w.W;
@@ -117,13 +120,50 @@ void plan_wave(const pstgf_wave_t &w, DevWave &d) {
   int tiles = d.n_i;
   for (int i = 0; i < d.n_i; ++i) tiles += pstgf::off_tiles_in_row(d.n_j, i);
   d.n_tiles = tiles;
+  d.n_eb_coarse = d.n_eb;
   d.use_tma = ((reinterpret_cast<uintptr_t>(w.W) & 15u) == 0 && (w.ldw % 2) == 0 && w.ldw * 8 < (1LL << 40)) ? 1 : 0;
 }
 
-long long wave_items(const DevWave &d) { return (long long)d.n_tiles * d.n_eb; }
+long long coarse_items(const DevWave &d) { return (long long)d.n_tiles * d.n_eb_coarse; }
+long long fine_items(const DevWave &d) { return (long long)pstgf::fine_tiles(d.n_j) * (d.n_eb - d.n_eb_coarse); }
+long long wave_items(const DevWave &d) { return coarse_items(d) + fine_items(d); }
 
 // Relative cost of a wave's items, for the largest-first order of the batch.
 double wave_item_cost(const pstgf_wave_t &w) { return (double)std::min(w.n_chan, pstgf::TM) * w.n_poles; }
+
+// Cost model in DMMA.8x8x4 per energy (full-size tiles; good enough to size the tail).
+double largest_item_cost(const DevWave &d) {
+  const int nb = std::min((d.n_chan + 7) / 8, pstgf::TM / 8);
+  return (double)d.n_kt * (nb * (nb + 1) / 2);
+}
+double cost_per_energy_block(const DevWave &d) {
+  return (double)d.n_kt * ((double)d.n_i * pstgf::COST_DIAG + (double)(d.n_tiles - d.n_i) * pstgf::COST_OFF);
+}
+
+// Tail of the schedule (see rmat_common.h): about one round of the grid's worth of work, taken from the
+// END of the largest-first order, is cut into fine tiles so that list scheduling finishes on small items.
+void plan_tails(std::vector<DevWave> &ds, int grid) {
+  const int policy = g_tail_policy.load();
+  if (policy == PSTGF_TAIL_NONE) return;
+  if (policy == PSTGF_TAIL_ALL) {
+    for (DevWave &d : ds) d.n_eb_coarse = 0;
+    return;
+  }
+  double c_max = 0.0;
+  for (const DevWave &d : ds) c_max = std::max(c_max, largest_item_cost(d));
+  double budget = c_max * grid;
+  for (size_t q = ds.size(); q-- > 0 && budget > 0.0;) {
+    DevWave &d = ds[q];
+    const double per_eb = cost_per_energy_block(d);
+    if (largest_item_cost(d) <= 0.45 * c_max) {   // a small wave at the end of the list: its coarse items are fine enough
+      budget -= d.n_eb * per_eb;
+      continue;
+    }
+    const int t = (int)std::min<double>((double)d.n_eb, std::ceil(budget / per_eb));
+    d.n_eb_coarse = d.n_eb - t;
+    budget -= t * per_eb;
+  }
+}
 
 pstgf_status_t encode_map(DevWave &d) {
   if (!d.use_tma) return PSTGF_OK;
@@ -153,12 +193,75 @@ pstgf_status_t zero_fill(const pstgf_wave_t &w, cudaStream_t s) {
 
 // workspace layout of the batch call
 constexpr size_t WS_COUNTER_BYTES = 256;
-size_t ws_item_begin_bytes(int n_waves) { return (((size_t)n_waves + 1) * sizeof(long long) + 255) & ~(size_t)255; }
+size_t ws_item_begin_bytes(int n_waves) { return ((2 * (size_t)n_waves + 1) * sizeof(long long) + 255) & ~(size_t)255; }
 size_t ws_bytes(int n_waves) { return WS_COUNTER_BYTES + ws_item_begin_bytes(n_waves) + (size_t)n_waves * sizeof(DevWave); }
+
+// ---- work counters of the single-wave call ---------------------------------------------------
+// pstgf_rmat_form has no workspace argument, so its atomic work counter comes from a small pool the library
+// keeps per device (COUNTER_SLOTS x 128 B, allocated at first use).  A slot is handed to one launch at a time:
+// an event recorded behind the launch tells when it is free again (the kernel's last CTA zeroes it).  With no
+// free slot, or under stream capture, the launch falls back to round-robin item assignment.
+constexpr int COUNTER_SLOTS = 64;
+struct CounterPool {
+  unsigned long long *base = nullptr;
+  cudaEvent_t ev[COUNTER_SLOTS] = {nullptr};
+  bool armed[COUNTER_SLOTS] = {false};
+  int next = 0;
+};
+std::mutex g_counter_mutex;
+CounterPool g_counters[64];
+
+// Called with g_counter_mutex held.  Returns the slot or -1.
+int acquire_counter(int dev, cudaStream_t s, unsigned long long **out) {
+  if (dev < 0 || dev >= 64) return -1;
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(s, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone) {
+    (void)cudaGetLastError();
+    return -1;
+  }
+  CounterPool &cp = g_counters[dev];
+  if (!cp.base) {
+    void *p = nullptr;
+    if (cudaMalloc(&p, COUNTER_SLOTS * 128) != cudaSuccess || cudaMemset(p, 0, COUNTER_SLOTS * 128) != cudaSuccess) {
+      (void)cudaGetLastError();
+      if (p) cudaFree(p);
+      return -1;
+    }
+    for (int i = 0; i < COUNTER_SLOTS; ++i) {
+      if (cudaEventCreateWithFlags(&cp.ev[i], cudaEventDisableTiming) != cudaSuccess) {
+        (void)cudaGetLastError();
+        for (int k = 0; k < i; ++k) cudaEventDestroy(cp.ev[k]);
+        cudaFree(p);
+        return -1;
+      }
+    }
+    cp.base = static_cast<unsigned long long *>(p);
+  }
+  for (int t = 0; t < COUNTER_SLOTS; ++t) {
+    const int slot = (cp.next + t) % COUNTER_SLOTS;
+    if (cp.armed[slot]) {
+      if (cudaEventQuery(cp.ev[slot]) != cudaSuccess) {
+        (void)cudaGetLastError();
+        continue;                                   // that launch has not finished yet
+      }
+      cp.armed[slot] = false;
+    }
+    cp.next = (slot + 1) % COUNTER_SLOTS;
+    *out = cp.base + (size_t)slot * 16;
+    return slot;
+  }
+  return -1;
+}
 
 }  // namespace
 
 extern "C" {
+
+pstgf_status_t pstgf_rmat_set_tail_policy(int policy) {
+  if (policy != PSTGF_TAIL_AUTO && policy != PSTGF_TAIL_NONE && policy != PSTGF_TAIL_ALL) return PSTGF_ERR_INVALID_VALUE;
+  g_tail_policy.store(policy);
+  return PSTGF_OK;
+}
 
 pstgf_status_t pstgf_rmat_form(const double *W, long long ldw, const double *E_k, const double *energies, int n_chan,
                                int n_poles, int n_E, double a, double *R_out, void *stream) {
@@ -172,15 +275,26 @@ pstgf_status_t pstgf_rmat_form(const double *W, long long ldw, const double *E_k
   if (st != PSTGF_OK) return st;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   if (n_poles == 0) return zero_fill(w, s);
-  DevWave d;
-  plan_wave(w, d);
-  st = encode_map(d);
+  std::vector<DevWave> d(1);
+  plan_wave(w, d[0]);
+  plan_tails(d, ds.sm_count);
+  st = encode_map(d[0]);
   if (st != PSTGF_OK) return st;
-  const long long n_items = wave_items(d);
+  const long long n_items = wave_items(d[0]);
   const int grid = (int)std::min<long long>(ds.sm_count, n_items);
-  pstgf::rmat_persistent_kernel<false><<<grid, pstgf::NUM_THREADS, pstgf::SMEM_BYTES, s>>>(d, nullptr, nullptr, 1,
-                                                                                         n_items, nullptr);
-  PSTGF_CUDA(cudaGetLastError());
+  {
+    std::lock_guard<std::mutex> lock(g_counter_mutex);
+    unsigned long long *counter = nullptr;
+    const int slot = acquire_counter(ds.device, s, &counter);
+    pstgf::rmat_persistent_kernel<false><<<grid, pstgf::NUM_THREADS, pstgf::SMEM_BYTES, s>>>(d[0], nullptr, nullptr, 1,
+                                                                                           n_items, counter);
+    PSTGF_CUDA(cudaGetLastError());
+    if (slot >= 0) {
+      CounterPool &cp = g_counters[ds.device];
+      PSTGF_CUDA(cudaEventRecord(cp.ev[slot], s));
+      cp.armed[slot] = true;
+    }
+  }
   tl_launches = 1;
   return PSTGF_OK;
 }
@@ -202,8 +316,8 @@ pstgf_status_t pstgf_rmat_form_batch(const pstgf_wave_t *waves, int n_waves, voi
   }
   if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) != 0 || workspace_bytes < ws_bytes(n_waves))
     return PSTGF_ERR_WORKSPACE;
-  DeviceState ds;
-  pstgf_status_t st = device_state(ds);
+  DeviceState dstate;
+  pstgf_status_t st = device_state(dstate);
   if (st != PSTGF_OK) return st;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   int launches = 0;
@@ -221,24 +335,30 @@ pstgf_status_t pstgf_rmat_form_batch(const pstgf_wave_t *waves, int n_waves, voi
   std::stable_sort(order.begin(), order.end(),
                    [&](int x, int y) { return wave_item_cost(waves[x]) > wave_item_cost(waves[y]); });
   const int nw = (int)order.size();
-  // host image of the workspace: [counter | item_begin[nw+1] | DevWave[nw]]
+  // host image of the workspace: [counter | item_begin[2 nw + 1] | DevWave[nw]]; item sections are the coarse
+  // items of every wave (largest first), then the fine items of every wave
   const size_t off_begin = WS_COUNTER_BYTES, off_waves = WS_COUNTER_BYTES + ws_item_begin_bytes(n_waves);
   std::vector<unsigned char> img(off_waves + (size_t)nw * sizeof(DevWave), 0);
   long long *item_begin = reinterpret_cast<long long *>(img.data() + off_begin);
+  std::vector<DevWave> ds((size_t)nw);
+  for (int q = 0; q < nw; ++q) plan_wave(waves[order[q]], ds[q]);
+  plan_tails(ds, dstate.sm_count);
   long long total = 0;
   for (int q = 0; q < nw; ++q) {
-    DevWave d;
-    plan_wave(waves[order[q]], d);
-    st = encode_map(d);
+    st = encode_map(ds[q]);
     if (st != PSTGF_OK) return st;
-    std::memcpy(img.data() + off_waves + (size_t)q * sizeof(DevWave), &d, sizeof(DevWave));
+    std::memcpy(img.data() + off_waves + (size_t)q * sizeof(DevWave), &ds[q], sizeof(DevWave));
     item_begin[q] = total;
-    total += wave_items(d);
+    total += coarse_items(ds[q]);
   }
-  item_begin[nw] = total;
+  for (int q = 0; q < nw; ++q) {
+    item_begin[nw + q] = total;
+    total += fine_items(ds[q]);
+  }
+  item_begin[2 * nw] = total;
   unsigned char *ws = static_cast<unsigned char *>(workspace);
   PSTGF_CUDA(cudaMemcpyAsync(ws, img.data(), img.size(), cudaMemcpyHostToDevice, s));
-  const int grid = (int)std::min<long long>(ds.sm_count, total);
+  const int grid = (int)std::min<long long>(dstate.sm_count, total);
   DevWave dummy;
   std::memset(&dummy, 0, sizeof(dummy));
   pstgf::rmat_persistent_kernel<true><<<grid, pstgf::NUM_THREADS, pstgf::SMEM_BYTES, s>>>(

@@ -4,11 +4,19 @@
 //
 // Work decomposition of eq. 4 for one partial wave with C = n_chan,
 // K = n_poles, N = n_E:
-//   tile kinds   DIAG(i)    rows/cols [64 i, 64 i + 64): upper triangle of 8x8 DMMA blocks
+//   coarse tiles DIAG(i)    rows/cols [64 i, 64 i + 64): upper triangle of 8x8 DMMA blocks
 //                OFF(i, j)  rows [64 i, 64 i + 64) x cols [32 j, 32 j + 32), j >= 2 i + 2
+//   fine tiles   OFF32(i,j) rows [32 i, 32 i + 32) x cols [32 j, 32 j + 32), j > i
+//                DIAG32(i)  rows/cols [32 i, 32 i + 32)
 //   energy block EB = 8 consecutive energies, one per consumer warp
-//   item         (wave, tile, energy block); item index inside a wave = tile * n_eb + eb
-//                (energy-fastest: CTAs running side by side share one W tile in L2)
+//   item         (wave, tile, energy block).  The first n_eb_coarse energy blocks of a wave are cut
+//                into coarse tiles, the remaining ones (the "tail", sized by the planner to about one
+//                round of the grid) into fine tiles of 16/36 and 10/36 of a coarse item's cost, and all
+//                fine items are handed out after all coarse ones: largest-first list scheduling ends
+//                on small items, so the CTAs finish together.  Inside a section the item index is
+//                tile * n_eb_section + eb (energy-fastest: CTAs running side by side share one W tile
+//                in L2).  An R element has the same operands and k order in both tilings (bitwise
+//                the same result).
 // Only tiles on or above the diagonal exist ("half of the symmetric R-matrix"),
 // the mirror is written by the epilogue ("symmetrised").
 #pragma once
@@ -50,9 +58,9 @@ struct alignas(128) DevWave {
   int n_i;                 // ceil(n_chan / TM): DIAG tiles
   int n_j;                 // ceil(n_chan / TN)
   int n_eb;                // ceil(n_E / EB)
-  int n_tiles;             // n_i + number of OFF tiles
+  int n_tiles;             // n_i + number of coarse OFF tiles
   int use_tma;             // W 16-byte aligned and ldw even
-  int pad_;
+  int n_eb_coarse;         // energy blocks [0, n_eb_coarse) use coarse tiles, [n_eb_coarse, n_eb) fine tiles
 };
 static_assert(sizeof(DevWave) == 256, "DevWave layout");
 
@@ -61,5 +69,11 @@ __host__ __device__ inline int off_tiles_in_row(int n_j, int i) {
   int c = n_j - (2 * i + 2);
   return c > 0 ? c : 0;
 }
+// Fine tiling: n_j row/column panels of 32; OFF32 tiles first (n_j (n_j - 1) / 2), then DIAG32 (n_j).
+__host__ __device__ inline int fine_tiles(int n_j) { return n_j * (n_j - 1) / 2 + n_j; }
+
+// Relative cost of one item in DMMA.8x8x4 per k-step of 4 and energy: coarse DIAG 36, coarse OFF 32,
+// fine OFF 16, fine DIAG 10 (full-size tiles; ragged edge tiles are cheaper).
+constexpr int COST_DIAG = 36, COST_OFF = 32, COST_OFF32 = 16, COST_DIAG32 = 10;
 
 }  // namespace pstgf

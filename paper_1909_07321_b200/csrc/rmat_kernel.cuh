@@ -24,7 +24,8 @@ struct ItemInfo {        // handed from the load warp to the pole-scaling and co
   int n_poles;
   int n_valid_e;         // energies in this block (1..EB)
   int row0, col0;
-  int kind;              // 0 DIAG, 1 OFF, -1 stop
+  short kind;            // 0 DIAG, 1 OFF, -1 stop
+  short nrb;             // OFF: 8-row blocks of the I panel (8 coarse, 4 fine)
   int nblk;              // DIAG: valid 8x8 block rows/cols; OFF: valid 8-wide column blocks
   int n_kt;
 };
@@ -87,14 +88,14 @@ __device__ __forceinline__ void consume_idle(int n_kt, PipeState &ps, uint32_t f
   }
 }
 
-// OFF tile: 64 x 32 block strictly above the diagonal; 8 x 4 DMMA blocks, all needed
-// (column blocks >= nblk lie beyond n_chan and are skipped).
-template <int NCB>
+// OFF tile: 64 x 32 (coarse, NRB = 8) or 32 x 32 (fine, NRB = 4) block strictly above the diagonal;
+// NRB x 4 DMMA blocks, all needed (column blocks >= nblk lie beyond n_chan and are skipped).
+template <int NCB, int NRB>
 __device__ __forceinline__ void consume_off(const ItemInfo &it, const unsigned char *smem, PipeState &ps,
                                             uint32_t full0, uint32_t empty0, int warp, int lane) {
-  double acc[8][NCB][2];
+  double acc[NRB][NCB][2];
 #pragma unroll
-  for (int bi = 0; bi < 8; ++bi)
+  for (int bi = 0; bi < NRB; ++bi)
 #pragma unroll
     for (int bj = 0; bj < NCB; ++bj) acc[bi][bj][0] = acc[bi][bj][1] = 0.0;
   const int g = lane >> 2, q = lane & 3;
@@ -107,14 +108,14 @@ __device__ __forceinline__ void consume_off(const ItemInfo &it, const unsigned c
 #pragma unroll
     for (int ks = 0; ks < KT / 4; ++ks) {
       const double dv = dd[ks * 4];
-      double a[8];
+      double a[NRB];
 #pragma unroll
-      for (int bi = 0; bi < 8; ++bi) a[bi] = wi[bi * 8 * KT + ks * 4];
+      for (int bi = 0; bi < NRB; ++bi) a[bi] = wi[bi * 8 * KT + ks * 4];
 #pragma unroll
       for (int bj = 0; bj < NCB; ++bj) {
         const double b = wj[bj * 8 * KT + ks * 4] * dv;   // pole scaling folded into the B fragment
 #pragma unroll
-        for (int bi = 0; bi < 8; ++bi) dmma884(acc[bi][bj][0], acc[bi][bj][1], a[bi], b);
+        for (int bi = 0; bi < NRB; ++bi) dmma884(acc[bi][bj][0], acc[bi][bj][1], a[bi], b);
       }
     }
     __syncwarp();
@@ -129,7 +130,7 @@ __device__ __forceinline__ void consume_off(const ItemInfo &it, const unsigned c
   for (int bj = 0; bj < NCB; ++bj) {
     const int c = it.col0 + bj * 8 + 2 * q;
 #pragma unroll
-    for (int bi = 0; bi < 8; ++bi) {
+    for (int bi = 0; bi < NRB; ++bi) {
       const int r = it.row0 + bi * 8 + g;
       const double v0 = acc[bi][bj][0] * s, v1 = acc[bi][bj][1] * s;
       if (c < C) { __stcs(R + (size_t)r * C + c, v0); __stcs(R + (size_t)c * C + r, v0); }
@@ -210,17 +211,49 @@ __device__ __forceinline__ void consume_item(const ItemInfo &it, const unsigned 
       default: consume_diag<1>(it, smem, ps, full0, empty0, warp, lane); break;
     }
   } else {
-    switch (it.nblk) {
-      case 4: consume_off<4>(it, smem, ps, full0, empty0, warp, lane); break;
-      case 3: consume_off<3>(it, smem, ps, full0, empty0, warp, lane); break;
-      case 2: consume_off<2>(it, smem, ps, full0, empty0, warp, lane); break;
-      default: consume_off<1>(it, smem, ps, full0, empty0, warp, lane); break;
+    if (it.nrb == 8) {
+      switch (it.nblk) {
+        case 4: consume_off<4, 8>(it, smem, ps, full0, empty0, warp, lane); break;
+        case 3: consume_off<3, 8>(it, smem, ps, full0, empty0, warp, lane); break;
+        case 2: consume_off<2, 8>(it, smem, ps, full0, empty0, warp, lane); break;
+        default: consume_off<1, 8>(it, smem, ps, full0, empty0, warp, lane); break;
+      }
+    } else {
+      switch (it.nblk) {
+        case 4: consume_off<4, 4>(it, smem, ps, full0, empty0, warp, lane); break;
+        case 3: consume_off<3, 4>(it, smem, ps, full0, empty0, warp, lane); break;
+        case 2: consume_off<2, 4>(it, smem, ps, full0, empty0, warp, lane); break;
+        default: consume_off<1, 4>(it, smem, ps, full0, empty0, warp, lane); break;
+      }
     }
   }
 }
 
 // ---- producer ----------------------------------------------------------------------------
-// Tile index inside a wave -> (kind, row0, col0, nblk).  DIAG tiles first (they are the most
+// Fine tile index -> OFF32 tiles first (16 DMMA per k-step), then DIAG32 (10).
+__device__ __forceinline__ void decode_tile_fine(const DevWave &w, int tile, int &kind, int &row0, int &col0, int &nblk) {
+  const int n = w.n_j, n_off = n * (n - 1) / 2;
+  if (tile < n_off) {
+    kind = 1;
+    int t = tile, i = 0;
+    for (;; ++i) {
+      const int cnt = n - 1 - i;
+      if (t < cnt) break;
+      t -= cnt;
+    }
+    row0 = i * TN;
+    col0 = (i + 1 + t) * TN;
+    const int left = w.n_chan - col0;
+    nblk = left >= TN ? TN / 8 : (left + 7) / 8;
+  } else {
+    kind = 0;
+    row0 = col0 = (tile - n_off) * TN;
+    const int left = w.n_chan - row0;
+    nblk = left >= TN ? TN / 8 : (left + 7) / 8;
+  }
+}
+
+// Coarse tile index inside a wave -> (kind, row0, col0, nblk).  DIAG tiles first (they are the most
 // expensive: 36 DMMA per k-step against 32), then OFF tiles row by row.
 __device__ __forceinline__ void decode_tile(const DevWave &w, int tile, int &kind, int &row0, int &col0, int &nblk) {
   if (tile < w.n_i) {
@@ -287,8 +320,10 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
       uint32_t iq = 0, iphase = 0;
       long long next_static = blockIdx.x;
       for (;;) {
+        // items are drawn from an atomic counter (batch call: in the workspace; single-wave call: a slot of
+        // the library's counter pool), or round-robin when the single-wave call found no free slot
         long long item;
-        if (BATCH) {
+        if (counter != nullptr) {
           unsigned long long got = 0;
           if (lane == 0) got = atomicAdd(counter, 1ULL);
           item = (long long)__shfl_sync(0xffffffffu, got, 0);
@@ -297,30 +332,41 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
           next_static += gridDim.x;
         }
         const bool stop = item >= n_items;
-        // locate the wave (batch: binary search in the item-range table)
+        // locate the section: [coarse items of wave 0, 1, ... | fine items of wave 0, 1, ...]
         int p = 0;
-        if (BATCH && !stop) {
-          int lo = 0, hi = n_waves;            // item_begin[lo] <= item < item_begin[hi]
-          while (hi - lo > 1) {
-            const int mid = (lo + hi) >> 1;
-            if (__ldg(item_begin + mid) <= item) lo = mid; else hi = mid;
+        bool fine = false;
+        if (!stop) {
+          if (BATCH) {
+            int lo = 0, hi = 2 * n_waves;        // item_begin[lo] <= item < item_begin[hi]
+            while (hi - lo > 1) {
+              const int mid = (lo + hi) >> 1;
+              if (__ldg(item_begin + mid) <= item) lo = mid; else hi = mid;
+            }
+            item -= __ldg(item_begin + lo);
+            fine = lo >= n_waves;
+            p = fine ? lo - n_waves : lo;
+          } else {
+            const long long n_coarse = (long long)single.n_tiles * single.n_eb_coarse;
+            fine = item >= n_coarse;
+            if (fine) item -= n_coarse;
           }
-          p = lo;
-          item -= __ldg(item_begin + p);
         }
         const DevWave &w = BATCH ? waves[p] : single;
-        int kind = -1, row0 = 0, col0 = 0, nblk = 0, eb = 0, n_valid = 0, n_kt = 0;
+        int kind = -1, row0 = 0, col0 = 0, nblk = 0, nrb = 0, eb = 0, n_valid = 0, n_kt = 0;
         if (!stop) {
-          const int tile = (int)(item / w.n_eb);
-          eb = (int)(item - (long long)tile * w.n_eb);
-          decode_tile(w, tile, kind, row0, col0, nblk);
+          const int n_eb_sec = fine ? w.n_eb - w.n_eb_coarse : w.n_eb_coarse;
+          const int tile = (int)(item / n_eb_sec);
+          eb = (int)(item - (long long)tile * n_eb_sec) + (fine ? w.n_eb_coarse : 0);
+          if (fine) decode_tile_fine(w, tile, kind, row0, col0, nblk);
+          else decode_tile(w, tile, kind, row0, col0, nblk);
+          nrb = kind == 0 ? nblk : (fine ? TN / 8 : TM / 8);   // 8-row blocks of the I panel that are read
           n_valid = min(EB, w.n_E - eb * EB);
           n_kt = w.n_kt;
         }
         mbar_wait(item_empty0 + 8 * iq, iphase ^ 1u);
         if (lane == 0) {
           ItemInfo &ii = ring[iq];
-          ii.kind = kind;
+          ii.kind = (short)kind;
           if (!stop) {
             ii.R = w.R_out + (size_t)eb * EB * w.n_chan * w.n_chan;
             ii.E_k = w.E_k;
@@ -331,6 +377,7 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
             ii.n_valid_e = n_valid;
             ii.row0 = row0;
             ii.col0 = col0;
+            ii.nrb = (short)nrb;
             ii.nblk = nblk;
             ii.n_kt = n_kt;
           }
@@ -341,7 +388,8 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
         if (stop) break;
 
         const CUtensorMap *map = &w.map;
-        const uint32_t tx_bytes = (kind == 0 ? 2 : 3) * BOX_BYTES;
+        const int i_boxes = nrb > TN / 8 ? 2 : 1;              // I panel: one or two boxes of 32 rows
+        const uint32_t tx_bytes = (i_boxes + (kind != 0 ? 1 : 0)) * BOX_BYTES;
         for (int kt = 0; kt < n_kt; ++kt) {
           const int k0 = kt * KT;
           mbar_wait(empty0 + 8 * ps.stage, ps.phase ^ 1u);
@@ -352,16 +400,23 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
               mbar_arrive_expect_tx(full, tx_bytes);
               const uint32_t dst = smem_u32(st);
               tma_load_2d(dst, map, k0, row0, full);
-              tma_load_2d(dst + BOX_BYTES, map, k0, row0 + TN, full);
+              if (i_boxes == 2) tma_load_2d(dst + BOX_BYTES, map, k0, row0 + TN, full);
               if (kind != 0) tma_load_2d(dst + WI_BYTES, map, k0, col0, full);
             }
           } else {
-            stage_panel_plain(reinterpret_cast<double *>(st), w, row0, TM, k0, lane);
+            stage_panel_plain(reinterpret_cast<double *>(st), w, row0, i_boxes * TN, k0, lane);
             if (kind != 0) stage_panel_plain(reinterpret_cast<double *>(st + WI_BYTES), w, col0, TN, k0, lane);
             __syncwarp();
             if (lane == 0) mbar_arrive(full);
           }
           ps.advance();
+        }
+      }
+      // single-wave call with a pool counter: the last CTA to run dry hands the slot back zeroed
+      if (!BATCH && counter != nullptr && lane == 0) {
+        if (atomicAdd(counter + 1, 1ULL) == (unsigned long long)gridDim.x - 1) {
+          counter[0] = 0ULL;
+          counter[1] = 0ULL;
         }
       }
     } else {

@@ -14,11 +14,12 @@ import torch
 from . import build as _build
 
 PSTGF_OK = 0
+PSTGF_TAIL_AUTO, PSTGF_TAIL_NONE, PSTGF_TAIL_ALL = 0, 1, 2
 _STATUS_NAMES = {0: "PSTGF_OK", 1: "PSTGF_ERR_INVALID_VALUE", 2: "PSTGF_ERR_ALIGNMENT", 3: "PSTGF_ERR_WORKSPACE",
                  4: "PSTGF_ERR_UNSUPPORTED_DEVICE", 5: "PSTGF_ERR_CUDA"}
 
 EXPORTS = ["pstgf_rmat_form", "pstgf_rmat_batch_workspace_bytes", "pstgf_rmat_form_batch", "pstgf_rmat_form_naive",
-           "pstgf_rmat_form_batch_host", "pstgf_fp64_probe", "pstgf_last_launch_count", "pstgf_status_string", "pstgf_last_cuda_error",
+           "pstgf_rmat_form_batch_host", "pstgf_rmat_set_tail_policy", "pstgf_fp64_probe", "pstgf_last_launch_count", "pstgf_status_string", "pstgf_last_cuda_error",
            "pstgf_version"]
 
 
@@ -66,6 +67,8 @@ def load(build_if_missing: bool = False):
     lib.pstgf_rmat_form_batch.restype = i
     lib.pstgf_rmat_form_batch_host.argtypes = [ctypes.POINTER(pstgf_wave_t), i, sz, vp]
     lib.pstgf_rmat_form_batch_host.restype = i
+    lib.pstgf_rmat_set_tail_policy.argtypes = [i]
+    lib.pstgf_rmat_set_tail_policy.restype = i
     lib.pstgf_fp64_probe.argtypes = [i, i, i, i, vp, ctypes.POINTER(d), vp]
     lib.pstgf_fp64_probe.restype = i
     lib.pstgf_last_launch_count.restype = i
@@ -180,6 +183,11 @@ def pstgf_rmat_form_batch_host(host_waves: Sequence[tuple], max_chunk_bytes: int
         arr[p] = pstgf_wave_t(n_chan, n_poles, int(energies.shape[0]), max(n_poles, 1) if n_chan <= 1 else int(W.stride(0)),
                               float(a), W.data_ptr(), E_k.data_ptr(), energies.data_ptr(), R_out.data_ptr())
     _check(lib.pstgf_rmat_form_batch_host(arr, len(host_waves), int(max_chunk_bytes), _stream_ptr(stream)))
+
+
+def pstgf_rmat_set_tail_policy(policy: int) -> None:
+    """Scheduling knob: PSTGF_TAIL_AUTO / PSTGF_TAIL_NONE / PSTGF_TAIL_ALL (results are bitwise the same)."""
+    _check(load().pstgf_rmat_set_tail_policy(int(policy)))
 
 
 def pstgf_fp64_probe(kind: int, iters: int, blocks: int, threads: int, sink: torch.Tensor, stream=None) -> float:

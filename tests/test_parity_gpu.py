@@ -92,12 +92,71 @@ EDGE_SHAPES = [
 ]
 
 
+@pytest.fixture
+def tail_policy(rmat):
+    """Sets the scheduling knob for one test and restores the default afterwards."""
+    def set_policy(policy):
+        rmat.pstgf_rmat_set_tail_policy(policy)
+    yield set_policy
+    rmat.pstgf_rmat_set_tail_policy(rmat.PSTGF_TAIL_AUTO)
+
+
 @pytest.mark.parametrize("C,K,N", EDGE_SHAPES)
-def test_edge_shapes(rmat, oracle, C, K, N):
+def test_edge_shapes(rmat, oracle, tail_policy, C, K, N):
+    """Small problems are all 'tail' under the default policy, so every shape is run with coarse tiles only,
+    fine tiles only and the automatic split, single-wave call and batch call."""
     from paper_1909_07321_b200 import inputs
     w = inputs.make_wave(1000 + C * 7 + K, C, K, N)
     R_ref = oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads())
-    _check(_form(rmat, w), R_ref)
+    results = []
+    for policy in (rmat.PSTGF_TAIL_NONE, rmat.PSTGF_TAIL_ALL, rmat.PSTGF_TAIL_AUTO):
+        tail_policy(policy)
+        R = _form(rmat, w)
+        _check(R, R_ref)
+        results.append(R)
+        Rb = _form_batch(rmat, [w])[0].cpu().numpy()
+        assert np.array_equal(R, Rb)
+    # the tilings give every element the same operands and summation order
+    assert np.array_equal(results[0], results[1]) and np.array_equal(results[0], results[2])
+
+
+def test_tail_split_inside_a_wave(rmat, oracle, tail_policy):
+    """Enough energy blocks that the automatic policy keeps coarse items AND cuts a fine tail (both sections of
+    the item list in one launch), on a shape with ragged tiles in both tilings."""
+    from paper_1909_07321_b200 import inputs
+    w = inputs.make_wave(4242, 150, 120, 8 * 40 + 3)
+    R_ref = oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads())
+    tail_policy(rmat.PSTGF_TAIL_AUTO)
+    R = _form(rmat, w)
+    _check(R, R_ref)
+    tail_policy(rmat.PSTGF_TAIL_NONE)
+    assert np.array_equal(R, _form(rmat, w))
+    tail_policy(rmat.PSTGF_TAIL_AUTO)
+    w2 = inputs.make_wave(4243, 40, 90, 8 * 30 + 1)
+    Rs = _form_batch(rmat, [w, w2])
+    assert np.array_equal(R, Rs[0].cpu().numpy())
+    _check(Rs[1].cpu().numpy(), oracle.rmat_form(w2.W, w2.E_k, w2.energies, w2.a, threads=_threads()))
+
+
+def test_many_launches_in_flight(rmat, oracle):
+    """More single-wave launches in flight than the counter pool has slots (64), on several streams: every
+    launch must still do all of its items exactly once (pool slot or round-robin fallback)."""
+    from paper_1909_07321_b200 import inputs
+    w = inputs.make_wave(99, 70, 200, 20)
+    Wd, Ek, en = _dev(w.W), _dev(w.E_k), _dev(w.energies)
+    R_ref = oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads())
+    streams = [torch.cuda.Stream() for _ in range(4)]
+    outs = []
+    torch.cuda.synchronize()
+    for i in range(200):
+        st = streams[i % 4]
+        with torch.cuda.stream(st):
+            outs.append(rmat.pstgf_rmat_form(Wd, Ek, en, w.a, stream=st))
+    torch.cuda.synchronize()
+    first = outs[0].cpu().numpy()
+    _check(first, R_ref)
+    for R in outs[1:]:
+        assert torch.equal(R, outs[0])
 
 
 def test_naive_kernel_matches_oracle(rmat, oracle):
