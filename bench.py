@@ -44,6 +44,9 @@ def parse_args():
     ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5, 6],
                     help="1-5: BASELINE.json configs[0..4]; 6: the paper-scale wave of PAPER.md:168 (7261 x 106661)")
+    ap.add_argument("--w-layout", choices=["poles", "channels"], default="poles",
+                    help="memory order of W on the device: pole-contiguous [n_chan][n_poles] (default, north_star's) or "
+                         "channel-contiguous [n_poles][n_chan], the H.DAT record order of PAPER.md:535")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
@@ -288,13 +291,19 @@ def run_cuda(args):
         for p, idx in shard.plan([w.n_E for w in wl_job.waves], rank, world):
             w = wl_job.waves[p]
             wl.waves.append(inputs.Wave(w.W, w.E_k, np.ascontiguousarray(w.energies[idx]), w.a))
+    hdat = args.w_layout == "channels"
+    layout = rmat.PSTGF_W_CHANNEL_CONTIGUOUS if hdat else rmat.PSTGF_W_POLE_CONTIGUOUS
+
     def dev_W(w):
-        """W on the device; an odd n_poles (config 6) gets an even row pitch so that the TMA staging path applies."""
-        if w.n_poles % 2 == 0:
-            return torch.from_numpy(w.W).cuda()
-        buf = torch.zeros((w.n_chan, w.n_poles + 1), dtype=torch.float64, device="cuda")
-        buf[:, :w.n_poles].copy_(torch.from_numpy(w.W))
-        return buf[:, :w.n_poles]
+        """W on the device in the chosen memory order; an odd fastest dimension (config 6's n_poles, an odd n_chan in
+        the H.DAT order) gets an even row pitch so that the TMA staging path applies."""
+        Wh = np.ascontiguousarray(w.W.T) if hdat else w.W
+        rows, cols = Wh.shape
+        if cols % 2 == 0:
+            return torch.from_numpy(Wh).cuda()
+        buf = torch.zeros((rows, cols + 1), dtype=torch.float64, device="cuda")
+        buf[:, :cols].copy_(torch.from_numpy(Wh))
+        return buf[:, :cols]
 
     dev_waves, shared = [], {}
     for w in wl.waves:
@@ -302,7 +311,7 @@ def run_cuda(args):
         if key not in shared:
             shared[key] = torch.from_numpy(w.energies).cuda()
         R = torch.empty((w.n_E, w.n_chan, w.n_chan), dtype=torch.float64, device="cuda")
-        dev_waves.append((dev_W(w), torch.from_numpy(w.E_k).cuda(), shared[key], w.a, R))
+        dev_waves.append((dev_W(w), torch.from_numpy(w.E_k).cuda(), shared[key], w.a, R, layout))
     single = len(dev_waves) == 1
     if not single:
         arr = rmat.make_wave_array(dev_waves)
@@ -311,8 +320,8 @@ def run_cuda(args):
 
     def step():
         if single:
-            W, E_k, en, a, R = dev_waves[0]
-            rmat.pstgf_rmat_form(W, E_k, en, a, R_out=R)
+            W, E_k, en, a, R, _ = dev_waves[0]
+            (rmat.pstgf_rmat_form_hdat if hdat else rmat.pstgf_rmat_form)(W, E_k, en, a, R_out=R)
         else:
             rmat.pstgf_rmat_form_batch(arr, ws)
         return rmat.pstgf_last_launch_count()
@@ -401,11 +410,11 @@ def run_cuda(args):
     if not args.no_e2e:
         host = []
         for w in wl.waves:
-            hW = torch.from_numpy(w.W).pin_memory()
+            hW = torch.from_numpy(np.ascontiguousarray(w.W.T) if hdat else w.W).pin_memory()
             hEk = torch.from_numpy(w.E_k).pin_memory()
             hEn = torch.from_numpy(w.energies).pin_memory()
             hR = torch.empty((w.n_E, w.n_chan, w.n_chan), dtype=torch.float64).pin_memory()
-            host.append((hW, hEk, hEn, w.a, hR))
+            host.append((hW, hEk, hEn, w.a, hR, layout))
         h2d = sum(8 * (a[0].numel() + a[1].numel() + a[2].numel()) for a in host)
         d2h = sum(8 * a[4].numel() for a in host)
         e2e_steps = max(1, min(args.steps, 5 if args.config != 6 else 2))
@@ -441,7 +450,7 @@ def run_cuda(args):
                 "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": vs_baseline, "dtype": "f64", "data": "synthetic",
                 "config": dict(workload_description(args.config, wl), n_energies_per_step=n_e_job, n_energies_per_rank=n_e,
-                               l2="flushed between timed steps (512 MiB write)",
+                               l2="flushed between timed steps (512 MiB write)", w_layout=args.w_layout,
                                sha256=wl.sha256()[:16]),
                 "tflops_counted": world * flop * args.steps / (total_ms_max * 1e-3) / 1e12,   # ranks carry equal shares
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,

@@ -28,7 +28,8 @@
  *    of the enqueued work.  Host structs (pstgf_wave_t arrays) are consumed
  *    before the call returns.
  *  - Layout: W is row-major [n_chan][ldw], element (n,k) at W[n*ldw + k],
- *    ldw >= n_poles (k contiguous).  R_out is dense row-major
+ *    ldw >= n_poles (k contiguous), unless the wave says
+ *    PSTGF_W_CHANNEL_CONTIGUOUS (the H.DAT record order).  R_out is dense row-major
  *    [n_E][n_chan][n_chan]; BOTH triangles are written and R_out[e][n][m] ==
  *    R_out[e][m][n] bitwise.  R_out must not overlap any input or another
  *    wave's R_out.  Inputs may be shared between waves.
@@ -39,7 +40,8 @@
  *    callers keep a clearance (the synthetic workloads use 1e-3 Ryd).
  *  - Alignment: every pointer must be 8-byte aligned (else
  *    PSTGF_ERR_ALIGNMENT).  W 16-byte aligned with even ldw selects the TMA
- *    staging path; otherwise a slower load path inside the same kernel is
+ *    staging path (for an H.DAT record with an odd NCHAN: copy it with an even
+ *    pitch, or accept the slower path); otherwise a slower load path inside the same kernel is
  *    used.  Any n_chan (odd included) is supported.
  *  - Results are deterministic: each R element is produced by exactly one
  *    thread with a fixed k order, whatever CTA picked the work item up.
@@ -55,11 +57,11 @@
 extern "C" {
 #endif
 
-#define PSTGF_RMAT_VERSION 101 /* major*100 + minor */
+#define PSTGF_RMAT_VERSION 102 /* major*100 + minor */
 
 typedef enum {
   PSTGF_OK = 0,
-  PSTGF_ERR_INVALID_VALUE = 1,      /* NULL where data is required, negative size, ldw < n_poles, a not finite or <= 0 */
+  PSTGF_ERR_INVALID_VALUE = 1,      /* NULL where data is required, negative size, ldw too small, unknown w_layout, a not finite or <= 0 */
   PSTGF_ERR_ALIGNMENT = 2,          /* a pointer is not 8-byte aligned */
   PSTGF_ERR_WORKSPACE = 3,          /* workspace NULL, not 256-byte aligned, or smaller than the query says */
   PSTGF_ERR_UNSUPPORTED_DEVICE = 4, /* no CUDA device, or the current device is not compute capability 10.x */
@@ -75,6 +77,7 @@ typedef struct {
   int n_chan;             /* NCHAN */
   int n_poles;            /* MNP2, */
   int n_E;                /* energies of this wave's mesh */
+  int w_layout;           /* PSTGF_W_POLE_CONTIGUOUS (0) or PSTGF_W_CHANNEL_CONTIGUOUS (1), see below */
   long long ldw;          /* leading dimension of W in elements, >= n_poles */
   double a;               /* RA, a.u., > 0 */
   const double *W;        /* [n_chan][ldw] */
@@ -82,6 +85,21 @@ typedef struct {
   const double *energies; /* [n_E] */
   double *R_out;          /* [n_E][n_chan][n_chan] */
 } pstgf_wave_t;
+
+/*
+ * Memory order of W.
+ *   PSTGF_W_POLE_CONTIGUOUS     W[n_chan][ldw], element (n,k) at W[n*ldw + k], ldw >= n_poles
+ *                               (north_star's W[n_chan x n_poles]).
+ *   PSTGF_W_CHANNEL_CONTIGUOUS  W[n_poles][ldw], element (n,k) at W[k*ldw + n], ldw >= n_chan:
+ *                               the order of the H.DAT record "((WMAT(I,K) K=1-NCHAN), I=1-MNP2)"
+ *                               (channels run fastest, one pole after the other), so a
+ *                               record read from H.DATXXX can be handed over as it is, with no
+ *                               transposition pass.  The panels are then staged pole-major in shared
+ *                               memory by TMA boxes of 36 channels x 20 poles.
+ * Both orders give bitwise the same R.
+ */
+#define PSTGF_W_POLE_CONTIGUOUS 0
+#define PSTGF_W_CHANNEL_CONTIGUOUS 1
 
 /*
  * Eq. 4 for one partial wave at n_E energies.
@@ -102,6 +120,15 @@ typedef struct {
 pstgf_status_t pstgf_rmat_form(const double *W, long long ldw, const double *E_k,
                                const double *energies, int n_chan, int n_poles, int n_E,
                                double a, double *R_out, void *stream);
+
+/*
+ * pstgf_rmat_form for W in the H.DAT record order (PSTGF_W_CHANNEL_CONTIGUOUS):
+ * DEVICE Wt [n_poles][ldw], element (n,k) at Wt[k*ldw + n], ldw >= n_chan.
+ * Everything else as pstgf_rmat_form.
+ */
+pstgf_status_t pstgf_rmat_form_hdat(const double *Wt, long long ldw, const double *E_k,
+                                    const double *energies, int n_chan, int n_poles, int n_E,
+                                    double a, double *R_out, void *stream);
 
 /*
  * Scheduling knob (process-wide; meant for tests and measurements).  Work
@@ -145,11 +172,11 @@ pstgf_status_t pstgf_rmat_form_batch(const pstgf_wave_t *waves, int n_waves, voi
  * that follows eq. 4 term by term ((w_n*w_m)/(E_k-E), k ascending,
  * compensated sum).  Slow; provided so that callers and tests can check every
  * energy of a large run against an independent device evaluation.
- * DEVICE: W, E_k, energies, R_out.
+ * DEVICE: W, E_k, energies, R_out.  `w_layout` as in pstgf_wave_t.
  */
 pstgf_status_t pstgf_rmat_form_naive(const double *W, long long ldw, const double *E_k,
                                      const double *energies, int n_chan, int n_poles, int n_E,
-                                     double a, double *R_out, void *stream);
+                                     double a, double *R_out, int w_layout, void *stream);
 
 /*
  * End-to-end convenience over HOST buffers: `waves` holds HOST pointers

@@ -93,7 +93,9 @@ pstgf_status_t check_wave(const pstgf_wave_t &w) {
   if (!(w.a > 0.0) || !std::isfinite(w.a)) return PSTGF_ERR_INVALID_VALUE;
   if (w.n_chan == 0 || w.n_E == 0) return PSTGF_OK;       // nothing to read or write
   if (!w.energies || !w.R_out) return PSTGF_ERR_INVALID_VALUE;
-  if (w.n_poles > 0 && (!w.W || !w.E_k || w.ldw < w.n_poles)) return PSTGF_ERR_INVALID_VALUE;
+  if (w.w_layout != PSTGF_W_POLE_CONTIGUOUS && w.w_layout != PSTGF_W_CHANNEL_CONTIGUOUS) return PSTGF_ERR_INVALID_VALUE;
+  const long long ld_min = w.w_layout == PSTGF_W_CHANNEL_CONTIGUOUS ? w.n_chan : w.n_poles;
+  if (w.n_poles > 0 && (!w.W || !w.E_k || w.ldw < ld_min)) return PSTGF_ERR_INVALID_VALUE;
   if (!aligned8(w.W) || !aligned8(w.E_k) || !aligned8(w.energies) || !aligned8(w.R_out)) return PSTGF_ERR_ALIGNMENT;
   return PSTGF_OK;
 }
@@ -121,6 +123,7 @@ void plan_wave(const pstgf_wave_t &w, DevWave &d) {
   for (int i = 0; i < d.n_i; ++i) tiles += pstgf::off_tiles_in_row(d.n_j, i);
   d.n_tiles = tiles;
   d.n_eb_coarse = d.n_eb;
+  d.tr = w.w_layout == PSTGF_W_CHANNEL_CONTIGUOUS ? 1 : 0;
   d.use_tma = ((reinterpret_cast<uintptr_t>(w.W) & 15u) == 0 && (w.ldw % 2) == 0 && w.ldw * 8 < (1LL << 40)) ? 1 : 0;
 }
 
@@ -167,9 +170,16 @@ void plan_tails(std::vector<DevWave> &ds, int grid) {
 
 pstgf_status_t encode_map(DevWave &d) {
   if (!d.use_tma) return PSTGF_OK;
+  // pole-contiguous W: dims (pole, channel), box 20 poles x 32 channels; channel-contiguous W (H.DAT order):
+  // dims (channel, pole), box 36 channels x 20 poles.  Out-of-range elements are zero-filled either way.
   cuuint64_t dims[2] = {(cuuint64_t)d.n_poles, (cuuint64_t)d.n_chan};
-  cuuint64_t strides[1] = {(cuuint64_t)d.ldw * 8};
   cuuint32_t box[2] = {(cuuint32_t)pstgf::KT, (cuuint32_t)pstgf::TN};
+  if (d.tr) {
+    std::swap(dims[0], dims[1]);
+    box[0] = (cuuint32_t)pstgf::TR_PITCH;
+    box[1] = (cuuint32_t)pstgf::KT;
+  }
+  cuuint64_t strides[1] = {(cuuint64_t)d.ldw * 8};
   cuuint32_t estr[2] = {1, 1};
   CUresult r = g_encode(&d.map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double *>(d.W), dims, strides, box, estr,
                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -263,10 +273,9 @@ pstgf_status_t pstgf_rmat_set_tail_policy(int policy) {
   return PSTGF_OK;
 }
 
-pstgf_status_t pstgf_rmat_form(const double *W, long long ldw, const double *E_k, const double *energies, int n_chan,
-                               int n_poles, int n_E, double a, double *R_out, void *stream) {
+static pstgf_status_t form_single(const pstgf_wave_t &w, void *stream) {
+  const int n_chan = w.n_chan, n_poles = w.n_poles, n_E = w.n_E;
   tl_launches = 0;
-  pstgf_wave_t w{n_chan, n_poles, n_E, ldw, a, W, E_k, energies, R_out};
   pstgf_status_t st = check_wave(w);
   if (st != PSTGF_OK) return st;
   if (n_chan == 0 || n_E == 0) return PSTGF_OK;
@@ -297,6 +306,18 @@ pstgf_status_t pstgf_rmat_form(const double *W, long long ldw, const double *E_k
   }
   tl_launches = 1;
   return PSTGF_OK;
+}
+
+pstgf_status_t pstgf_rmat_form(const double *W, long long ldw, const double *E_k, const double *energies, int n_chan,
+                               int n_poles, int n_E, double a, double *R_out, void *stream) {
+  pstgf_wave_t w{n_chan, n_poles, n_E, PSTGF_W_POLE_CONTIGUOUS, ldw, a, W, E_k, energies, R_out};
+  return form_single(w, stream);
+}
+
+pstgf_status_t pstgf_rmat_form_hdat(const double *Wt, long long ldw, const double *E_k, const double *energies,
+                                    int n_chan, int n_poles, int n_E, double a, double *R_out, void *stream) {
+  pstgf_wave_t w{n_chan, n_poles, n_E, PSTGF_W_CHANNEL_CONTIGUOUS, ldw, a, Wt, E_k, energies, R_out};
+  return form_single(w, stream);
 }
 
 size_t pstgf_rmat_batch_workspace_bytes(const pstgf_wave_t *waves, int n_waves) {
@@ -370,9 +391,10 @@ pstgf_status_t pstgf_rmat_form_batch(const pstgf_wave_t *waves, int n_waves, voi
 }
 
 pstgf_status_t pstgf_rmat_form_naive(const double *W, long long ldw, const double *E_k, const double *energies,
-                                     int n_chan, int n_poles, int n_E, double a, double *R_out, void *stream) {
+                                     int n_chan, int n_poles, int n_E, double a, double *R_out, int w_layout,
+                                     void *stream) {
   tl_launches = 0;
-  pstgf_wave_t w{n_chan, n_poles, n_E, ldw, a, W, E_k, energies, R_out};
+  pstgf_wave_t w{n_chan, n_poles, n_E, w_layout, ldw, a, W, E_k, energies, R_out};
   pstgf_status_t st = check_wave(w);
   if (st != PSTGF_OK) return st;
   if (n_chan == 0 || n_E == 0) return PSTGF_OK;
@@ -384,7 +406,8 @@ pstgf_status_t pstgf_rmat_form_naive(const double *W, long long ldw, const doubl
   const long long blocks = (n_elems + threads - 1) / threads;
   if (blocks > 0x7fffffffLL) return PSTGF_ERR_INVALID_VALUE;
   pstgf::rmat_naive_kernel<<<(unsigned)blocks, threads, 0, static_cast<cudaStream_t>(stream)>>>(
-      W, ldw, E_k, energies, n_chan, n_poles, n_elems, a, R_out);
+      W, w_layout == PSTGF_W_CHANNEL_CONTIGUOUS ? 1LL : ldw, w_layout == PSTGF_W_CHANNEL_CONTIGUOUS ? ldw : 1LL, E_k, energies,
+      n_chan, n_poles, n_elems, a, R_out);
   PSTGF_CUDA(cudaGetLastError());
   tl_launches = 1;
   return PSTGF_OK;
@@ -488,12 +511,14 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
       std::memset(w.R_out, 0, sizeof(double) * (size_t)w.n_E * w.n_chan * w.n_chan);
       continue;
     }
-    const long long pitch = ((long long)w.n_poles + 1) & ~1LL;
+    const bool tr = w.w_layout == PSTGF_W_CHANNEL_CONTIGUOUS;
+    const long long w_rows = tr ? w.n_poles : w.n_chan, w_cols = tr ? w.n_chan : w.n_poles;
+    const long long pitch = (w_cols + 1) & ~1LL;
     void *dW, *dEk, *dEn;
-    PSTGF_CUDA(dev_alloc(sizeof(double) * (size_t)pitch * w.n_chan, &dW));
+    PSTGF_CUDA(dev_alloc(sizeof(double) * (size_t)pitch * w_rows, &dW));
     PSTGF_CUDA(dev_alloc(sizeof(double) * (size_t)w.n_poles, &dEk));
     PSTGF_CUDA(dev_alloc(sizeof(double) * (size_t)w.n_E, &dEn));
-    PSTGF_CUDA(cudaMemcpy2DAsync(dW, pitch * 8, w.W, w.ldw * 8, (size_t)w.n_poles * 8, w.n_chan, cudaMemcpyHostToDevice, res.s));
+    PSTGF_CUDA(cudaMemcpy2DAsync(dW, pitch * 8, w.W, w.ldw * 8, (size_t)w_cols * 8, (size_t)w_rows, cudaMemcpyHostToDevice, res.s));
     PSTGF_CUDA(cudaMemcpyAsync(dEk, w.E_k, sizeof(double) * (size_t)w.n_poles, cudaMemcpyHostToDevice, res.s));
     PSTGF_CUDA(cudaMemcpyAsync(dEn, w.energies, sizeof(double) * (size_t)w.n_E, cudaMemcpyHostToDevice, res.s));
     dev[p].W = static_cast<double *>(dW);

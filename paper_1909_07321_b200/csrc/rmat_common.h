@@ -38,7 +38,26 @@ constexpr int BOX_BYTES = TN * KT * 8;               // one TMA box: 32 rows x 2
 constexpr int WI_BYTES = TM * KT * 8;                // two boxes
 constexpr int WJ_BYTES = TN * KT * 8;
 constexpr int D_BYTES = EB * KT * 8;                 // d_e[k] = 1/(E_k - E_e) for the stage
-constexpr int STAGE_BYTES = WI_BYTES + WJ_BYTES + D_BYTES;   // 16640
+// Channel-contiguous W (the H.DAT record order) is staged pole-major: three panels
+// [KT poles][TR_PITCH channels] (I rows 0..31, I rows 32..63, J), each one TMA box of 36 channels x 20 poles
+// (32 used + 4 spare: the row pitch 36 == 4 (mod 16) doubles keeps the LDS.64 fragment loads conflict-free).
+constexpr int TR_PITCH = TN + 4;
+constexpr int TR_BOX_BYTES = KT * TR_PITCH * 8;      // 5760
+constexpr int STAGE_BYTES_ROWMAJOR = WI_BYTES + WJ_BYTES + D_BYTES;   // 16640
+constexpr int STAGE_BYTES_TR = 3 * TR_BOX_BYTES + D_BYTES;            // 18560
+constexpr int STAGE_BYTES = STAGE_BYTES_TR > STAGE_BYTES_ROWMAJOR ? STAGE_BYTES_TR : STAGE_BYTES_ROWMAJOR;
+
+// Offsets (in doubles) inside a stage, per layout.  i_off / j_off are additive in (row, k): the offset of
+// element (8 bi + g, 4 ks + q) is off(g, q) + off(8 bi, 4 ks).
+template <bool TR>
+struct StageLayout {
+  static constexpr int J_BASE = TR ? 2 * KT * TR_PITCH : TM * KT;
+  static constexpr int D_BASE = TR ? 3 * KT * TR_PITCH : (TM + TN) * KT;
+  __host__ __device__ static constexpr int i_off(int r, int k) {
+    return TR ? (r >> 5) * KT * TR_PITCH + k * TR_PITCH + (r & 31) : r * KT + k;
+  }
+  __host__ __device__ static constexpr int j_off(int c, int k) { return TR ? k * TR_PITCH + c : c * KT + k; }
+};
 constexpr int SMEM_BARRIER_OFFSET = STAGES * STAGE_BYTES;
 constexpr int SMEM_ITEM_OFFSET = SMEM_BARRIER_OFFSET + (2 * STAGES + 4) * 8;
 constexpr int SMEM_BYTES = SMEM_ITEM_OFFSET + 2 * 64 + 128;  // + alignment slack
@@ -46,7 +65,7 @@ constexpr int SMEM_BYTES = SMEM_ITEM_OFFSET + 2 * 64 + 128;  // + alignment slac
 // One partial wave as the kernel sees it.  Built on the host, lives in kernel parameter
 // space (single-wave call) or in the caller's workspace (batch call).
 struct alignas(128) DevWave {
-  CUtensorMap map;         // W viewed as [n_chan][n_poles] (row stride ldw*8), box [TN][KT], no swizzle
+  CUtensorMap map;         // W viewed as [n_chan][n_poles] (row stride ldw*8), box [TN][KT], no swizzle (tr: see below)
   const double *W;
   const double *E_k;
   const double *energies;
@@ -61,6 +80,7 @@ struct alignas(128) DevWave {
   int n_tiles;             // n_i + number of coarse OFF tiles
   int use_tma;             // W 16-byte aligned and ldw even
   int n_eb_coarse;         // energy blocks [0, n_eb_coarse) use coarse tiles, [n_eb_coarse, n_eb) fine tiles
+  int tr;                  // 1: W is channel-contiguous [n_poles][ldw] (H.DAT record order), map box [KT][TR_PITCH]
 };
 static_assert(sizeof(DevWave) == 256, "DevWave layout");
 

@@ -25,7 +25,8 @@ struct ItemInfo {        // handed from the load warp to the pole-scaling and co
   int n_valid_e;         // energies in this block (1..EB)
   int row0, col0;
   short kind;            // 0 DIAG, 1 OFF, -1 stop
-  short nrb;             // OFF: 8-row blocks of the I panel (8 coarse, 4 fine)
+  unsigned char nrb;     // OFF: 8-row blocks of the I panel (8 coarse, 4 fine)
+  unsigned char tr;      // stage layout: 0 row-major panels, 1 pole-major panels (channel-contiguous W)
   int nblk;              // DIAG: valid 8x8 block rows/cols; OFF: valid 8-wide column blocks
   int n_kt;
 };
@@ -90,7 +91,7 @@ __device__ __forceinline__ void consume_idle(int n_kt, PipeState &ps, uint32_t f
 
 // OFF tile: 64 x 32 (coarse, NRB = 8) or 32 x 32 (fine, NRB = 4) block strictly above the diagonal;
 // NRB x 4 DMMA blocks, all needed (column blocks >= nblk lie beyond n_chan and are skipped).
-template <int NCB, int NRB>
+template <int NCB, int NRB, bool TR>
 __device__ __forceinline__ void consume_off(const ItemInfo &it, const unsigned char *smem, PipeState &ps,
                                             uint32_t full0, uint32_t empty0, int warp, int lane) {
   double acc[NRB][NCB][2];
@@ -101,19 +102,20 @@ __device__ __forceinline__ void consume_off(const ItemInfo &it, const unsigned c
   const int g = lane >> 2, q = lane & 3;
   for (int kt = 0; kt < it.n_kt; ++kt) {
     mbar_wait(full0 + 8 * ps.stage, ps.phase);
-    const double *wi = reinterpret_cast<const double *>(smem + ps.stage * STAGE_BYTES) + g * KT + q;
-    const double *wj = wi + TM * KT;
-    const double *dd = reinterpret_cast<const double *>(smem + ps.stage * STAGE_BYTES + WI_BYTES + WJ_BYTES) +
-                       warp * KT + q;
+    using L = StageLayout<TR>;
+    const double *st = reinterpret_cast<const double *>(smem + ps.stage * STAGE_BYTES);
+    const double *wi = st + L::i_off(g, q);
+    const double *wj = st + L::J_BASE + L::j_off(g, q);
+    const double *dd = st + L::D_BASE + warp * KT + q;
 #pragma unroll
     for (int ks = 0; ks < KT / 4; ++ks) {
       const double dv = dd[ks * 4];
       double a[NRB];
 #pragma unroll
-      for (int bi = 0; bi < NRB; ++bi) a[bi] = wi[bi * 8 * KT + ks * 4];
+      for (int bi = 0; bi < NRB; ++bi) a[bi] = wi[L::i_off(bi * 8, ks * 4)];
 #pragma unroll
       for (int bj = 0; bj < NCB; ++bj) {
-        const double b = wj[bj * 8 * KT + ks * 4] * dv;   // pole scaling folded into the B fragment
+        const double b = wj[L::j_off(bj * 8, ks * 4)] * dv;   // pole scaling folded into the B fragment
 #pragma unroll
         for (int bi = 0; bi < NRB; ++bi) dmma884(acc[bi][bj][0], acc[bi][bj][1], a[bi], b);
       }
@@ -142,7 +144,7 @@ __device__ __forceinline__ void consume_off(const ItemInfo &it, const unsigned c
 // DIAG tile: 64 x 64 block on the diagonal; only 8x8 blocks (bi <= bj) are computed, and in
 // blocks on the diagonal only elements c >= r are stored (with their mirror), so that
 // R[n][m] == R[m][n] bitwise.
-template <int NB>
+template <int NB, bool TR>
 __device__ __forceinline__ void consume_diag(const ItemInfo &it, const unsigned char *smem, PipeState &ps,
                                              uint32_t full0, uint32_t empty0, int warp, int lane) {
   double acc[NB * (NB + 1) / 2][2];
@@ -151,15 +153,16 @@ __device__ __forceinline__ void consume_diag(const ItemInfo &it, const unsigned 
   const int g = lane >> 2, q = lane & 3;
   for (int kt = 0; kt < it.n_kt; ++kt) {
     mbar_wait(full0 + 8 * ps.stage, ps.phase);
-    const double *wi = reinterpret_cast<const double *>(smem + ps.stage * STAGE_BYTES) + g * KT + q;
-    const double *dd = reinterpret_cast<const double *>(smem + ps.stage * STAGE_BYTES + WI_BYTES + WJ_BYTES) +
-                       warp * KT + q;
+    using L = StageLayout<TR>;
+    const double *st = reinterpret_cast<const double *>(smem + ps.stage * STAGE_BYTES);
+    const double *wi = st + L::i_off(g, q);
+    const double *dd = st + L::D_BASE + warp * KT + q;
 #pragma unroll
     for (int ks = 0; ks < KT / 4; ++ks) {
       const double dv = dd[ks * 4];
       double a[NB];
 #pragma unroll
-      for (int bi = 0; bi < NB; ++bi) a[bi] = wi[bi * 8 * KT + ks * 4];
+      for (int bi = 0; bi < NB; ++bi) a[bi] = wi[L::i_off(bi * 8, ks * 4)];
 #pragma unroll
       for (int bj = 0; bj < NB; ++bj) {
         const double b = a[bj] * dv;
@@ -197,36 +200,41 @@ __device__ __forceinline__ void consume_diag(const ItemInfo &it, const unsigned 
 
 // The tile shapes are compile-time variants (no predicates inside the DMMA loop); ragged edges of
 // a wave pick the variant with fewer 8-wide blocks.
-__device__ __forceinline__ void consume_item(const ItemInfo &it, const unsigned char *smem, PipeState &ps,
-                                             uint32_t full0, uint32_t empty0, int warp, int lane) {
+template <bool TR>
+__device__ __forceinline__ void consume_item_layout(const ItemInfo &it, const unsigned char *smem, PipeState &ps,
+                                                    uint32_t full0, uint32_t empty0, int warp, int lane) {
   if (it.kind == 0) {
     switch (it.nblk) {
-      case 8: consume_diag<8>(it, smem, ps, full0, empty0, warp, lane); break;
-      case 7: consume_diag<7>(it, smem, ps, full0, empty0, warp, lane); break;
-      case 6: consume_diag<6>(it, smem, ps, full0, empty0, warp, lane); break;
-      case 5: consume_diag<5>(it, smem, ps, full0, empty0, warp, lane); break;
-      case 4: consume_diag<4>(it, smem, ps, full0, empty0, warp, lane); break;
-      case 3: consume_diag<3>(it, smem, ps, full0, empty0, warp, lane); break;
-      case 2: consume_diag<2>(it, smem, ps, full0, empty0, warp, lane); break;
-      default: consume_diag<1>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 8: consume_diag<8, TR>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 7: consume_diag<7, TR>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 6: consume_diag<6, TR>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 5: consume_diag<5, TR>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 4: consume_diag<4, TR>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 3: consume_diag<3, TR>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 2: consume_diag<2, TR>(it, smem, ps, full0, empty0, warp, lane); break;
+      default: consume_diag<1, TR>(it, smem, ps, full0, empty0, warp, lane); break;
+    }
+  } else if (it.nrb == 8) {
+    switch (it.nblk) {
+      case 4: consume_off<4, 8, TR>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 3: consume_off<3, 8, TR>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 2: consume_off<2, 8, TR>(it, smem, ps, full0, empty0, warp, lane); break;
+      default: consume_off<1, 8, TR>(it, smem, ps, full0, empty0, warp, lane); break;
     }
   } else {
-    if (it.nrb == 8) {
-      switch (it.nblk) {
-        case 4: consume_off<4, 8>(it, smem, ps, full0, empty0, warp, lane); break;
-        case 3: consume_off<3, 8>(it, smem, ps, full0, empty0, warp, lane); break;
-        case 2: consume_off<2, 8>(it, smem, ps, full0, empty0, warp, lane); break;
-        default: consume_off<1, 8>(it, smem, ps, full0, empty0, warp, lane); break;
-      }
-    } else {
-      switch (it.nblk) {
-        case 4: consume_off<4, 4>(it, smem, ps, full0, empty0, warp, lane); break;
-        case 3: consume_off<3, 4>(it, smem, ps, full0, empty0, warp, lane); break;
-        case 2: consume_off<2, 4>(it, smem, ps, full0, empty0, warp, lane); break;
-        default: consume_off<1, 4>(it, smem, ps, full0, empty0, warp, lane); break;
-      }
+    switch (it.nblk) {
+      case 4: consume_off<4, 4, TR>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 3: consume_off<3, 4, TR>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 2: consume_off<2, 4, TR>(it, smem, ps, full0, empty0, warp, lane); break;
+      default: consume_off<1, 4, TR>(it, smem, ps, full0, empty0, warp, lane); break;
     }
   }
+}
+
+__device__ __forceinline__ void consume_item(const ItemInfo &it, const unsigned char *smem, PipeState &ps,
+                                             uint32_t full0, uint32_t empty0, int warp, int lane) {
+  if (it.tr) consume_item_layout<true>(it, smem, ps, full0, empty0, warp, lane);
+  else consume_item_layout<false>(it, smem, ps, full0, empty0, warp, lane);
 }
 
 // ---- producer ----------------------------------------------------------------------------
@@ -283,6 +291,14 @@ __device__ __forceinline__ void stage_panel_plain(double *dst, const DevWave &w,
     const int r = idx / KT, kk = idx - r * KT;
     const int row = row0 + r, k = k0 + kk;
     dst[idx] = (row < w.n_chan && k < w.n_poles) ? __ldg(w.W + (size_t)row * w.ldw + k) : 0.0;
+  }
+}
+
+// The same for channel-contiguous W: one pole-major panel [KT][TR_PITCH] of 32 channels.
+__device__ __forceinline__ void stage_panel_plain_tr(double *dst, const DevWave &w, int row0, int k0, int lane) {
+  for (int kk = 0; kk < KT; ++kk) {
+    const int row = row0 + lane, k = k0 + kk;
+    dst[kk * TR_PITCH + lane] = (row < w.n_chan && k < w.n_poles) ? __ldg(w.W + (size_t)k * w.ldw + row) : 0.0;
   }
 }
 
@@ -377,7 +393,8 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
             ii.n_valid_e = n_valid;
             ii.row0 = row0;
             ii.col0 = col0;
-            ii.nrb = (short)nrb;
+            ii.nrb = (unsigned char)nrb;
+            ii.tr = (unsigned char)w.tr;
             ii.nblk = nblk;
             ii.n_kt = n_kt;
           }
@@ -389,27 +406,41 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
 
         const CUtensorMap *map = &w.map;
         const int i_boxes = nrb > TN / 8 ? 2 : 1;              // I panel: one or two boxes of 32 rows
-        const uint32_t tx_bytes = (i_boxes + (kind != 0 ? 1 : 0)) * BOX_BYTES;
-        for (int kt = 0; kt < n_kt; ++kt) {
-          const int k0 = kt * KT;
-          mbar_wait(empty0 + 8 * ps.stage, ps.phase ^ 1u);
-          unsigned char *st = smem + ps.stage * STAGE_BYTES;
-          const uint32_t full = full0 + 8 * ps.stage;
-          if (w.use_tma) {
+        const uint32_t tx_bytes = (i_boxes + (kind != 0 ? 1 : 0)) * (w.tr ? TR_BOX_BYTES : BOX_BYTES);
+        if (w.use_tma) {
+          // TMA box coordinates: (pole, channel) for pole-contiguous W, (channel, pole) for the H.DAT order
+          const int tr = w.tr;
+          const uint32_t box = tr ? TR_BOX_BYTES : BOX_BYTES;
+          for (int kt = 0; kt < n_kt; ++kt) {
+            const int k0 = kt * KT;
+            mbar_wait(empty0 + 8 * ps.stage, ps.phase ^ 1u);
             if (lane == 0) {
+              const uint32_t full = full0 + 8 * ps.stage;
+              const uint32_t dst = smem_u32(smem + ps.stage * STAGE_BYTES);
               mbar_arrive_expect_tx(full, tx_bytes);
-              const uint32_t dst = smem_u32(st);
-              tma_load_2d(dst, map, k0, row0, full);
-              if (i_boxes == 2) tma_load_2d(dst + BOX_BYTES, map, k0, row0 + TN, full);
-              if (kind != 0) tma_load_2d(dst + WI_BYTES, map, k0, col0, full);
+              tma_load_2d(dst, map, tr ? row0 : k0, tr ? k0 : row0, full);
+              if (i_boxes == 2) tma_load_2d(dst + box, map, tr ? row0 + TN : k0, tr ? k0 : row0 + TN, full);
+              if (kind != 0) tma_load_2d(dst + 2 * box, map, tr ? col0 : k0, tr ? k0 : col0, full);
             }
-          } else {
-            stage_panel_plain(reinterpret_cast<double *>(st), w, row0, i_boxes * TN, k0, lane);
-            if (kind != 0) stage_panel_plain(reinterpret_cast<double *>(st + WI_BYTES), w, col0, TN, k0, lane);
-            __syncwarp();
-            if (lane == 0) mbar_arrive(full);
+            ps.advance();
           }
-          ps.advance();
+        } else {
+          for (int kt = 0; kt < n_kt; ++kt) {
+            const int k0 = kt * KT;
+            mbar_wait(empty0 + 8 * ps.stage, ps.phase ^ 1u);
+            double *sd = reinterpret_cast<double *>(smem + ps.stage * STAGE_BYTES);
+            if (w.tr) {
+              stage_panel_plain_tr(sd, w, row0, k0, lane);
+              if (i_boxes == 2) stage_panel_plain_tr(sd + KT * TR_PITCH, w, row0 + TN, k0, lane);
+              if (kind != 0) stage_panel_plain_tr(sd + 2 * KT * TR_PITCH, w, col0, k0, lane);
+            } else {
+              stage_panel_plain(sd, w, row0, i_boxes * TN, k0, lane);
+              if (kind != 0) stage_panel_plain(sd + TM * KT, w, col0, TN, k0, lane);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(full0 + 8 * ps.stage);
+            ps.advance();
+          }
         }
       }
       // single-wave call with a pool counter: the last CTA to run dry hands the slot back zeroed
@@ -460,7 +491,8 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
             ek_next[t] = (ev[t] && k < it.n_poles) ? __ldg(it.E_k + k) : 0.0;
           }
           mbar_wait(empty0 + 8 * ps.stage, ps.phase ^ 1u);
-          double *dsm = reinterpret_cast<double *>(smem + ps.stage * STAGE_BYTES + WI_BYTES + WJ_BYTES);
+          double *dsm = reinterpret_cast<double *>(smem + ps.stage * STAGE_BYTES) +
+                        (it.tr ? StageLayout<true>::D_BASE : StageLayout<false>::D_BASE);
 #pragma unroll
           for (int t = 0; t < DT; ++t) {
             // 0 beyond n_poles / n_E so that zero-filled W columns stay zero
@@ -494,9 +526,9 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
 }
 
 // ---- verification kernel: eq. 4 term by term, one thread per R element ----------------------
-__global__ void rmat_naive_kernel(const double *__restrict__ W, long long ldw, const double *__restrict__ E_k,
-                                  const double *__restrict__ energies, int n_chan, int n_poles, long long n_elems,
-                                  double a, double *__restrict__ R_out) {
+__global__ void rmat_naive_kernel(const double *__restrict__ W, long long stride_n, long long stride_k,
+                                  const double *__restrict__ E_k, const double *__restrict__ energies, int n_chan,
+                                  int n_poles, long long n_elems, double a, double *__restrict__ R_out) {
   const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= n_elems) return;
   const long long cc = (long long)n_chan * n_chan;
@@ -504,10 +536,10 @@ __global__ void rmat_naive_kernel(const double *__restrict__ W, long long ldw, c
   const int rem = (int)(idx - e * cc);
   const int n = rem / n_chan, m = rem - n * n_chan;
   const double E = energies[e];
-  const double *wn = W + (size_t)n * ldw, *wm = W + (size_t)m * ldw;
+  const double *wn = W + (size_t)n * stride_n, *wm = W + (size_t)m * stride_n;
   double s = 0.0, c = 0.0;
   for (int k = 0; k < n_poles; ++k) {
-    const double t = __ddiv_rn(__dmul_rn(wn[k], wm[k]), __dsub_rn(E_k[k], E));
+    const double t = __ddiv_rn(__dmul_rn(wn[(size_t)k * stride_k], wm[(size_t)k * stride_k]), __dsub_rn(E_k[k], E));
     const double u = __dadd_rn(s, t);
     c = __dadd_rn(c, fabs(s) >= fabs(t) ? __dadd_rn(__dsub_rn(s, u), t) : __dadd_rn(__dsub_rn(t, u), s));
     s = u;

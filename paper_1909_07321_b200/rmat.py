@@ -15,10 +15,11 @@ from . import build as _build
 
 PSTGF_OK = 0
 PSTGF_TAIL_AUTO, PSTGF_TAIL_NONE, PSTGF_TAIL_ALL = 0, 1, 2
+PSTGF_W_POLE_CONTIGUOUS, PSTGF_W_CHANNEL_CONTIGUOUS = 0, 1
 _STATUS_NAMES = {0: "PSTGF_OK", 1: "PSTGF_ERR_INVALID_VALUE", 2: "PSTGF_ERR_ALIGNMENT", 3: "PSTGF_ERR_WORKSPACE",
                  4: "PSTGF_ERR_UNSUPPORTED_DEVICE", 5: "PSTGF_ERR_CUDA"}
 
-EXPORTS = ["pstgf_rmat_form", "pstgf_rmat_batch_workspace_bytes", "pstgf_rmat_form_batch", "pstgf_rmat_form_naive",
+EXPORTS = ["pstgf_rmat_form", "pstgf_rmat_form_hdat", "pstgf_rmat_batch_workspace_bytes", "pstgf_rmat_form_batch", "pstgf_rmat_form_naive",
            "pstgf_rmat_form_batch_host", "pstgf_rmat_set_tail_policy", "pstgf_fp64_probe", "pstgf_last_launch_count", "pstgf_status_string", "pstgf_last_cuda_error",
            "pstgf_version"]
 
@@ -30,7 +31,7 @@ class PstgfError(RuntimeError):
 
 
 class pstgf_wave_t(ctypes.Structure):
-    _fields_ = [("n_chan", ctypes.c_int), ("n_poles", ctypes.c_int), ("n_E", ctypes.c_int),
+    _fields_ = [("n_chan", ctypes.c_int), ("n_poles", ctypes.c_int), ("n_E", ctypes.c_int), ("w_layout", ctypes.c_int),
                 ("ldw", ctypes.c_longlong), ("a", ctypes.c_double),
                 ("W", ctypes.c_void_p), ("E_k", ctypes.c_void_p), ("energies", ctypes.c_void_p),
                 ("R_out", ctypes.c_void_p)]
@@ -59,7 +60,9 @@ def load(build_if_missing: bool = False):
     vp, ll, i, d, sz = ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
     lib.pstgf_rmat_form.argtypes = [vp, ll, vp, vp, i, i, i, d, vp, vp]
     lib.pstgf_rmat_form.restype = i
-    lib.pstgf_rmat_form_naive.argtypes = [vp, ll, vp, vp, i, i, i, d, vp, vp]
+    lib.pstgf_rmat_form_hdat.argtypes = [vp, ll, vp, vp, i, i, i, d, vp, vp]
+    lib.pstgf_rmat_form_hdat.restype = i
+    lib.pstgf_rmat_form_naive.argtypes = [vp, ll, vp, vp, i, i, i, d, vp, i, vp]
     lib.pstgf_rmat_form_naive.restype = i
     lib.pstgf_rmat_batch_workspace_bytes.argtypes = [ctypes.POINTER(pstgf_wave_t), i]
     lib.pstgf_rmat_batch_workspace_bytes.restype = sz
@@ -101,12 +104,19 @@ def _dev_f64(t: torch.Tensor, name: str):
     return t
 
 
-def _wave_struct(W, E_k, energies, a, R_out) -> pstgf_wave_t:
-    _dev_f64(W, "W"); _dev_f64(E_k, "E_k"); _dev_f64(energies, "energies"); _dev_f64(R_out, "R_out")
+def _w_dims(W, layout: int):
+    """(n_chan, n_poles, ldw) of a 2-D W tensor: [n_chan, n_poles] pole-contiguous, or, for
+    PSTGF_W_CHANNEL_CONTIGUOUS (the H.DAT record order), [n_poles, n_chan]."""
     if W.dim() != 2 or W.stride(1) != 1 and W.shape[1] > 1:
-        raise ValueError("W must be [n_chan, n_poles] with unit stride along poles")
-    n_chan, n_poles = int(W.shape[0]), int(W.shape[1])
-    ldw = int(W.stride(0)) if n_chan > 1 else max(n_poles, int(W.stride(0)))
+        raise ValueError("W must be 2-D with unit stride along its last dimension")
+    rows, cols = int(W.shape[0]), int(W.shape[1])
+    ldw = int(W.stride(0)) if rows > 1 else max(cols, int(W.stride(0)), 1)
+    return (cols, rows, ldw) if layout == PSTGF_W_CHANNEL_CONTIGUOUS else (rows, cols, ldw)
+
+
+def _wave_struct(W, E_k, energies, a, R_out, layout: int = PSTGF_W_POLE_CONTIGUOUS) -> pstgf_wave_t:
+    _dev_f64(W, "W"); _dev_f64(E_k, "E_k"); _dev_f64(energies, "energies"); _dev_f64(R_out, "R_out")
+    n_chan, n_poles, ldw = _w_dims(W, layout)
     n_E = int(energies.shape[0])
     if E_k.dim() != 1 or int(E_k.shape[0]) != n_poles or not E_k.is_contiguous():
         raise ValueError("E_k must be contiguous [n_poles]")
@@ -114,8 +124,8 @@ def _wave_struct(W, E_k, energies, a, R_out) -> pstgf_wave_t:
         raise ValueError("energies must be contiguous [n_E]")
     if tuple(R_out.shape) != (n_E, n_chan, n_chan) or not R_out.is_contiguous():
         raise ValueError("R_out must be contiguous [n_E, n_chan, n_chan]")
-    return pstgf_wave_t(n_chan, n_poles, n_E, ldw, float(a), W.data_ptr(), E_k.data_ptr(), energies.data_ptr(),
-                        R_out.data_ptr())
+    return pstgf_wave_t(n_chan, n_poles, n_E, int(layout), ldw, float(a), W.data_ptr(), E_k.data_ptr(),
+                        energies.data_ptr(), R_out.data_ptr())
 
 
 def pstgf_rmat_form(W, E_k, energies, a: float, R_out=None, stream=None) -> torch.Tensor:
@@ -134,23 +144,37 @@ def pstgf_rmat_form(W, E_k, energies, a: float, R_out=None, stream=None) -> torc
     return R_out
 
 
-def pstgf_rmat_form_naive(W, E_k, energies, a: float, R_out=None, stream=None) -> torch.Tensor:
-    """Same result from the library's term-by-term verification kernel (slow)."""
+def pstgf_rmat_form_hdat(Wt, E_k, energies, a: float, R_out=None, stream=None) -> torch.Tensor:
+    """pstgf_rmat_form for W in the H.DAT record order: Wt [n_poles, n_chan], channels contiguous."""
     lib = load()
     if R_out is None:
-        R_out = torch.empty((energies.shape[0], W.shape[0], W.shape[0]), dtype=torch.float64, device=W.device)
-    w = _wave_struct(W, E_k, energies, a, R_out)
+        R_out = torch.empty((energies.shape[0], Wt.shape[1], Wt.shape[1]), dtype=torch.float64, device=Wt.device)
+    w = _wave_struct(Wt, E_k, energies, a, R_out, PSTGF_W_CHANNEL_CONTIGUOUS)
+    with torch.cuda.device(Wt.device):
+        _check(lib.pstgf_rmat_form_hdat(w.W, w.ldw, w.E_k, w.energies, w.n_chan, w.n_poles, w.n_E, w.a, w.R_out,
+                                        _stream_ptr(stream)))
+    return R_out
+
+
+def pstgf_rmat_form_naive(W, E_k, energies, a: float, R_out=None, stream=None,
+                          layout: int = PSTGF_W_POLE_CONTIGUOUS) -> torch.Tensor:
+    """Same result from the library's term-by-term verification kernel (slow)."""
+    lib = load()
+    n_chan = W.shape[1] if layout == PSTGF_W_CHANNEL_CONTIGUOUS else W.shape[0]
+    if R_out is None:
+        R_out = torch.empty((energies.shape[0], n_chan, n_chan), dtype=torch.float64, device=W.device)
+    w = _wave_struct(W, E_k, energies, a, R_out, layout)
     with torch.cuda.device(W.device):
         _check(lib.pstgf_rmat_form_naive(w.W, w.ldw, w.E_k, w.energies, w.n_chan, w.n_poles, w.n_E, w.a, w.R_out,
-                                         _stream_ptr(stream)))
+                                         int(layout), _stream_ptr(stream)))
     return R_out
 
 
 def make_wave_array(waves: Sequence[tuple]) -> "ctypes.Array[pstgf_wave_t]":
-    """waves: sequence of (W, E_k, energies, a, R_out) tuples of CUDA tensors."""
+    """waves: sequence of (W, E_k, energies, a, R_out[, w_layout]) tuples of CUDA tensors."""
     arr = (pstgf_wave_t * len(waves))()
-    for p, (W, E_k, energies, a, R_out) in enumerate(waves):
-        arr[p] = _wave_struct(W, E_k, energies, a, R_out)
+    for p, wv in enumerate(waves):
+        arr[p] = _wave_struct(*wv)
     return arr
 
 
@@ -171,17 +195,19 @@ def pstgf_rmat_form_batch(wave_array, workspace: torch.Tensor, stream=None, n_wa
 
 
 def pstgf_rmat_form_batch_host(host_waves: Sequence[tuple], max_chunk_bytes: int = 0, stream=None) -> None:
-    """End-to-end call over HOST tensors (pinned recommended): (W, E_k, energies, a, R_out) per wave, all CPU
-    float64 contiguous tensors; R_out is filled on return (the call synchronises)."""
+    """End-to-end call over HOST tensors (pinned recommended): (W, E_k, energies, a, R_out[, w_layout]) per wave,
+    all CPU float64 contiguous tensors; R_out is filled on return (the call synchronises)."""
     lib = load()
     arr = (pstgf_wave_t * len(host_waves))()
-    for p, (W, E_k, energies, a, R_out) in enumerate(host_waves):
+    for p, wv in enumerate(host_waves):
+        W, E_k, energies, a, R_out = wv[:5]
+        layout = int(wv[5]) if len(wv) > 5 else PSTGF_W_POLE_CONTIGUOUS
         for t, nm in ((W, "W"), (E_k, "E_k"), (energies, "energies"), (R_out, "R_out")):
             if t.dtype != torch.float64 or t.is_cuda or not t.is_contiguous():
                 raise TypeError(f"{nm} must be a contiguous CPU float64 tensor")
-        n_chan, n_poles = int(W.shape[0]), int(W.shape[1])
-        arr[p] = pstgf_wave_t(n_chan, n_poles, int(energies.shape[0]), max(n_poles, 1) if n_chan <= 1 else int(W.stride(0)),
-                              float(a), W.data_ptr(), E_k.data_ptr(), energies.data_ptr(), R_out.data_ptr())
+        n_chan, n_poles, ldw = _w_dims(W, layout)
+        arr[p] = pstgf_wave_t(n_chan, n_poles, int(energies.shape[0]), layout, ldw, float(a), W.data_ptr(), E_k.data_ptr(),
+                              energies.data_ptr(), R_out.data_ptr())
     _check(lib.pstgf_rmat_form_batch_host(arr, len(host_waves), int(max_chunk_bytes), _stream_ptr(stream)))
 
 

@@ -64,7 +64,7 @@ def test_wave_struct_layout_matches_binding():
     from paper_1909_07321_b200 import rmat
     assert ctypes.sizeof(rmat.pstgf_wave_t) == 64
     off = {n: getattr(rmat.pstgf_wave_t, n).offset for n, _ in rmat.pstgf_wave_t._fields_}
-    assert off == {"n_chan": 0, "n_poles": 4, "n_E": 8, "ldw": 16, "a": 24, "W": 32, "E_k": 40, "energies": 48,
+    assert off == {"n_chan": 0, "n_poles": 4, "n_E": 8, "w_layout": 12, "ldw": 16, "a": 24, "W": 32, "E_k": 40, "energies": 48,
                    "R_out": 56}
 
 
@@ -95,6 +95,18 @@ def test_argument_errors_need_no_device(lib):
     assert lib.pstgf_rmat_form(fake + 4, 6, fake, fake, 4, 6, 1, 20.0, fake, None) == 2  # misaligned
     assert lib.pstgf_rmat_form(fake, 6, fake, fake, 0, 6, 1, 20.0, fake, None) == 0     # n_chan == 0: nothing to do
     assert lib.pstgf_rmat_form(fake, 6, fake, fake, 4, 6, 0, 20.0, fake, None) == 0     # n_E == 0
+    # H.DAT record order: the leading dimension runs over channels
+    lib.pstgf_rmat_form_hdat.argtypes = [vp, ll, vp, vp, i, i, i, d, vp, vp]
+    lib.pstgf_rmat_form_hdat.restype = i
+    assert lib.pstgf_rmat_form_hdat(fake, 3, fake, fake, 4, 6, 1, 20.0, fake, None) == 1   # ldw < n_chan
+    assert lib.pstgf_rmat_form_hdat(fake, 4, fake, fake, 4, 6, 0, 20.0, fake, None) == 0   # n_E == 0
+    lib.pstgf_rmat_form_naive.argtypes = [vp, ll, vp, vp, i, i, i, d, vp, i, vp]
+    lib.pstgf_rmat_form_naive.restype = i
+    assert lib.pstgf_rmat_form_naive(fake, 6, fake, fake, 4, 6, 1, 20.0, fake, 7, None) == 1   # unknown w_layout
+    lib.pstgf_rmat_set_tail_policy.argtypes = [i]
+    lib.pstgf_rmat_set_tail_policy.restype = i
+    assert lib.pstgf_rmat_set_tail_policy(5) == 1
+    assert lib.pstgf_rmat_set_tail_policy(0) == 0
 
 
 def test_no_device_is_an_error_not_a_fallback(lib):

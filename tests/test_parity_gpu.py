@@ -138,6 +138,68 @@ def test_tail_split_inside_a_wave(rmat, oracle, tail_policy):
     _check(Rs[1].cpu().numpy(), oracle.rmat_form(w2.W, w2.E_k, w2.energies, w2.a, threads=_threads()))
 
 
+# ---- W in the H.DAT record order (channels fastest, one pole after the other) ----------------
+HDAT_SHAPES = [(1, 1, 1), (7, 5, 3), (8, 20, 8), (31, 21, 2), (34, 45, 9), (64, 80, 8), (65, 61, 5), (70, 100, 17),
+               (97, 77, 9), (128, 60, 3), (130, 41, 10), (200, 104, 7), (257, 50, 2)]
+
+
+@pytest.mark.parametrize("C,K,N", HDAT_SHAPES)
+def test_hdat_order_edge_shapes(rmat, oracle, tail_policy, C, K, N):
+    """Channel-contiguous W: even n_chan takes the TMA boxes of 36 channels x 20 poles, odd n_chan the plain
+    staging path and, re-pitched to an even leading dimension, the TMA path again.  Same bits as the
+    pole-contiguous call under every tiling."""
+    from paper_1909_07321_b200 import inputs
+    w = inputs.make_wave(3000 + C * 5 + K, C, K, N)
+    R_ref = oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads())
+    Ek, en = _dev(w.E_k), _dev(w.energies)
+    Wt = _dev(w.W.T)                                  # [n_poles][n_chan], ldw = n_chan
+    pitched = torch.zeros((K, C + 1 + (C + 1) % 2), dtype=torch.float64, device="cuda")
+    pitched[:, :C].copy_(Wt)
+    R_plain = _form(rmat, w)
+    for policy in (rmat.PSTGF_TAIL_NONE, rmat.PSTGF_TAIL_ALL, rmat.PSTGF_TAIL_AUTO):
+        tail_policy(policy)
+        for Wdev in (Wt, pitched[:, :C]):
+            R = rmat.pstgf_rmat_form_hdat(Wdev, Ek, en, w.a)
+            torch.cuda.synchronize()
+            R = R.cpu().numpy()
+            _check(R, R_ref)
+            assert np.array_equal(R, R_plain)
+    Rn = rmat.pstgf_rmat_form_naive(Wt, Ek, en, w.a, layout=rmat.PSTGF_W_CHANNEL_CONTIGUOUS).cpu().numpy()
+    _check(Rn, R_ref, tol=1e-15)
+
+
+def test_hdat_order_in_batch_and_host_call(rmat, oracle):
+    """A batch mixing both memory orders, through the device batch call and the host end-to-end call."""
+    from paper_1909_07321_b200 import inputs
+    waves = [inputs.make_wave(31, 150, 300, 19), inputs.make_wave(32, 72, 144, 33), inputs.make_wave(33, 40, 61, 8)]
+    layouts = [rmat.PSTGF_W_CHANNEL_CONTIGUOUS, rmat.PSTGF_W_POLE_CONTIGUOUS, rmat.PSTGF_W_CHANNEL_CONTIGUOUS]
+    refs = [oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads()) for w in waves]
+    dev, host = [], []
+    for w, lay in zip(waves, layouts):
+        Wh = np.ascontiguousarray(w.W.T) if lay == rmat.PSTGF_W_CHANNEL_CONTIGUOUS else w.W
+        R = torch.empty((w.n_E, w.n_chan, w.n_chan), dtype=torch.float64, device="cuda")
+        dev.append((_dev(Wh), _dev(w.E_k), _dev(w.energies), w.a, R, lay))
+        Rh = torch.full((w.n_E, w.n_chan, w.n_chan), np.nan, dtype=torch.float64).pin_memory()
+        host.append((torch.from_numpy(Wh).pin_memory(), torch.from_numpy(w.E_k).pin_memory(),
+                     torch.from_numpy(w.energies).pin_memory(), w.a, Rh, lay))
+    arr = rmat.make_wave_array(dev)
+    ws = torch.empty(rmat.pstgf_rmat_batch_workspace_bytes(arr), dtype=torch.uint8, device="cuda")
+    rmat.pstgf_rmat_form_batch(arr, ws)
+    torch.cuda.synchronize()
+    rmat.pstgf_rmat_form_batch_host(host, max_chunk_bytes=150 * 150 * 8 * 8)
+    for d, h, ref in zip(dev, host, refs):
+        _check(d[4].cpu().numpy(), ref)
+        assert np.array_equal(d[4].cpu().numpy(), h[4].numpy())
+
+
+def test_hdat_order_config2_every_energy(rmat, oracle):
+    from paper_1909_07321_b200 import inputs
+    w = inputs.make_config(2).waves[0]
+    R = rmat.pstgf_rmat_form_hdat(_dev(w.W.T), _dev(w.E_k), _dev(w.energies), w.a)
+    torch.cuda.synchronize()
+    _check(R.cpu().numpy(), oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads()))
+
+
 def test_many_launches_in_flight(rmat, oracle):
     """More single-wave launches in flight than the counter pool has slots (64), on several streams: every
     launch must still do all of its items exactly once (pool slot or round-robin fallback)."""
