@@ -47,6 +47,10 @@ def parse_args():
     ap.add_argument("--w-layout", choices=["poles", "channels"], default="poles",
                     help="memory order of W on the device: pole-contiguous [n_chan][n_poles] (default, north_star's) or "
                          "channel-contiguous [n_poles][n_chan], the H.DAT record order of PAPER.md:535")
+    ap.add_argument("--prior-art", action="store_true",
+                    help="also time the paper's own GPU scheme (PAPER.md:164-166: scaled copy, 10 upper-triangle block "
+                         "multiplies per energy, symmetrise) with cuBLAS DGEMM through torch.matmul: context, not a path "
+                         "of the library")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
@@ -257,6 +261,80 @@ def ncu_traffic(cfg: int):
     return None
 
 
+# ---- prior art on the same GPU (context) ---------------------------------------------------------
+def prior_art_leg(wl, n_sample: int = 16) -> dict:
+    """The scheme the paper describes for its CUDA-Fortran RINIT (Fig. 2), with a library DGEMM
+    (cuBLAS through torch.matmul, float64) standing in for its matrix-multiply routine: per energy, form the scaled
+    copy W diag(d), compute the 10 upper-triangle blocks of a 4 x 4 block grid one after another, symmetrise.
+    Timed on the first `n_sample` energies of every wave with CUDA events; every energy costs the same."""
+    import torch
+    total_ms, n_done, worst = 0.0, 0, 0.0
+    for w in wl.waves:
+        W = torch.from_numpy(w.W).cuda()
+        Ek = torch.from_numpy(w.E_k).cuda()
+        en = torch.from_numpy(w.energies).cuda()
+        C = w.n_chan
+        cuts = [round(i * C / 4) for i in range(5)]
+        blocks = [(cuts[i], cuts[i + 1]) for i in range(4) if cuts[i + 1] > cuts[i]]
+        k = min(n_sample, w.n_E)
+        R = torch.empty((k, C, C), dtype=torch.float64, device="cuda")
+
+        def form(e):
+            Ws = W * (1.0 / (Ek - en[e]))                       # the scaled operand, a full copy in HBM
+            for bi, (r0, r1) in enumerate(blocks):
+                for (c0, c1) in blocks[bi:]:
+                    blk = torch.matmul(W[r0:r1], Ws[c0:c1].t())
+                    R[e, r0:r1, c0:c1] = blk
+                    if c0 != r0:
+                        R[e, c0:c1, r0:r1] = blk.t()            # "symmetrised to provide the full result"
+            R[e].mul_(1.0 / (2.0 * w.a))
+
+        for e in range(min(3, k)):
+            form(e)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for e in range(k):
+            form(e)
+        e1.record()
+        torch.cuda.synchronize()
+        total_ms += e0.elapsed_time(e1)
+        n_done += k
+    # a stronger library baseline: scaled copies of 8 energies at once and ONE batched DGEMM for the full squares
+    b_ms, b_done = 0.0, 0
+    for w in wl.waves:
+        W = torch.from_numpy(w.W).cuda()
+        Ek = torch.from_numpy(w.E_k).cuda()
+        en = torch.from_numpy(w.energies).cuda()
+        k = min(n_sample, w.n_E)
+        k -= k % 8 if k >= 8 else 0
+        Rb = torch.empty((k, w.n_chan, w.n_chan), dtype=torch.float64, device="cuda")
+
+        def form_batched():
+            for e in range(0, k, 8):
+                d = 1.0 / (Ek[None, :] - en[e:e + 8, None])                    # [8, K]
+                torch.matmul(W[None] * d[:, None, :], W.t(), out=Rb[e:e + 8])   # [8, C, K] scaled copies, batched DGEMM
+            Rb.mul_(1.0 / (2.0 * w.a))
+
+        form_batched()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        form_batched()
+        e1.record()
+        torch.cuda.synchronize()
+        b_ms += e0.elapsed_time(e1)
+        b_done += k
+    flop = sum(min(n_sample, w.n_E) * w.n_chan ** 2 * w.n_poles for w in wl.waves)
+    return {"cublas_batched": {"value": b_done / (b_ms * 1e-3), "unit": UNIT,
+                               "kind": "scaled copies of 8 energies + one batched cuBLAS DGEMM of the full squares (torch.matmul)",
+                               "sample": f"{b_done} energies, {b_ms:.2f} ms"},
+            "value": n_done / (total_ms * 1e-3), "unit": UNIT, "kind": "paper's scheme (PAPER.md:164-166) with cuBLAS DGEMM via "
+            "torch.matmul: scaled copy + 10 upper-triangle block multiplies + symmetrise, one energy at a time",
+            "sample": f"first {n_sample} energies of each wave ({n_done} energies, {total_ms:.2f} ms)",
+            "tflops_counted": flop / (total_ms * 1e-3) / 1e12}
+
+
 # ---- CUDA arm ----------------------------------------------------------------------------------
 def run_cuda(args):
     import numpy as np
@@ -437,6 +515,12 @@ def run_cuda(args):
                "api": "pstgf_rmat_form_batch_host (pinned host buffers; whole R copied back)"}
         del host
 
+    prior = None
+    if rank == 0 and world == 1 and args.prior_art:
+        del dev_waves
+        torch.cuda.empty_cache()
+        prior = prior_art_leg(wl)
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline(wl, args.cpu_seconds)
@@ -454,6 +538,7 @@ def run_cuda(args):
                                sha256=wl.sha256()[:16]),
                 "tflops_counted": world * flop * args.steps / (total_ms_max * 1e-3) / 1e12,   # ranks carry equal shares
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,
+                **({"prior_art": prior} if prior else {}),
                 "clocks": clocks, "wall_s_timed_region": wall, "step_ms_min_max": [min(step_ms), max(step_ms)]}
         print(json.dumps(line), flush=True)
     if world > 1:
