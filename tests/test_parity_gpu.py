@@ -200,6 +200,33 @@ def test_hdat_order_config2_every_energy(rmat, oracle):
     _check(R.cpu().numpy(), oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads()))
 
 
+def test_single_wave_call_in_a_cuda_graph(rmat, oracle):
+    """Under stream capture the single-wave call must not touch its counter pool (a replayed launch would
+    reuse a slot it no longer owns): it falls back to round-robin item assignment.  Captured once, replayed
+    several times, also while ordinary launches are in flight; same bits as the eager call."""
+    from paper_1909_07321_b200 import inputs
+    w = inputs.make_wave(4711, 137, 260, 27)
+    Wd, Ek, en = _dev(w.W), _dev(w.E_k), _dev(w.energies)
+    R_ref = oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads())
+    eager = rmat.pstgf_rmat_form(Wd, Ek, en, w.a)
+    torch.cuda.synchronize()
+    out = torch.zeros_like(eager)
+    g = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(g, stream=side):
+            rmat.pstgf_rmat_form(Wd, Ek, en, w.a, R_out=out, stream=side)
+    torch.cuda.current_stream().wait_stream(side)
+    for _ in range(3):
+        out.zero_()
+        g.replay()
+        other = rmat.pstgf_rmat_form(Wd, Ek, en, w.a)          # an eager launch beside the replay
+        torch.cuda.synchronize()
+        assert torch.equal(out, eager) and torch.equal(other, eager)
+    _check(out.cpu().numpy(), R_ref)
+
+
 def test_many_launches_in_flight(rmat, oracle):
     """More single-wave launches in flight than the counter pool has slots (64), on several streams: every
     launch must still do all of its items exactly once (pool slot or round-robin fallback)."""
