@@ -51,6 +51,9 @@ def parse_args():
                     help="also time the paper's own GPU scheme (PAPER.md:164-166: scaled copy, 10 upper-triangle block "
                          "multiplies per energy, symmetrise) with cuBLAS DGEMM through torch.matmul: context, not a path "
                          "of the library")
+    ap.add_argument("--tail-policy", choices=["auto", "none", "all"], default="auto",
+                    help="scheduling knob of the library (pstgf_rmat_set_tail_policy): fine-tile tail sized automatically "
+                         "(default), coarse tiles only, fine tiles only; same bits, for measurements")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
@@ -352,6 +355,8 @@ def run_cuda(args):
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     rmat.load()          # raises if libpstgf_rmat.so is missing
+    rmat.pstgf_rmat_set_tail_policy({"auto": rmat.PSTGF_TAIL_AUTO, "none": rmat.PSTGF_TAIL_NONE,
+                                     "all": rmat.PSTGF_TAIL_ALL}[args.tail_policy])
     peaks = measured_peaks()
 
     # Weak scaling over ranks: at N ranks the job is the configuration with an N times
@@ -535,7 +540,7 @@ def run_cuda(args):
                 "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": vs_baseline, "dtype": "f64", "data": "synthetic",
                 "config": dict(workload_description(args.config, wl), n_energies_per_step=n_e_job, n_energies_per_rank=n_e,
-                               l2="flushed between timed steps (512 MiB write)", w_layout=args.w_layout,
+                               l2="flushed between timed steps (512 MiB write)", w_layout=args.w_layout, tail_policy=args.tail_policy,
                                sha256=wl.sha256()[:16]),
                 "tflops_counted": world * flop * args.steps / (total_ms_max * 1e-3) / 1e12,   # ranks carry equal shares
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,

@@ -8,6 +8,9 @@
 #include <atomic>
 #include <cmath>
 #include <cstring>
+#include <map>
+#include <queue>
+#include <tuple>
 #include <mutex>
 #include <numeric>
 #include <vector>
@@ -143,6 +146,86 @@ double cost_per_energy_block(const DevWave &d) {
   return (double)d.n_kt * ((double)d.n_i * pstgf::COST_DIAG + (double)(d.n_tiles - d.n_i) * pstgf::COST_OFF);
 }
 
+// ---- tail size of a single wave by simulation ------------------------------------------------------
+// Relative cost of one 8x8 block per k-step in the four tile kinds, fitted to sweeps of the tail size on the
+// B200 (configs 2 and 5; the fit reproduces the measured step times to 0.2 %): coarse OFF 1, coarse DIAG 1.04
+// (8 DMUL per 36 DMMA), fine OFF32 1.03, fine DIAG32 1.2 (4 DMUL per 10 DMMA and a stage consumed in a
+// quarter of the time).
+constexpr double BLK_OFF = 1.0, BLK_DIAG = 1.04, BLK_OFF32 = 1.03, BLK_DIAG32 = 1.2;
+
+// Item costs of one wave in the order the counter hands them out, with `t` energy blocks in the fine tail.
+void item_costs(const DevWave &d, int t, std::vector<std::pair<double, int>> &runs) {
+  runs.clear();
+  const int C = d.n_chan, n_c = d.n_eb - t;
+  auto blocks8 = [&](int first, int cap) { return std::min(cap, (C - first + 7) / 8); };
+  if (n_c > 0) {
+    for (int i = 0; i < d.n_i; ++i) {
+      const int nb = blocks8(pstgf::TM * i, pstgf::TM / 8);
+      runs.emplace_back(BLK_DIAG * nb * (nb + 1) / 2, n_c);
+    }
+    for (int i = 0; i < d.n_i; ++i)
+      for (int j = 2 * i + 2; j < d.n_j; ++j) runs.emplace_back(BLK_OFF * 8 * blocks8(pstgf::TN * j, pstgf::TN / 8), n_c);
+  }
+  if (t > 0) {
+    for (int i = 0; i < d.n_j; ++i)
+      for (int j = i + 1; j < d.n_j; ++j) runs.emplace_back(BLK_OFF32 * 4 * blocks8(pstgf::TN * j, pstgf::TN / 8), t);
+    for (int i = 0; i < d.n_j; ++i) {
+      const int nb = blocks8(pstgf::TN * i, pstgf::TN / 8);
+      runs.emplace_back(BLK_DIAG32 * nb * (nb + 1) / 2, t);
+    }
+  }
+}
+
+// Makespan of greedy list scheduling (what the atomic counter does) of those items on `grid` CTAs.
+double simulate_makespan(const std::vector<std::pair<double, int>> &runs, int grid) {
+  std::priority_queue<double, std::vector<double>, std::greater<double>> free_at;
+  for (int b = 0; b < grid; ++b) free_at.push(0.0);
+  double last = 0.0;
+  for (const auto &r : runs)
+    for (int n = 0; n < r.second; ++n) {
+      const double f = free_at.top() + r.first;
+      free_at.pop();
+      free_at.push(f);
+      last = std::max(last, f);
+    }
+  return last;
+}
+
+std::mutex g_tail_mutex;
+std::map<std::tuple<int, int, int>, int> g_tail_cache;   // (n_chan, n_eb, grid) -> energy blocks in the fine tail
+
+// Tail size of a single wave: the candidate with the smallest simulated makespan among up to 17 sizes between
+// 0 and twice the heuristic budget.  Cached per shape (the cost does not depend on n_poles: every item of a wave
+// has the same number of k-steps).  Returns -1 when the wave has too many items for a simulation to be worth its
+// host time (then the tail matters little anyway).
+int best_tail_single_wave(const DevWave &d, int grid, double budget) {
+  const long long items = (long long)d.n_tiles * d.n_eb;
+  if (items > 8192) return -1;
+  const auto key = std::make_tuple(d.n_chan, d.n_eb, grid);
+  {
+    std::lock_guard<std::mutex> lock(g_tail_mutex);
+    auto it = g_tail_cache.find(key);
+    if (it != g_tail_cache.end()) return it->second;
+  }
+  const double per_eb = cost_per_energy_block(d) / std::max(1, d.n_kt);
+  const int t_max = (int)std::min<double>((double)d.n_eb, std::ceil(2.0 * budget / std::max(1, d.n_kt) / per_eb) + 1.0);
+  const int stride = std::max(1, t_max / 16);
+  std::vector<std::pair<double, int>> runs;
+  int best_t = 0;
+  double best = 0.0;
+  for (int t = 0; t <= t_max; t += stride) {
+    item_costs(d, t, runs);
+    const double m = simulate_makespan(runs, grid);
+    if (t == 0 || m < best * (1.0 - 1e-9)) {
+      best = m;
+      best_t = t;
+    }
+  }
+  std::lock_guard<std::mutex> lock(g_tail_mutex);
+  g_tail_cache[key] = best_t;
+  return best_t;
+}
+
 // Tail of the schedule (see rmat_common.h): about one round of the grid's worth of work, taken from the
 // END of the largest-first order, is cut into fine tiles so that list scheduling finishes on small items.
 void plan_tails(std::vector<DevWave> &ds, int grid) {
@@ -155,6 +238,13 @@ void plan_tails(std::vector<DevWave> &ds, int grid) {
   double c_max = 0.0;
   for (const DevWave &d : ds) c_max = std::max(c_max, largest_item_cost(d));
   double budget = c_max * grid;
+  if (ds.size() == 1) {
+    const int t = best_tail_single_wave(ds[0], grid, c_max * grid);
+    if (t >= 0) {
+      ds[0].n_eb_coarse = ds[0].n_eb - t;
+      return;
+    }
+  }
   for (size_t q = ds.size(); q-- > 0 && budget > 0.0;) {
     DevWave &d = ds[q];
     const double per_eb = cost_per_energy_block(d);
