@@ -122,9 +122,7 @@ void plan_wave(const pstgf_wave_t &w, DevWave &d) {
   d.n_i = (w.n_chan + pstgf::TM - 1) / pstgf::TM;
   d.n_j = (w.n_chan + pstgf::TN - 1) / pstgf::TN;
   d.n_eb = (w.n_E + pstgf::EB - 1) / pstgf::EB;
-  int tiles = d.n_i;
-  for (int i = 0; i < d.n_i; ++i) tiles += pstgf::off_tiles_in_row(d.n_j, i);
-  d.n_tiles = tiles;
+  d.n_tiles = pstgf::coarse_tiles(w.n_chan);
   d.n_eb_coarse = d.n_eb;
   d.tr = w.w_layout == PSTGF_W_CHANNEL_CONTIGUOUS ? 1 : 0;
   d.use_tma = ((reinterpret_cast<uintptr_t>(w.W) & 15u) == 0 && (w.ldw % 2) == 0 && w.ldw * 8 < (1LL << 40)) ? 1 : 0;
@@ -151,7 +149,7 @@ double cost_per_energy_block(const DevWave &d) {
 // B200 (configs 2 and 5; the fit reproduces the measured step times to 0.2 %): coarse OFF 1, coarse DIAG 1.04
 // (8 DMUL per 36 DMMA), fine OFF32 1.03, fine DIAG32 1.2 (4 DMUL per 10 DMMA and a stage consumed in a
 // quarter of the time).
-constexpr double BLK_OFF = 1.0, BLK_DIAG = 1.04, BLK_OFF32 = 1.03, BLK_DIAG32 = 1.2;
+constexpr double BLK_OFF = 1.0, BLK_WIDE = 0.985, BLK_DIAG = 1.04, BLK_OFF32 = 1.03, BLK_DIAG32 = 1.2;
 
 // Item costs of one wave in the order the counter hands them out, with `t` energy blocks in the fine tail.
 void item_costs(const DevWave &d, int t, std::vector<std::pair<double, int>> &runs) {
@@ -163,8 +161,12 @@ void item_costs(const DevWave &d, int t, std::vector<std::pair<double, int>> &ru
       const int nb = blocks8(pstgf::TM * i, pstgf::TM / 8);
       runs.emplace_back(BLK_DIAG * nb * (nb + 1) / 2, n_c);
     }
-    for (int i = 0; i < d.n_i; ++i)
-      for (int j = 2 * i + 2; j < d.n_j; ++j) runs.emplace_back(BLK_OFF * 8 * blocks8(pstgf::TN * j, pstgf::TN / 8), n_c);
+    for (int p = 0; pstgf::TW * p + pstgf::TM < C; ++p)
+      for (int c = 0; c < pstgf::wide_tiles_in_pair(C, p); ++c)
+        runs.emplace_back(BLK_WIDE * 16 * blocks8(pstgf::TW * (p + 1) + pstgf::TWN * c, pstgf::TWN / 8), n_c);
+    for (int p = 0; pstgf::TW * p + pstgf::TM < C; ++p)
+      for (int t2 = 0; t2 < pstgf::off_tiles_in_pair(C, p); ++t2)
+        runs.emplace_back(BLK_OFF * 8 * blocks8(pstgf::TW * p + pstgf::TM + pstgf::TN * t2, pstgf::TN / 8), n_c);
   }
   if (t > 0) {
     for (int i = 0; i < d.n_j; ++i)

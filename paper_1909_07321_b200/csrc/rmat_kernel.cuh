@@ -24,8 +24,8 @@ struct ItemInfo {        // handed from the load warp to the pole-scaling and co
   int n_poles;
   int n_valid_e;         // energies in this block (1..EB)
   int row0, col0;
-  short kind;            // 0 DIAG, 1 OFF, -1 stop
-  unsigned char nrb;     // OFF: 8-row blocks of the I panel (8 coarse, 4 fine)
+  short kind;            // 0 DIAG, 1 OFF / WIDE (rectangular, strictly above the diagonal), -1 stop
+  unsigned char nrb;     // rectangular tiles: 8-row blocks of the I panel (16 WIDE, 8 OFF, 4 fine OFF32)
   unsigned char tr;      // stage layout: 0 row-major panels, 1 pole-major panels (channel-contiguous W)
   int nblk;              // DIAG: valid 8x8 block rows/cols; OFF: valid 8-wide column blocks
   int n_kt;
@@ -89,8 +89,9 @@ __device__ __forceinline__ void consume_idle(int n_kt, PipeState &ps, uint32_t f
   }
 }
 
-// OFF tile: 64 x 32 (coarse, NRB = 8) or 32 x 32 (fine, NRB = 4) block strictly above the diagonal;
-// NRB x 4 DMMA blocks, all needed (column blocks >= nblk lie beyond n_chan and are skipped).
+// Rectangular tile strictly above the diagonal: WIDE 128 x 16 (NRB = 16, NCB <= 2), OFF 64 x 32 (NRB = 8) or
+// fine OFF32 32 x 32 (NRB = 4); NRB x NCB DMMA blocks, all needed (column blocks >= nblk lie beyond n_chan and
+// are skipped).  One scaled B fragment feeds NRB DMMAs: the WIDE shape halves the DMULs per DMMA of OFF.
 template <int NCB, int NRB, bool TR>
 __device__ __forceinline__ void consume_off(const ItemInfo &it, const unsigned char *smem, PipeState &ps,
                                             uint32_t full0, uint32_t empty0, int warp, int lane) {
@@ -214,6 +215,9 @@ __device__ __forceinline__ void consume_item_layout(const ItemInfo &it, const un
       case 2: consume_diag<2, TR>(it, smem, ps, full0, empty0, warp, lane); break;
       default: consume_diag<1, TR>(it, smem, ps, full0, empty0, warp, lane); break;
     }
+  } else if (it.nrb == 16) {
+    if (it.nblk == 2) consume_off<2, 16, TR>(it, smem, ps, full0, empty0, warp, lane);
+    else consume_off<1, 16, TR>(it, smem, ps, full0, empty0, warp, lane);
   } else if (it.nrb == 8) {
     switch (it.nblk) {
       case 4: consume_off<4, 8, TR>(it, smem, ps, full0, empty0, warp, lane); break;
@@ -261,26 +265,43 @@ __device__ __forceinline__ void decode_tile_fine(const DevWave &w, int tile, int
   }
 }
 
-// Coarse tile index inside a wave -> (kind, row0, col0, nblk).  DIAG tiles first (they are the most
-// expensive: 36 DMMA per k-step against 32), then OFF tiles row by row.
-__device__ __forceinline__ void decode_tile(const DevWave &w, int tile, int &kind, int &row0, int &col0, int &nblk) {
+// Coarse tile index inside a wave -> (kind, row0, col0, nblk, nrb).  DIAG tiles first (they are the most
+// expensive), then the WIDE tiles pair by pair, then the OFF squares inside the pairs.
+__device__ __forceinline__ void decode_tile(const DevWave &w, int tile, int &kind, int &row0, int &col0, int &nblk,
+                                            int &nrb) {
   if (tile < w.n_i) {
     kind = 0;
     row0 = col0 = tile * TM;
     const int left = w.n_chan - row0;
     nblk = left >= TM ? TM / 8 : (left + 7) / 8;
-  } else {
-    kind = 1;
-    int t = tile - w.n_i, i = 0;
-    for (;; ++i) {
-      const int cnt = off_tiles_in_row(w.n_j, i);
-      if (t < cnt) break;
-      t -= cnt;
+    nrb = nblk;
+    return;
+  }
+  kind = 1;
+  int t = tile - w.n_i;
+  for (int p = 0; TW * p + TM < w.n_chan; ++p) {
+    const int cnt = wide_tiles_in_pair(w.n_chan, p);
+    if (t < cnt) {
+      row0 = p * TW;
+      col0 = (p + 1) * TW + t * TWN;
+      const int left = w.n_chan - col0;
+      nblk = left >= TWN ? TWN / 8 : (left + 7) / 8;
+      nrb = TW / 8;
+      return;
     }
-    row0 = i * TM;
-    col0 = (2 * i + 2 + t) * TN;
-    const int left = w.n_chan - col0;
-    nblk = left >= TN ? TN / 8 : (left + 7) / 8;
+    t -= cnt;
+  }
+  for (int p = 0;; ++p) {
+    const int cnt = off_tiles_in_pair(w.n_chan, p);
+    if (t < cnt) {
+      row0 = p * TW;
+      col0 = p * TW + TM + t * TN;
+      const int left = w.n_chan - col0;
+      nblk = left >= TN ? TN / 8 : (left + 7) / 8;
+      nrb = TM / 8;
+      return;
+    }
+    t -= cnt;
   }
 }
 
@@ -373,9 +394,12 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
           const int n_eb_sec = fine ? w.n_eb - w.n_eb_coarse : w.n_eb_coarse;
           const int tile = (int)(item / n_eb_sec);
           eb = (int)(item - (long long)tile * n_eb_sec) + (fine ? w.n_eb_coarse : 0);
-          if (fine) decode_tile_fine(w, tile, kind, row0, col0, nblk);
-          else decode_tile(w, tile, kind, row0, col0, nblk);
-          nrb = kind == 0 ? nblk : (fine ? TN / 8 : TM / 8);   // 8-row blocks of the I panel that are read
+          if (fine) {
+            decode_tile_fine(w, tile, kind, row0, col0, nblk);
+            nrb = kind == 0 ? nblk : TN / 8;                   // 8-row blocks of the I panel that are read
+          } else {
+            decode_tile(w, tile, kind, row0, col0, nblk, nrb);
+          }
           n_valid = min(EB, w.n_E - eb * EB);
           n_kt = w.n_kt;
         }
@@ -405,7 +429,7 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
         if (stop) break;
 
         const CUtensorMap *map = &w.map;
-        const int i_boxes = nrb > TN / 8 ? 2 : 1;              // I panel: one or two boxes of 32 rows
+        const int i_boxes = (nrb + TN / 8 - 1) / (TN / 8);     // I panel: one to four boxes of 32 rows
         const uint32_t tx_bytes = (i_boxes + (kind != 0 ? 1 : 0)) * (w.tr ? TR_BOX_BYTES : BOX_BYTES);
         if (w.use_tma) {
           // TMA box coordinates: (pole, channel) for pole-contiguous W, (channel, pole) for the H.DAT order
@@ -418,9 +442,9 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
               const uint32_t full = full0 + 8 * ps.stage;
               const uint32_t dst = smem_u32(smem + ps.stage * STAGE_BYTES);
               mbar_arrive_expect_tx(full, tx_bytes);
-              tma_load_2d(dst, map, tr ? row0 : k0, tr ? k0 : row0, full);
-              if (i_boxes == 2) tma_load_2d(dst + box, map, tr ? row0 + TN : k0, tr ? k0 : row0 + TN, full);
-              if (kind != 0) tma_load_2d(dst + 2 * box, map, tr ? col0 : k0, tr ? k0 : col0, full);
+              for (int b = 0; b < i_boxes; ++b)
+                tma_load_2d(dst + b * box, map, tr ? row0 + b * TN : k0, tr ? k0 : row0 + b * TN, full);
+              if (kind != 0) tma_load_2d(dst + (TW / TN) * box, map, tr ? col0 : k0, tr ? k0 : col0, full);
             }
             ps.advance();
           }
@@ -430,12 +454,11 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
             mbar_wait(empty0 + 8 * ps.stage, ps.phase ^ 1u);
             double *sd = reinterpret_cast<double *>(smem + ps.stage * STAGE_BYTES);
             if (w.tr) {
-              stage_panel_plain_tr(sd, w, row0, k0, lane);
-              if (i_boxes == 2) stage_panel_plain_tr(sd + KT * TR_PITCH, w, row0 + TN, k0, lane);
-              if (kind != 0) stage_panel_plain_tr(sd + 2 * KT * TR_PITCH, w, col0, k0, lane);
+              for (int b = 0; b < i_boxes; ++b) stage_panel_plain_tr(sd + b * KT * TR_PITCH, w, row0 + b * TN, k0, lane);
+              if (kind != 0) stage_panel_plain_tr(sd + StageLayout<true>::J_BASE, w, col0, k0, lane);
             } else {
               stage_panel_plain(sd, w, row0, i_boxes * TN, k0, lane);
-              if (kind != 0) stage_panel_plain(sd + TM * KT, w, col0, TN, k0, lane);
+              if (kind != 0) stage_panel_plain(sd + StageLayout<false>::J_BASE, w, col0, TN, k0, lane);
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(full0 + 8 * ps.stage);
