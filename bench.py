@@ -54,6 +54,8 @@ def parse_args():
     ap.add_argument("--tail-policy", choices=["auto", "none", "all"], default="auto",
                     help="scheduling knob of the library (pstgf_rmat_set_tail_policy): fine-tile tail sized automatically "
                          "(default), coarse tiles only, fine tiles only; same bits, for measurements")
+    ap.add_argument("--e2e-chunk-mib", type=int, default=0,
+                    help="max_chunk_bytes of pstgf_rmat_form_batch_host in MiB (0 = the library's default)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
@@ -502,13 +504,13 @@ def run_cuda(args):
         d2h = sum(8 * a[4].numel() for a in host)
         e2e_steps = max(1, min(args.steps, 5 if args.config != 6 else 2))
         for _ in range(2):
-            rmat.pstgf_rmat_form_batch_host(host)    # warm-up (allocator pool, pinned pages touched)
+            rmat.pstgf_rmat_form_batch_host(host, max_chunk_bytes=args.e2e_chunk_mib << 20)    # warm-up (allocator pool, pinned pages touched)
         barrier()
         t0 = time.perf_counter()
         e2e_launches, e2e_ms = 0, []
         for _ in range(e2e_steps):
             t1 = time.perf_counter()
-            rmat.pstgf_rmat_form_batch_host(host)    # synchronises before returning
+            rmat.pstgf_rmat_form_batch_host(host, max_chunk_bytes=args.e2e_chunk_mib << 20)    # synchronises before returning
             e2e_ms.append(1e3 * (time.perf_counter() - t1))
             e2e_launches += rmat.pstgf_last_launch_count()
         torch.cuda.synchronize()
