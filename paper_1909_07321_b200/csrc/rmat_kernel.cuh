@@ -1,8 +1,8 @@
 // rmat_kernel.cuh -- the persistent sm_100a kernel behind pstgf_rmat_form / pstgf_rmat_form_batch.
 //
 // One CTA per SM, 12 warps.  Warps 8..11 are the producer warpgroup: they hand most of their
-// registers to the consumers (setmaxnreg).  Warp 8 takes work items (atomic counter in the batch
-// call, round-robin in the single-wave call), publishes them and issues the TMA loads of the W
+// registers to the consumers (setmaxnreg).  Warp 8 takes work items (atomic counter: in the workspace
+// for the batch call, in a pool slot for the single-wave call), publishes them and issues the TMA loads of the W
 // panels; warps 9..11 build the pole scaling d_e[k] = 1/(E_k - E_e) of every
 // stage in shared memory (S1; the denominator of eq. 4).  Warps 0..7 are consumers, one energy of the
 // item's block each: they contract acc[n][m] += W[n][k] * (W[m][k] * d_e[k]) on the FP64 tensor
@@ -27,7 +27,7 @@ struct ItemInfo {        // handed from the load warp to the pole-scaling and co
   short kind;            // 0 DIAG, 1 OFF / WIDE (rectangular, strictly above the diagonal), -1 stop
   unsigned char nrb;     // rectangular tiles: 8-row blocks of the I panel (16 WIDE, 8 OFF, 4 fine OFF32)
   unsigned char tr;      // stage layout: 0 row-major panels, 1 pole-major panels (channel-contiguous W)
-  int nblk;              // DIAG: valid 8x8 block rows/cols; OFF: valid 8-wide column blocks
+  int nblk;              // DIAG: valid 8x8 block rows/cols; rectangular tiles: valid 8-wide column blocks
   int n_kt;
 };
 static_assert(sizeof(ItemInfo) <= 64, "ItemInfo slot");
