@@ -18,7 +18,10 @@
  *
  * Conventions for every call
  *  - Pointers named in "DEVICE" lists are device pointers owned by the caller
- *    (allocate them with any CUDA allocator, e.g. PyTorch).  The library
+ *    (allocate them with any CUDA allocator, e.g. PyTorch).  Any pointer the
+ *    device can dereference works, mapped pinned host memory included (R_out
+ *    there makes every store a PCIe write: about six times slower than device
+ *    memory plus a copy; pstgf_rmat_form_batch_host is the fast host path).  The library
  *    allocates no device memory in the DEVICE-pointer calls (but for the 8 KiB
  *    counter pool of pstgf_rmat_form, once per device); the batch call keeps
  *    its tables in the caller's workspace.

@@ -79,6 +79,19 @@ struct PipeState {
 };
 
 // ---- consumers ---------------------------------------------------------------------------
+// Releasing a stage.  mbarrier.arrive does not wait for the warp's LDS that are still in flight, so an arrive
+// issued right after the stage's last fragment load leaves a window in which the refill (TMA, async proxy)
+// can overwrite rows a delayed LDS has yet to read.  With R_out in device memory the window never opens (an
+// LDS takes tens of cycles, a refill hundreds), but with the LSU backed up for microseconds -- R_out in mapped
+// host memory, every store a PCIe write -- it showed as a few wrong rows per launch.  A CTA-scope fence executed
+// by the whole warp before the release closes it: the warp's loads have been performed when the fence retires
+// (costs 0.5 % on config 5; releasing one stage late instead was measured and is no cheaper).
+__device__ __forceinline__ void release_stage(uint32_t empty0, uint32_t stage, int lane) {
+  __threadfence_block();
+  __syncwarp();
+  if (lane == 0) mbar_arrive(empty0 + 8 * stage);
+}
+
 // Warps whose energy slot lies beyond n_E only keep the ring moving.
 __device__ __forceinline__ void consume_idle(int n_kt, PipeState &ps, uint32_t full0, uint32_t empty0, int lane) {
   for (int kt = 0; kt < n_kt; ++kt) {
@@ -121,8 +134,7 @@ __device__ __forceinline__ void consume_off(const ItemInfo &it, const unsigned c
         for (int bi = 0; bi < NRB; ++bi) dmma884(acc[bi][bj][0], acc[bi][bj][1], a[bi], b);
       }
     }
-    __syncwarp();
-    if (lane == 0) mbar_arrive(empty0 + 8 * ps.stage);
+    release_stage(empty0, ps.stage, lane);
     ps.advance();
   }
   // epilogue: R[r][c] and the mirror R[c][r]; rows are always inside the matrix for OFF tiles
@@ -171,8 +183,7 @@ __device__ __forceinline__ void consume_diag(const ItemInfo &it, const unsigned 
         for (int bi = 0; bi <= bj; ++bi) dmma884(acc[bj * (bj + 1) / 2 + bi][0], acc[bj * (bj + 1) / 2 + bi][1], a[bi], b);
       }
     }
-    __syncwarp();
-    if (lane == 0) mbar_arrive(empty0 + 8 * ps.stage);
+    release_stage(empty0, ps.stage, lane);
     ps.advance();
   }
   const int C = it.n_chan;

@@ -200,6 +200,28 @@ def test_hdat_order_config2_every_energy(rmat, oracle):
     _check(R.cpu().numpy(), oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads()))
 
 
+def test_R_out_in_mapped_host_memory(rmat):
+    """R_out may be any device-accessible pointer.  Pinned host memory makes every store of the epilogue a PCIe
+    write and backs the load/store unit up for microseconds: consumer warps drift far apart and a shared-memory
+    stage released while one of its fragment loads was still in flight got refilled under that load (a few
+    wrong rows per launch before the fence in release_stage).  Same bits as the run into device memory."""
+    from paper_1909_07321_b200 import inputs
+    w = inputs.make_wave(5150, 512, 5120, 96)
+    Wd, Ek, en = _dev(w.W), _dev(w.E_k), _dev(w.energies)
+    R_dev = rmat.pstgf_rmat_form(Wd, Ek, en, w.a)
+    torch.cuda.synchronize()
+    ref = R_dev.cpu()
+    lib = rmat.load()
+    for trial in range(3):
+        R_host = torch.full((w.n_E, w.n_chan, w.n_chan), float("nan"), dtype=torch.float64).pin_memory()
+        st = lib.pstgf_rmat_form(Wd.data_ptr(), Wd.stride(0), Ek.data_ptr(), en.data_ptr(), w.n_chan, w.n_poles, w.n_E,
+                                 w.a, R_host.data_ptr(), torch.cuda.current_stream().cuda_stream)
+        assert st == 0
+        torch.cuda.synchronize()
+        bad = int((R_host != ref).sum())
+        assert bad == 0, f"trial {trial}: {bad} elements differ from the device-memory run"
+
+
 def test_single_wave_call_in_a_cuda_graph(rmat, oracle):
     """Under stream capture the single-wave call must not touch its counter pool (a replayed launch would
     reuse a slot it no longer owns): it falls back to round-robin item assignment.  Captured once, replayed
