@@ -471,6 +471,7 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
               stage_panel_plain(sd, w, row0, i_boxes * TN, k0, lane);
               if (kind != 0) stage_panel_plain(sd + StageLayout<false>::J_BASE, w, col0, TN, k0, lane);
             }
+            __threadfence_block();   // all lanes' stores performed before lane 0 publishes the stage
             __syncwarp();
             if (lane == 0) mbar_arrive(full0 + 8 * ps.stage);
             ps.advance();
@@ -497,6 +498,7 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
       for (;;) {
         mbar_wait(item_full0 + 8 * iq, iphase);
         const ItemInfo it = ring[iq];
+        __threadfence_block();       // the copy above has been read before the slot is handed back
         __syncwarp();
         if (lane == 0) mbar_arrive(item_empty0 + 8 * iq);
         iq ^= 1u;
@@ -534,6 +536,7 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
             if (slot[t] >= 0) dsm[slot[t]] = ok ? 1.0 / (ek[t] - en[t]) : 0.0;
             ek[t] = ek_next[t];
           }
+          __threadfence_block();     // every lane's d has been written before lane 0 arrives
           __syncwarp();
           if (lane == 0) mbar_arrive(full0 + 8 * ps.stage);
           ps.advance();
