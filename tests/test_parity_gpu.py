@@ -220,6 +220,26 @@ def test_R_out_in_mapped_host_memory(rmat):
         torch.cuda.synchronize()
         bad = int((R_host != ref).sum())
         assert bad == 0, f"trial {trial}: {bad} elements differ from the device-memory run"
+    # the same through the batch call: ragged waves, both memory orders of W, every tile kind
+    waves = [inputs.make_wave(5151, 333, 1000, 40), inputs.make_wave(5152, 150, 3000, 51), inputs.make_wave(5153, 64, 2560, 64)]
+    layouts = [rmat.PSTGF_W_CHANNEL_CONTIGUOUS, rmat.PSTGF_W_POLE_CONTIGUOUS, rmat.PSTGF_W_POLE_CONTIGUOUS]
+    dev, mapped = [], []
+    for wv, lay in zip(waves, layouts):
+        Wh = np.ascontiguousarray(wv.W.T) if lay == rmat.PSTGF_W_CHANNEL_CONTIGUOUS else wv.W
+        args = (_dev(Wh), _dev(wv.E_k), _dev(wv.energies), wv.a)
+        dev.append(args + (torch.empty((wv.n_E, wv.n_chan, wv.n_chan), dtype=torch.float64, device="cuda"), lay))
+        mapped.append((args, torch.full((wv.n_E, wv.n_chan, wv.n_chan), float("nan"), dtype=torch.float64).pin_memory(), lay))
+    arr = rmat.make_wave_array(dev)
+    ws = torch.empty(rmat.pstgf_rmat_batch_workspace_bytes(arr), dtype=torch.uint8, device="cuda")
+    rmat.pstgf_rmat_form_batch(arr, ws)
+    arr_h = (rmat.pstgf_wave_t * len(waves))()
+    for p, (d, (_, Rh, lay)) in enumerate(zip(dev, mapped)):
+        arr_h[p] = arr[p]
+        arr_h[p].R_out = Rh.data_ptr()
+    rmat.pstgf_rmat_form_batch(arr_h, ws)
+    torch.cuda.synchronize()
+    for d, (_, Rh, _) in zip(dev, mapped):
+        assert torch.equal(d[4].cpu(), Rh)
 
 
 def test_single_wave_call_in_a_cuda_graph(rmat, oracle):
