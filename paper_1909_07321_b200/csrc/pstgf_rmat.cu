@@ -254,7 +254,11 @@ void plan_tails(std::vector<DevWave> &ds, int grid) {
       budget -= d.n_eb * per_eb;
       continue;
     }
-    const int t = (int)std::min<double>((double)d.n_eb, std::ceil(budget / per_eb));
+    // whole energy blocks, rounded to the nearest: a wave whose single energy block already outweighs the
+    // budget (many tiles, few energies: the paper-scale wave) keeps its coarse tiles -- its items are small
+    // against the whole job, and fine tiles run 5 % slower
+    const int t = (int)std::min<double>((double)d.n_eb, std::floor(budget / per_eb + 0.5));
+    if (t == 0) break;
     d.n_eb_coarse = d.n_eb - t;
     budget -= t * per_eb;
   }
