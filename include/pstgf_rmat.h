@@ -60,7 +60,7 @@
 extern "C" {
 #endif
 
-#define PSTGF_RMAT_VERSION 102 /* major*100 + minor */
+#define PSTGF_RMAT_VERSION 103 /* major*100 + minor */
 
 typedef enum {
   PSTGF_OK = 0,
@@ -184,18 +184,32 @@ pstgf_status_t pstgf_rmat_form_naive(const double *W, long long ldw, const doubl
 /*
  * End-to-end convenience over HOST buffers: `waves` holds HOST pointers
  * (pinned memory recommended; pageable memory works but copies synchronously).
- * Inputs are copied to the device on `stream`, R is formed in chunks of whole
- * energy blocks on two streams of the library's own and copied back into the
- * host R_out on a third while the next chunks are being formed (three staging
- * buffers in flight).  Device memory comes from a stream-ordered pool the
+ * Inputs are copied to the device on `stream`, R is formed on streams of the
+ * library's own in pieces of whole energy blocks and copied back into the host
+ * R_out on another stream while the next pieces are being formed (see
+ * pstgf_rmat_set_host_pipeline; device staging for R is bounded by a third
+ * of the free device memory, at most 16 GiB, per chunk).  Device memory comes from a stream-ordered pool the
  * library owns (one per device, kept for the life of the process so that
  * repeated calls do not re-grow it).  SYNCHRONISES before returning.
- * `max_chunk_bytes` bounds the device R staging per chunk (0 = default: one
- * eighth of all R, clamped to [16 MiB, 256 MiB]); a chunk always holds at
- * least one energy block.
+ * `max_chunk_bytes` bounds a piece (0 = default: 1/32 of all R in [8, 64] MiB
+ * for the signalled pipeline, 1/8 in [16, 256] MiB for the chunked one); a
+ * piece always holds at least one energy block.
  */
 pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves,
                                           size_t max_chunk_bytes, void *stream);
+
+/*
+ * How pstgf_rmat_form_batch_host overlaps formation and copy-back (process-wide knob for tests and
+ * measurements).  PSTGF_HOST_PIPELINE_AUTO (default): one launch per device-sized chunk of R; every piece of at
+ * most max_chunk_bytes has a completion counter the kernel bumps, the arrival that completes a piece raises a
+ * flag in mapped host memory, and the calling thread, which polls the flags, enqueues the piece's copy-back
+ * while the same launch goes on forming the next ones (jobs of under about 2 ms of formation take the CHUNKED
+ * route anyway).  PSTGF_HOST_PIPELINE_CHUNKED: one launch per piece, copy-back ordered by events.  Same bits
+ * either way.
+ */
+#define PSTGF_HOST_PIPELINE_AUTO 0
+#define PSTGF_HOST_PIPELINE_CHUNKED 1
+pstgf_status_t pstgf_rmat_set_host_pipeline(int mode);
 
 /*
  * Measurement utility (not on the hot path): a register-resident FP64

@@ -13,7 +13,9 @@
 #include <tuple>
 #include <mutex>
 #include <numeric>
+#include <thread>
 #include <vector>
+#include <chrono>
 
 #include "../../include/pstgf_rmat.h"
 #include "rmat_kernel.cuh"
@@ -421,8 +423,16 @@ size_t pstgf_rmat_batch_workspace_bytes(const pstgf_wave_t *waves, int n_waves) 
   return n_waves > 0 ? ws_bytes(n_waves) : 0;
 }
 
-pstgf_status_t pstgf_rmat_form_batch(const pstgf_wave_t *waves, int n_waves, void *workspace, size_t workspace_bytes,
-                                     void *stream) {
+// What the host-buffer call needs to know about a batch launch to copy the waves back as they finish.
+struct BatchCompletion {
+  unsigned int *const *done = nullptr;   // in: per input wave, a zeroed device counter or null
+  unsigned int *const *flag = nullptr;   // in: per input wave, a zeroed host-mapped word (device-visible address)
+  std::vector<int> order;                // out: input wave indices in the order the launch completes them
+  std::vector<long long> items;          // out: items of each input wave (arrivals = items * EB)
+};
+
+static pstgf_status_t form_batch_impl(const pstgf_wave_t *waves, int n_waves, void *workspace, size_t workspace_bytes,
+                                      void *stream, BatchCompletion *completion) {
   tl_launches = 0;
   if (n_waves < 0) return PSTGF_ERR_INVALID_VALUE;
   if (n_waves == 0) return PSTGF_OK;
@@ -458,8 +468,25 @@ pstgf_status_t pstgf_rmat_form_batch(const pstgf_wave_t *waves, int n_waves, voi
   std::vector<unsigned char> img(off_waves + (size_t)nw * sizeof(DevWave), 0);
   long long *item_begin = reinterpret_cast<long long *>(img.data() + off_begin);
   std::vector<DevWave> ds((size_t)nw);
-  for (int q = 0; q < nw; ++q) plan_wave(waves[order[q]], ds[q]);
+  for (int q = 0; q < nw; ++q) {
+    plan_wave(waves[order[q]], ds[q]);
+  }
   plan_tails(ds, dstate.sm_count);
+  if (completion && completion->done)
+    for (int q = 0; q < nw; ++q) {
+      ds[q].done = completion->done[order[q]];
+      ds[q].done_flag = completion->flag[order[q]];
+      ds[q].done_target = (unsigned int)(wave_items(ds[q]) * pstgf::EB);   // one arrival per consumer warp and item
+    }
+  if (completion) {
+    // all coarse items come before all fine items: waves with a fine tail finish last
+    completion->items.assign((size_t)n_waves, 0);
+    completion->order.clear();
+    for (int pass = 0; pass < 2; ++pass)
+      for (int q = 0; q < nw; ++q)
+        if ((ds[q].n_eb_coarse < ds[q].n_eb) == (pass == 1)) completion->order.push_back(order[q]);
+    for (int q = 0; q < nw; ++q) completion->items[(size_t)order[q]] = wave_items(ds[q]);
+  }
   long long total = 0;
   for (int q = 0; q < nw; ++q) {
     st = encode_map(ds[q]);
@@ -484,6 +511,11 @@ pstgf_status_t pstgf_rmat_form_batch(const pstgf_wave_t *waves, int n_waves, voi
   PSTGF_CUDA(cudaGetLastError());
   tl_launches = launches + 1;
   return PSTGF_OK;
+}
+
+pstgf_status_t pstgf_rmat_form_batch(const pstgf_wave_t *waves, int n_waves, void *workspace, size_t workspace_bytes,
+                                     void *stream) {
+  return form_batch_impl(waves, n_waves, workspace, workspace_bytes, stream, nullptr);
 }
 
 pstgf_status_t pstgf_rmat_form_naive(const double *W, long long ldw, const double *E_k, const double *energies,
@@ -542,6 +574,40 @@ cudaError_t host_call_pool(int dev, cudaMemPool_t *out) {
   return cudaSuccess;
 }
 
+constexpr size_t MAX_CHUNK_SEGMENTS = 4096;
+std::atomic<int> g_host_pipeline{PSTGF_HOST_PIPELINE_AUTO};
+
+// Completion state of the signalled pipeline, per device and host thread, allocated at the thread's first host
+// call and kept: 2 x MAX_CHUNK_SEGMENTS device counters and as many flag words in mapped pinned host memory.
+struct HostFlags {
+  unsigned int *counters = nullptr;            // device
+  volatile unsigned int *flags_host = nullptr; // host view
+  unsigned int *flags_dev = nullptr;           // device view of the same words
+};
+cudaError_t host_call_flags(int dev, HostFlags *out) {
+  static thread_local HostFlags cache[64];
+  if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+  HostFlags &f = cache[dev];
+  if (!f.counters) {
+    void *c = nullptr, *h = nullptr, *d = nullptr;
+    const size_t bytes = 2 * MAX_CHUNK_SEGMENTS * sizeof(unsigned int);
+    cudaError_t e = cudaMalloc(&c, bytes);
+    if (e != cudaSuccess) return e;
+    e = cudaHostAlloc(&h, bytes, cudaHostAllocMapped);
+    if (e == cudaSuccess) e = cudaHostGetDevicePointer(&d, h, 0);
+    if (e != cudaSuccess) {
+      cudaFree(c);
+      if (h) cudaFreeHost(h);
+      return e;
+    }
+    f.counters = static_cast<unsigned int *>(c);
+    f.flags_host = static_cast<volatile unsigned int *>(h);
+    f.flags_dev = static_cast<unsigned int *>(d);
+  }
+  *out = f;
+  return cudaSuccess;
+}
+
 struct HostCallResources {
   cudaStream_t s = nullptr, copy = nullptr, compute[HOST_COMPUTE_STREAMS] = {nullptr, nullptr};
   cudaEvent_t inputs = nullptr, computed[HOST_RING] = {nullptr}, copied[HOST_RING] = {nullptr};
@@ -578,10 +644,18 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
   DeviceState ds;
   pstgf_status_t st = device_state(ds);
   if (st != PSTGF_OK) return st;
-  // chunk size: about eight chunks per call so that the copy-back of one hides behind the formation of the
-  // next ones, never below 16 MiB (launch and tail overheads) nor above 256 MiB (device footprint)
+  // Pipeline choice: the signalled single launch, unless the knob asks for one launch per piece or the whole
+  // job is a matter of a millisecond or two (then the naps of the flag polling cost more than launches do).
+  double est_flop = 0.0;
+  for (int p = 0; p < n_waves; ++p)
+    if (wave_has_items(waves[p])) est_flop += (double)waves[p].n_E * waves[p].n_chan * (double)waves[p].n_chan * waves[p].n_poles;
+  const bool signalled = g_host_pipeline.load() == PSTGF_HOST_PIPELINE_AUTO && est_flop / 33e12 >= 2e-3;
+  // copy-back granularity (a piece): 1/32 of R in [8, 64] MiB when pieces are free (signalled), 1/8 of R in
+  // [16, 256] MiB when each piece is a launch
   size_t cap = max_chunk_bytes;
-  if (!cap) cap = std::min<size_t>((size_t)256 << 20, std::max<size_t>((size_t)16 << 20, total_r / 8));
+  if (!cap)
+    cap = signalled ? std::min<size_t>((size_t)64 << 20, std::max<size_t>((size_t)8 << 20, total_r / 32))
+                    : std::min<size_t>((size_t)256 << 20, std::max<size_t>((size_t)16 << 20, total_r / 8));
   HostCallResources res;
   res.s = static_cast<cudaStream_t>(stream);
   cudaMemPool_t pool;
@@ -622,7 +696,30 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
     dev[p].E_k = static_cast<double *>(dEk);
     dev[p].energies = static_cast<double *>(dEn);
   }
-  // chunks of (wave, energy range) segments, each at most `cap` bytes of R (at least one energy block)
+  // Two ways to overlap the copy-back with the formation (pstgf_rmat_set_host_pipeline):
+  //  signalled  ONE launch forms a whole chunk (as much of R as the device budget allows); its segments (a wave's
+  //             energy range of at most `cap` bytes) are the waves of that launch, each with a completion
+  //             counter; the warp whose arrival completes a segment raises a flag in mapped host memory, and
+  //             this thread, which polls the flags in completion order, enqueues the segment's copy-back at
+  //             once.  No launch boundaries, no per-chunk tails.  (Stream wait-value on the counters was tried
+  //             first: its polling made the copy stream erratic, 7-20 ms against 3 ms on config 2.)
+  //  chunked    one launch per chunk of at most `cap` bytes, copy-back ordered by events.
+  size_t chunk_cap = cap;
+  if (signalled) {
+    // device budget of a chunk: a quarter of the device's memory, at most 16 GiB (two chunks may be in flight);
+    // queried once per device -- cudaMemGetInfo on every call showed up as occasional stalls of tens of ms
+    static std::atomic<size_t> budget[64];
+    size_t bud = ds.device < 64 ? budget[ds.device].load() : 0;
+    if (!bud) {
+      size_t free_b = 0, total_b = 0;
+      PSTGF_CUDA(cudaMemGetInfo(&free_b, &total_b));
+      bud = std::min<size_t>((size_t)16 << 30, total_b / 4);
+      if (ds.device < 64) budget[ds.device].store(bud);
+    }
+    chunk_cap = std::max<size_t>(cap, bud);
+  }
+  // chunks of (wave, energy range) segments: a segment holds at most `cap` bytes of R (at least one energy
+  // block), a chunk at most `chunk_cap` bytes and MAX_CHUNK_SEGMENTS segments
   std::vector<std::vector<Segment>> chunks;
   size_t max_chunk = 0, cur = 0;
   size_t max_segs = 1;
@@ -633,10 +730,12 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
     const size_t per_e = sizeof(double) * (size_t)w.n_chan * w.n_chan;
     int e0 = 0;
     while (e0 < w.n_E) {
-      size_t room = cap > cur ? cap - cur : 0;
+      size_t room = chunk_cap > cur ? chunk_cap - cur : 0;
+      if (signalled) room = std::min(room, cap);
       int ne = (int)std::min<size_t>((size_t)(w.n_E - e0), room / per_e);
       if (ne < w.n_E - e0) ne -= ne % pstgf::EB;      // split only at energy-block boundaries
-      if (ne <= 0) {
+      if (signalled && ne <= 0 && chunk_cap > cur && chunk_cap - cur >= per_e * (size_t)pstgf::EB) ne = std::min(pstgf::EB, w.n_E - e0);
+      if (ne <= 0 || chunks.back().size() >= MAX_CHUNK_SEGMENTS) {
         if (cur > 0) {                               // close the chunk and retry in an empty one
           chunks.emplace_back();
           cur = 0;
@@ -653,41 +752,79 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
   }
   if (chunks.back().empty()) chunks.pop_back();
   if (chunks.empty()) return PSTGF_OK;
-  const int ring = (int)std::min<size_t>(HOST_RING, chunks.size());
+  const int ring = (int)std::min<size_t>(signalled ? 2 : HOST_RING, chunks.size());
   void *rbuf[HOST_RING], *wsbuf[HOST_RING];
   const size_t wsb = ws_bytes((int)max_segs);
   for (int b = 0; b < ring; ++b) {
     PSTGF_CUDA(dev_alloc(max_chunk, &rbuf[b]));
     PSTGF_CUDA(dev_alloc(wsb, &wsbuf[b]));
   }
+  HostFlags flags;
+  if (signalled) PSTGF_CUDA(host_call_flags(ds.device, &flags));
   // the formation kernels run on two streams of the library's own, so that the first CTAs of chunk c+1 start on
   // the SMs the tail of chunk c has left; both wait for the inputs (and the allocations) enqueued on `stream`
   PSTGF_CUDA(cudaEventRecord(res.inputs, res.s));
   for (cudaStream_t c : res.compute) PSTGF_CUDA(cudaStreamWaitEvent(c, res.inputs, 0));
   int launches = 0;
   std::vector<pstgf_wave_t> sub;
+  std::vector<unsigned int *> done, flag;
+  BatchCompletion completion;
   for (size_t c = 0; c < chunks.size(); ++c) {
     const int b = (int)(c % ring);
     cudaStream_t cs = res.compute[c % HOST_COMPUTE_STREAMS];
     if (c >= (size_t)ring) PSTGF_CUDA(cudaStreamWaitEvent(cs, res.copied[b], 0));
     sub.clear();
+    done.clear();
+    flag.clear();
+    const size_t f0 = (size_t)b * MAX_CHUNK_SEGMENTS;
     for (const Segment &g : chunks[c]) {
       pstgf_wave_t w = dev[g.wave];
       w.energies = dev[g.wave].energies + g.e0;
       w.n_E = g.ne;
       w.R_out = reinterpret_cast<double *>(static_cast<unsigned char *>(rbuf[b]) + g.off);
       sub.push_back(w);
+      if (signalled) {
+        done.push_back(flags.counters + f0 + (sub.size() - 1));
+        flag.push_back(flags.flags_dev + f0 + (sub.size() - 1));
+      }
     }
-    st = pstgf_rmat_form_batch(sub.data(), (int)sub.size(), wsbuf[b], wsb, cs);
-    if (st != PSTGF_OK) return st;
-    launches += tl_launches;
-    PSTGF_CUDA(cudaEventRecord(res.computed[b], cs));
-    PSTGF_CUDA(cudaStreamWaitEvent(res.copy, res.computed[b], 0));
-    for (const Segment &g : chunks[c]) {
+    auto copy_back = [&](const Segment &g) -> cudaError_t {
       const pstgf_wave_t &w = waves[g.wave];
       const size_t per_e = sizeof(double) * (size_t)w.n_chan * w.n_chan;
-      PSTGF_CUDA(cudaMemcpyAsync(w.R_out + (size_t)g.e0 * w.n_chan * w.n_chan, static_cast<unsigned char *>(rbuf[b]) + g.off,
-                                 per_e * (size_t)g.ne, cudaMemcpyDeviceToHost, res.copy));
+      return cudaMemcpyAsync(w.R_out + (size_t)g.e0 * w.n_chan * w.n_chan, static_cast<unsigned char *>(rbuf[b]) + g.off,
+                             per_e * (size_t)g.ne, cudaMemcpyDeviceToHost, res.copy);
+    };
+    if (signalled) {
+      if (c >= (size_t)ring) PSTGF_CUDA(cudaEventSynchronize(res.copied[b]));   // this slot's flags are being reused
+      for (size_t q = 0; q < sub.size(); ++q) flags.flags_host[f0 + q] = 0u;
+      PSTGF_CUDA(cudaMemsetAsync(flags.counters + f0, 0, sizeof(unsigned int) * sub.size(), cs));
+      completion.done = done.data();
+      completion.flag = flag.data();
+      st = form_batch_impl(sub.data(), (int)sub.size(), wsbuf[b], wsb, cs, &completion);
+      if (st != PSTGF_OK) return st;
+      launches += tl_launches;
+      // poll the flags in completion order: a short spin, then naps of 20 us (a thread that spins for the whole
+      // launch can run into the CPU quota of a container and be parked for tens of milliseconds)
+      for (int q : completion.order) {
+        unsigned long long polls = 0;
+        while (flags.flags_host[f0 + (size_t)q] == 0u) {
+          if (++polls < 2000) continue;
+          std::this_thread::sleep_for(std::chrono::microseconds(20));
+          if ((polls & 0x3ffULL) == 0) {                // every ~1000 naps: has the launch died?
+            const cudaError_t e = cudaStreamQuery(cs);
+            if (e != cudaSuccess && e != cudaErrorNotReady) return cuda_fail(e);
+            if (e == cudaSuccess && flags.flags_host[f0 + (size_t)q] == 0u) return cuda_fail(cudaErrorUnknown);
+          }
+        }
+        PSTGF_CUDA(copy_back(chunks[c][(size_t)q]));
+      }
+    } else {
+      st = pstgf_rmat_form_batch(sub.data(), (int)sub.size(), wsbuf[b], wsb, cs);
+      if (st != PSTGF_OK) return st;
+      launches += tl_launches;
+      PSTGF_CUDA(cudaEventRecord(res.computed[b], cs));
+      PSTGF_CUDA(cudaStreamWaitEvent(res.copy, res.computed[b], 0));
+      for (const Segment &g : chunks[c]) PSTGF_CUDA(copy_back(g));
     }
     PSTGF_CUDA(cudaEventRecord(res.copied[b], res.copy));
   }
@@ -695,6 +832,12 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
   for (cudaStream_t c : res.compute) PSTGF_CUDA(cudaStreamSynchronize(c));
   PSTGF_CUDA(cudaStreamSynchronize(res.s));
   tl_launches = launches;
+  return PSTGF_OK;
+}
+
+pstgf_status_t pstgf_rmat_set_host_pipeline(int mode) {
+  if (mode != PSTGF_HOST_PIPELINE_AUTO && mode != PSTGF_HOST_PIPELINE_CHUNKED) return PSTGF_ERR_INVALID_VALUE;
+  g_host_pipeline.store(mode);
   return PSTGF_OK;
 }
 

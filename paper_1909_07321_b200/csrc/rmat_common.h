@@ -65,7 +65,7 @@ struct StageLayout {
 };
 constexpr int SMEM_BARRIER_OFFSET = STAGES * STAGE_BYTES;
 constexpr int SMEM_ITEM_OFFSET = SMEM_BARRIER_OFFSET + (2 * STAGES + 4) * 8;
-constexpr int SMEM_BYTES = SMEM_ITEM_OFFSET + 2 * 64 + 128;  // + alignment slack
+constexpr int SMEM_BYTES = SMEM_ITEM_OFFSET + 2 * 96 + 128;  // two ItemInfo slots + alignment slack
 
 // One partial wave as the kernel sees it.  Built on the host, lives in kernel parameter
 // space (single-wave call) or in the caller's workspace (batch call).
@@ -75,6 +75,8 @@ struct alignas(128) DevWave {
   const double *E_k;
   const double *energies;
   double *R_out;
+  unsigned int *done;      // optional completion counter of this wave (host-buffer call): += 1 per consumer warp and item
+  unsigned int *done_flag; // ... and the (host-mapped) word that is set to 1 by the arrival that makes it done_target
   long long ldw;
   double inv2a;            // 1/(2a), PAPER.md:108 prefactor
   int n_chan, n_poles, n_E;
@@ -85,6 +87,7 @@ struct alignas(128) DevWave {
   int n_tiles;             // coarse tiles: n_i DIAG + WIDE + OFF
   int use_tma;             // W 16-byte aligned and ldw even
   int n_eb_coarse;         // energy blocks [0, n_eb_coarse) use coarse tiles, [n_eb_coarse, n_eb) fine tiles
+  unsigned int done_target;
   int tr;                  // 1: W is channel-contiguous [n_poles][ldw] (H.DAT record order), map box [KT][TR_PITCH]
 };
 static_assert(sizeof(DevWave) == 256, "DevWave layout");

@@ -15,8 +15,11 @@
 
 namespace pstgf {
 
-struct ItemInfo {        // handed from the load warp to the pole-scaling and consumer warps through smem
+struct alignas(16) ItemInfo {   // handed from the load warp to the pole-scaling and consumer warps through smem
   double *R;             // R_out of the block's first energy
+  unsigned int *done;    // completion counter of the item's wave, or null
+  unsigned int *done_flag;   // host-mapped word set to 1 when the counter reaches done_target
+  unsigned int done_target;
   const double *E_k;     // the wave's poles
   const double *energies;// the block's first energy
   double inv2a;
@@ -30,7 +33,7 @@ struct ItemInfo {        // handed from the load warp to the pole-scaling and co
   int nblk;              // DIAG: valid 8x8 block rows/cols; rectangular tiles: valid 8-wide column blocks
   int n_kt;
 };
-static_assert(sizeof(ItemInfo) <= 64, "ItemInfo slot");
+static_assert(sizeof(ItemInfo) == 96, "ItemInfo slot (SMEM_BYTES reserves 2 x 96)");
 
 // ---- PTX wrappers ------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p) {
@@ -343,7 +346,7 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
   const uint32_t bar0 = smem_u32(smem + SMEM_BARRIER_OFFSET);
   const uint32_t full0 = bar0, empty0 = bar0 + 8 * STAGES;
   const uint32_t item_full0 = bar0 + 16 * STAGES, item_empty0 = item_full0 + 16;
-  ItemInfo *ring = reinterpret_cast<ItemInfo *>(smem + SMEM_ITEM_OFFSET);   // 2 slots of 64 B
+  ItemInfo *ring = reinterpret_cast<ItemInfo *>(smem + SMEM_ITEM_OFFSET);   // 2 slots of 96 B
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (threadIdx.x == 0) {
@@ -420,6 +423,9 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
           ii.kind = (short)kind;
           if (!stop) {
             ii.R = w.R_out + (size_t)eb * EB * w.n_chan * w.n_chan;
+            ii.done = w.done;
+            ii.done_flag = w.done_flag;
+            ii.done_target = w.done_target;
             ii.E_k = w.E_k;
             ii.energies = w.energies + (size_t)eb * EB;
             ii.inv2a = w.inv2a;
@@ -554,6 +560,17 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
       if (it.kind < 0) break;
       if (warp >= it.n_valid_e) consume_idle(it.n_kt, ps, full0, empty0, lane);
       else consume_item(it, smem, ps, full0, empty0, warp, lane);
+      if (it.done != nullptr) {
+        // host-buffer call: the host copies a wave's R back as soon as its last item has been stored.  Every warp
+        // makes its stores visible device-wide and counts itself in; the arrival that completes the wave raises
+        // the wave's flag in host-mapped memory, which the calling thread polls.
+        __threadfence();
+        __syncwarp();
+        if (lane == 0 && atomicAdd(it.done, 1u) + 1u == it.done_target) {
+          __threadfence_system();
+          *reinterpret_cast<volatile unsigned int *>(it.done_flag) = 1u;
+        }
+      }
       __syncwarp();
       if (lane == 0) mbar_arrive(item_empty0 + 8 * iq);
       iq ^= 1u;

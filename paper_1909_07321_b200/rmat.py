@@ -16,11 +16,12 @@ from . import build as _build
 PSTGF_OK = 0
 PSTGF_TAIL_AUTO, PSTGF_TAIL_NONE, PSTGF_TAIL_ALL = 0, 1, 2
 PSTGF_W_POLE_CONTIGUOUS, PSTGF_W_CHANNEL_CONTIGUOUS = 0, 1
+PSTGF_HOST_PIPELINE_AUTO, PSTGF_HOST_PIPELINE_CHUNKED = 0, 1
 _STATUS_NAMES = {0: "PSTGF_OK", 1: "PSTGF_ERR_INVALID_VALUE", 2: "PSTGF_ERR_ALIGNMENT", 3: "PSTGF_ERR_WORKSPACE",
                  4: "PSTGF_ERR_UNSUPPORTED_DEVICE", 5: "PSTGF_ERR_CUDA"}
 
 EXPORTS = ["pstgf_rmat_form", "pstgf_rmat_form_hdat", "pstgf_rmat_batch_workspace_bytes", "pstgf_rmat_form_batch", "pstgf_rmat_form_naive",
-           "pstgf_rmat_form_batch_host", "pstgf_rmat_set_tail_policy", "pstgf_fp64_probe", "pstgf_last_launch_count", "pstgf_status_string", "pstgf_last_cuda_error",
+           "pstgf_rmat_form_batch_host", "pstgf_rmat_set_tail_policy", "pstgf_rmat_set_host_pipeline", "pstgf_fp64_probe", "pstgf_last_launch_count", "pstgf_status_string", "pstgf_last_cuda_error",
            "pstgf_version"]
 
 
@@ -72,6 +73,8 @@ def load(build_if_missing: bool = False):
     lib.pstgf_rmat_form_batch_host.restype = i
     lib.pstgf_rmat_set_tail_policy.argtypes = [i]
     lib.pstgf_rmat_set_tail_policy.restype = i
+    lib.pstgf_rmat_set_host_pipeline.argtypes = [i]
+    lib.pstgf_rmat_set_host_pipeline.restype = i
     lib.pstgf_fp64_probe.argtypes = [i, i, i, i, vp, ctypes.POINTER(d), vp]
     lib.pstgf_fp64_probe.restype = i
     lib.pstgf_last_launch_count.restype = i
@@ -214,6 +217,11 @@ def pstgf_rmat_form_batch_host(host_waves: Sequence[tuple], max_chunk_bytes: int
 def pstgf_rmat_set_tail_policy(policy: int) -> None:
     """Scheduling knob: PSTGF_TAIL_AUTO / PSTGF_TAIL_NONE / PSTGF_TAIL_ALL (results are bitwise the same)."""
     _check(load().pstgf_rmat_set_tail_policy(int(policy)))
+
+
+def pstgf_rmat_set_host_pipeline(mode: int) -> None:
+    """PSTGF_HOST_PIPELINE_AUTO (signalled single launch) or PSTGF_HOST_PIPELINE_CHUNKED (one launch per piece)."""
+    _check(load().pstgf_rmat_set_host_pipeline(int(mode)))
 
 
 def pstgf_fp64_probe(kind: int, iters: int, blocks: int, threads: int, sink: torch.Tensor, stream=None) -> float:
