@@ -286,6 +286,43 @@ def test_host_call_signalled_pipeline(rmat, oracle):
     _check(R.numpy()[pick], oracle.rmat_form(w.W, w.E_k, w.energies[pick], w.a, threads=_threads()))
 
 
+def test_random_shapes_layouts_policies(rmat, tail_policy):
+    """Seeded fuzz: random batches of 1-4 waves with random shapes (n_chan 1..700), leading dimensions, memory
+    orders of W and scheduling policies, single-wave or batch call, every energy against the term-by-term device
+    kernel (itself checked against the oracle above).  The bound is 1e-12 rather than 1e-13 because a wave with
+    one or two channels has no large diagonal to normalise by: cancellation in a single sum shows directly."""
+    from paper_1909_07321_b200 import inputs
+    rng = np.random.default_rng(20260101)
+    for case in range(40):
+        waves, dev = [], []
+        for _ in range(int(rng.integers(1, 5))):
+            C = int(rng.choice([rng.integers(1, 40), rng.integers(40, 200), rng.integers(200, 700)]))
+            K = int(rng.choice([rng.integers(1, 30), rng.integers(30, 300), rng.integers(300, 900)]))
+            N = int(rng.choice([rng.integers(1, 9), rng.integers(9, 70), rng.integers(70, 300)])) if C < 300 else int(rng.integers(1, 40))
+            w = inputs.make_wave(int(rng.integers(1 << 30)), C, K, N)
+            lay = int(rng.integers(0, 2))
+            Wh = np.ascontiguousarray(w.W.T) if lay else w.W
+            buf = torch.zeros((Wh.shape[0], Wh.shape[1] + int(rng.integers(0, 4))), dtype=torch.float64, device="cuda")
+            buf[:, :Wh.shape[1]].copy_(torch.from_numpy(Wh))
+            R = torch.full((N, C, C), float("nan"), dtype=torch.float64, device="cuda")
+            waves.append(w)
+            dev.append((buf[:, :Wh.shape[1]], _dev(w.E_k), _dev(w.energies), w.a, R, lay))
+        tail_policy(int(rng.integers(0, 3)))
+        if len(dev) == 1 and rng.integers(0, 2):
+            d = dev[0]
+            (rmat.pstgf_rmat_form_hdat if d[5] else rmat.pstgf_rmat_form)(d[0], d[1], d[2], d[3], R_out=d[4])
+        else:
+            arr = rmat.make_wave_array(dev)
+            ws = torch.empty(rmat.pstgf_rmat_batch_workspace_bytes(arr), dtype=torch.uint8, device="cuda")
+            rmat.pstgf_rmat_form_batch(arr, ws)
+        torch.cuda.synchronize()
+        for w, d in zip(waves, dev):
+            R, Rn = d[4], rmat.pstgf_rmat_form_naive(d[0], d[1], d[2], d[3], layout=d[5])
+            assert bool(torch.isfinite(R).all()) and torch.equal(R, R.transpose(1, 2)), (case, w.n_chan, w.n_poles, w.n_E)
+            err = (R - Rn).abs().flatten(1).max(dim=1).values / Rn.abs().flatten(1).max(dim=1).values.clamp_min(1e-300)
+            assert float(err.max()) <= 1e-12, (case, float(err.max()), w.n_chan, w.n_poles, w.n_E, d[5])
+
+
 def test_many_launches_in_flight(rmat, oracle):
     """More single-wave launches in flight than the counter pool has slots (64), on several streams: every
     launch must still do all of its items exactly once (pool slot or round-robin fallback)."""
