@@ -427,6 +427,7 @@ size_t pstgf_rmat_batch_workspace_bytes(const pstgf_wave_t *waves, int n_waves) 
 struct BatchCompletion {
   unsigned int *const *done = nullptr;   // in: per input wave, a zeroed device counter or null
   unsigned int *const *flag = nullptr;   // in: per input wave, a zeroed host-mapped word (device-visible address)
+  const unsigned int *const *rows_ready = nullptr;   // in, optional: per input wave, the upload counter of its W
   std::vector<int> order;                // out: input wave indices in the order the launch completes them
   std::vector<long long> items;          // out: items of each input wave (arrivals = items * EB)
 };
@@ -477,6 +478,7 @@ static pstgf_status_t form_batch_impl(const pstgf_wave_t *waves, int n_waves, vo
       ds[q].done = completion->done[order[q]];
       ds[q].done_flag = completion->flag[order[q]];
       ds[q].done_target = (unsigned int)(wave_items(ds[q]) * pstgf::EB);   // one arrival per consumer warp and item
+      if (completion->rows_ready) ds[q].rows_ready = completion->rows_ready[order[q]];
     }
   if (completion) {
     // all coarse items come before all fine items: waves with a fine tail finish last
@@ -579,10 +581,13 @@ std::atomic<int> g_host_pipeline{PSTGF_HOST_PIPELINE_AUTO};
 
 // Completion state of the signalled pipeline, per device and host thread, allocated at the thread's first host
 // call and kept: 2 x MAX_CHUNK_SEGMENTS device counters and as many flag words in mapped pinned host memory.
+constexpr size_t MAX_UPLOAD_WAVES = 1024, MAX_UPLOAD_SLABS = 16;
 struct HostFlags {
   unsigned int *counters = nullptr;            // device
   volatile unsigned int *flags_host = nullptr; // host view
   unsigned int *flags_dev = nullptr;           // device view of the same words
+  unsigned int *upload_counters = nullptr;     // device: rows of each wave's W uploaded so far
+  unsigned int *upload_values = nullptr;       // pinned host: the values the upload stream copies into them
 };
 cudaError_t host_call_flags(int dev, HostFlags *out) {
   static thread_local HostFlags cache[64];
@@ -600,9 +605,20 @@ cudaError_t host_call_flags(int dev, HostFlags *out) {
       if (h) cudaFreeHost(h);
       return e;
     }
+    void *uc = nullptr, *uv = nullptr;
+    e = cudaMalloc(&uc, MAX_UPLOAD_WAVES * sizeof(unsigned int));
+    if (e == cudaSuccess) e = cudaHostAlloc(&uv, MAX_UPLOAD_WAVES * (MAX_UPLOAD_SLABS + 1) * sizeof(unsigned int), cudaHostAllocDefault);
+    if (e != cudaSuccess) {
+      cudaFree(c);
+      cudaFreeHost(h);
+      if (uc) cudaFree(uc);
+      return e;
+    }
     f.counters = static_cast<unsigned int *>(c);
     f.flags_host = static_cast<volatile unsigned int *>(h);
     f.flags_dev = static_cast<unsigned int *>(d);
+    f.upload_counters = static_cast<unsigned int *>(uc);
+    f.upload_values = static_cast<unsigned int *>(uv);
   }
   *out = f;
   return cudaSuccess;
@@ -672,8 +688,20 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
     if (e == cudaSuccess) res.allocs.push_back(*out);
     return e;
   };
-  // inputs: W re-pitched to an even leading dimension so that the TMA staging path applies
+  // inputs, first part: allocations and the small arrays (poles, energies).  W follows further down: in the
+  // signalled pipeline it is uploaded in slabs of rows WHILE the launch runs, each slab followed by an update of
+  // the wave's upload counter that the kernel's load warp waits on (the launch starts on the first rows).
+  HostFlags flags;
+  if (signalled) PSTGF_CUDA(host_call_flags(ds.device, &flags));
+  const bool overlap_upload = signalled && (size_t)n_waves <= MAX_UPLOAD_WAVES;
+  if (overlap_upload) PSTGF_CUDA(cudaMemsetAsync(flags.upload_counters, 0, sizeof(unsigned int) * (size_t)n_waves, res.s));
   std::vector<pstgf_wave_t> dev(waves, waves + n_waves);
+  auto upload_W = [&](int p, long long r0, long long r1) -> cudaError_t {   // rows [r0, r1) of the W array of wave p
+    const pstgf_wave_t &w = waves[p];
+    const long long w_cols = w.w_layout == PSTGF_W_CHANNEL_CONTIGUOUS ? w.n_chan : w.n_poles;
+    return cudaMemcpy2DAsync(const_cast<double *>(dev[p].W) + r0 * dev[p].ldw, (size_t)dev[p].ldw * 8, w.W + r0 * w.ldw,
+                             (size_t)w.ldw * 8, (size_t)w_cols * 8, (size_t)(r1 - r0), cudaMemcpyHostToDevice, res.s);
+  };
   for (int p = 0; p < n_waves; ++p) {
     const pstgf_wave_t &w = waves[p];
     if (w.n_chan == 0 || w.n_E == 0) continue;
@@ -683,18 +711,18 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
     }
     const bool tr = w.w_layout == PSTGF_W_CHANNEL_CONTIGUOUS;
     const long long w_rows = tr ? w.n_poles : w.n_chan, w_cols = tr ? w.n_chan : w.n_poles;
-    const long long pitch = (w_cols + 1) & ~1LL;
+    const long long pitch = (w_cols + 1) & ~1LL;     // even leading dimension: the TMA staging path applies
     void *dW, *dEk, *dEn;
     PSTGF_CUDA(dev_alloc(sizeof(double) * (size_t)pitch * w_rows, &dW));
     PSTGF_CUDA(dev_alloc(sizeof(double) * (size_t)w.n_poles, &dEk));
     PSTGF_CUDA(dev_alloc(sizeof(double) * (size_t)w.n_E, &dEn));
-    PSTGF_CUDA(cudaMemcpy2DAsync(dW, pitch * 8, w.W, w.ldw * 8, (size_t)w_cols * 8, (size_t)w_rows, cudaMemcpyHostToDevice, res.s));
     PSTGF_CUDA(cudaMemcpyAsync(dEk, w.E_k, sizeof(double) * (size_t)w.n_poles, cudaMemcpyHostToDevice, res.s));
     PSTGF_CUDA(cudaMemcpyAsync(dEn, w.energies, sizeof(double) * (size_t)w.n_E, cudaMemcpyHostToDevice, res.s));
     dev[p].W = static_cast<double *>(dW);
     dev[p].ldw = pitch;
     dev[p].E_k = static_cast<double *>(dEk);
     dev[p].energies = static_cast<double *>(dEn);
+    if (!overlap_upload) PSTGF_CUDA(upload_W(p, 0, w_rows));
   }
   // Two ways to overlap the copy-back with the formation (pstgf_rmat_set_host_pipeline):
   //  signalled  ONE launch forms a whole chunk (as much of R as the device budget allows); its segments (a wave's
@@ -759,15 +787,32 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
     PSTGF_CUDA(dev_alloc(max_chunk, &rbuf[b]));
     PSTGF_CUDA(dev_alloc(wsb, &wsbuf[b]));
   }
-  HostFlags flags;
-  if (signalled) PSTGF_CUDA(host_call_flags(ds.device, &flags));
   // the formation kernels run on two streams of the library's own, so that the first CTAs of chunk c+1 start on
   // the SMs the tail of chunk c has left; both wait for the inputs (and the allocations) enqueued on `stream`
   PSTGF_CUDA(cudaEventRecord(res.inputs, res.s));
   for (cudaStream_t c : res.compute) PSTGF_CUDA(cudaStreamWaitEvent(c, res.inputs, 0));
+  // inputs, second part: W in slabs of rows on `stream`, behind the event the launches wait for, so that the
+  // formation starts on the first slab while the others are still on their way
+  if (overlap_upload) {
+    for (int p = 0; p < n_waves; ++p) {
+      const pstgf_wave_t &w = waves[p];
+      if (!wave_has_items(w)) continue;
+      const long long w_rows = w.w_layout == PSTGF_W_CHANNEL_CONTIGUOUS ? w.n_poles : w.n_chan;
+      const size_t bytes = sizeof(double) * (size_t)dev[p].ldw * (size_t)w_rows;
+      const long long n_slabs = std::max<long long>(1, std::min<long long>({(long long)MAX_UPLOAD_SLABS, w_rows, (long long)(bytes >> 22)}));
+      unsigned int *vals = flags.upload_values + (size_t)p * (MAX_UPLOAD_SLABS + 1);
+      for (long long sl = 0; sl < n_slabs; ++sl) {
+        const long long r0 = w_rows * sl / n_slabs, r1 = w_rows * (sl + 1) / n_slabs;
+        PSTGF_CUDA(upload_W(p, r0, r1));
+        vals[sl] = (unsigned int)r1;
+        PSTGF_CUDA(cudaMemcpyAsync(flags.upload_counters + p, vals + sl, sizeof(unsigned int), cudaMemcpyHostToDevice, res.s));
+      }
+    }
+  }
   int launches = 0;
   std::vector<pstgf_wave_t> sub;
   std::vector<unsigned int *> done, flag;
+  std::vector<const unsigned int *> rows_ready;
   BatchCompletion completion;
   for (size_t c = 0; c < chunks.size(); ++c) {
     const int b = (int)(c % ring);
@@ -776,6 +821,7 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
     sub.clear();
     done.clear();
     flag.clear();
+    rows_ready.clear();
     const size_t f0 = (size_t)b * MAX_CHUNK_SEGMENTS;
     for (const Segment &g : chunks[c]) {
       pstgf_wave_t w = dev[g.wave];
@@ -786,6 +832,7 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
       if (signalled) {
         done.push_back(flags.counters + f0 + (sub.size() - 1));
         flag.push_back(flags.flags_dev + f0 + (sub.size() - 1));
+        rows_ready.push_back(overlap_upload ? flags.upload_counters + g.wave : nullptr);
       }
     }
     auto copy_back = [&](const Segment &g) -> cudaError_t {
@@ -800,6 +847,7 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
       PSTGF_CUDA(cudaMemsetAsync(flags.counters + f0, 0, sizeof(unsigned int) * sub.size(), cs));
       completion.done = done.data();
       completion.flag = flag.data();
+      completion.rows_ready = rows_ready.data();
       st = form_batch_impl(sub.data(), (int)sub.size(), wsbuf[b], wsb, cs, &completion);
       if (st != PSTGF_OK) return st;
       launches += tl_launches;

@@ -77,6 +77,7 @@ struct alignas(128) DevWave {
   double *R_out;
   unsigned int *done;      // optional completion counter of this wave (host-buffer call): += 1 per consumer warp and item
   unsigned int *done_flag; // ... and the (host-mapped) word that is set to 1 by the arrival that makes it done_target
+  const unsigned int *rows_ready;   // optional (host-buffer call): rows of the W array uploaded so far, see the load warp
   long long ldw;
   double inv2a;            // 1/(2a), PAPER.md:108 prefactor
   int n_chan, n_poles, n_E;

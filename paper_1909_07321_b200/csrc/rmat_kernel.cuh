@@ -74,6 +74,25 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
                : "d"(a), "d"(b));
 }
 
+// Host-buffer call: W may still be on its way up while the launch runs.  The upload stream bumps a counter
+// after every slab of rows (channels of a pole-contiguous W, poles of a channel-contiguous one); the load warp
+// waits here until the rows its next TMA boxes cover have landed.
+__device__ __forceinline__ void wait_rows_uploaded(const unsigned int *rows_ready, unsigned int need, unsigned int &seen,
+                                                   int lane) {
+  if (seen >= need) return;
+  if (lane == 0) {
+    unsigned int v;
+    for (;;) {
+      asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(rows_ready) : "memory");
+      if (v >= need) break;
+      __nanosleep(500);
+    }
+    seen = v;
+    asm volatile("fence.proxy.async;" ::: "memory");   // the loads that follow go through the async proxy (TMA)
+  }
+  seen = __shfl_sync(0xffffffffu, seen, 0);
+}
+
 struct PipeState {
   uint32_t stage = 0, phase = 0;
   __device__ __forceinline__ void advance() {
@@ -448,12 +467,21 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
         const CUtensorMap *map = &w.map;
         const int i_boxes = (nrb + TN / 8 - 1) / (TN / 8);     // I panel: one to four boxes of 32 rows
         const uint32_t tx_bytes = (i_boxes + (kind != 0 ? 1 : 0)) * (w.tr ? TR_BOX_BYTES : BOX_BYTES);
+        // rows of W this item reads (pole-contiguous W: channels; the poles of a channel-contiguous W are waited
+        // for stage by stage below)
+        const unsigned int *rows_ready = w.rows_ready;
+        unsigned int rows_seen = rows_ready ? 0u : 0xffffffffu;
+        if (rows_ready && !w.tr) {
+          const int last = kind == 0 ? row0 + nrb * 8 : max(row0 + nrb * 8, col0 + nblk * 8);
+          wait_rows_uploaded(rows_ready, (unsigned int)min(last, w.n_chan), rows_seen, lane);
+        }
         if (w.use_tma) {
           // TMA box coordinates: (pole, channel) for pole-contiguous W, (channel, pole) for the H.DAT order
           const int tr = w.tr;
           const uint32_t box = tr ? TR_BOX_BYTES : BOX_BYTES;
           for (int kt = 0; kt < n_kt; ++kt) {
             const int k0 = kt * KT;
+            if (tr) wait_rows_uploaded(rows_ready, (unsigned int)min(k0 + KT, w.n_poles), rows_seen, lane);
             mbar_wait(empty0 + 8 * ps.stage, ps.phase ^ 1u);
             if (lane == 0) {
               const uint32_t full = full0 + 8 * ps.stage;
@@ -468,6 +496,7 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
         } else {
           for (int kt = 0; kt < n_kt; ++kt) {
             const int k0 = kt * KT;
+            if (w.tr) wait_rows_uploaded(rows_ready, (unsigned int)min(k0 + KT, w.n_poles), rows_seen, lane);
             mbar_wait(empty0 + 8 * ps.stage, ps.phase ^ 1u);
             double *sd = reinterpret_cast<double *>(smem + ps.stage * STAGE_BYTES);
             if (w.tr) {
