@@ -203,7 +203,7 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
  * measurements).  PSTGF_HOST_PIPELINE_AUTO (default): one launch per device-sized chunk of R; every piece of at
  * most max_chunk_bytes has a completion counter the kernel bumps, the arrival that completes a piece raises a
  * flag in mapped host memory, and the calling thread, which polls the flags, enqueues the piece's copy-back
- * while the same launch goes on forming the next ones; W is uploaded in slabs of rows behind the launch, whose
+ * while the same launch goes on forming the next ones; W is uploaded in slabs (ranges of poles or of channels) behind the launch, whose
  * load warp waits on a per-wave upload counter (jobs of under about 2 ms of formation take the CHUNKED
  * route anyway).  PSTGF_HOST_PIPELINE_CHUNKED: one launch per piece, copy-back ordered by events.  Same bits
  * either way.

@@ -428,6 +428,7 @@ struct BatchCompletion {
   unsigned int *const *done = nullptr;   // in: per input wave, a zeroed device counter or null
   unsigned int *const *flag = nullptr;   // in: per input wave, a zeroed host-mapped word (device-visible address)
   const unsigned int *const *rows_ready = nullptr;   // in, optional: per input wave, the upload counter of its W
+  const int *ready_counts_channels = nullptr;        // ... and what it counts (DevWave::ready_counts_channels)
   std::vector<int> order;                // out: input wave indices in the order the launch completes them
   std::vector<long long> items;          // out: items of each input wave (arrivals = items * EB)
 };
@@ -478,7 +479,10 @@ static pstgf_status_t form_batch_impl(const pstgf_wave_t *waves, int n_waves, vo
       ds[q].done = completion->done[order[q]];
       ds[q].done_flag = completion->flag[order[q]];
       ds[q].done_target = (unsigned int)(wave_items(ds[q]) * pstgf::EB);   // one arrival per consumer warp and item
-      if (completion->rows_ready) ds[q].rows_ready = completion->rows_ready[order[q]];
+      if (completion->rows_ready) {
+        ds[q].rows_ready = completion->rows_ready[order[q]];
+        ds[q].ready_counts_channels = completion->ready_counts_channels[order[q]];
+      }
     }
   if (completion) {
     // all coarse items come before all fine items: waves with a fine tail finish last
@@ -689,19 +693,25 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
     return e;
   };
   // inputs, first part: allocations and the small arrays (poles, energies).  W follows further down: in the
-  // signalled pipeline it is uploaded in slabs of rows WHILE the launch runs, each slab followed by an update of
-  // the wave's upload counter that the kernel's load warp waits on (the launch starts on the first rows).
+  // signalled pipeline it is uploaded in slabs of poles WHILE the launch runs, each slab followed by an update of
+  // the wave's upload counter that the kernel's load warp waits on stage by stage.
   HostFlags flags;
   if (signalled) PSTGF_CUDA(host_call_flags(ds.device, &flags));
   const bool overlap_upload = signalled && (size_t)n_waves <= MAX_UPLOAD_WAVES;
   if (overlap_upload) PSTGF_CUDA(cudaMemsetAsync(flags.upload_counters, 0, sizeof(unsigned int) * (size_t)n_waves, res.s));
   std::vector<pstgf_wave_t> dev(waves, waves + n_waves);
-  auto upload_W = [&](int p, long long r0, long long r1) -> cudaError_t {   // rows [r0, r1) of the W array of wave p
+  // poles [k0, k1) of all channels, or (by_channels, pole-contiguous W only) channels [k0, k1) with all their poles
+  auto upload_W = [&](int p, long long k0, long long k1, bool by_channels) -> cudaError_t {
     const pstgf_wave_t &w = waves[p];
-    const long long w_cols = w.w_layout == PSTGF_W_CHANNEL_CONTIGUOUS ? w.n_chan : w.n_poles;
-    return cudaMemcpy2DAsync(const_cast<double *>(dev[p].W) + r0 * dev[p].ldw, (size_t)dev[p].ldw * 8, w.W + r0 * w.ldw,
-                             (size_t)w.ldw * 8, (size_t)w_cols * 8, (size_t)(r1 - r0), cudaMemcpyHostToDevice, res.s);
+    double *dst = const_cast<double *>(dev[p].W);
+    const bool tr = w.w_layout == PSTGF_W_CHANNEL_CONTIGUOUS;
+    if (tr || by_channels)                              // whole rows of the array
+      return cudaMemcpy2DAsync(dst + k0 * dev[p].ldw, (size_t)dev[p].ldw * 8, w.W + k0 * w.ldw, (size_t)w.ldw * 8,
+                               (size_t)(tr ? w.n_chan : w.n_poles) * 8, (size_t)(k1 - k0), cudaMemcpyHostToDevice, res.s);
+    return cudaMemcpy2DAsync(dst + k0, (size_t)dev[p].ldw * 8, w.W + k0, (size_t)w.ldw * 8, (size_t)(k1 - k0) * 8,
+                             (size_t)w.n_chan, cudaMemcpyHostToDevice, res.s);   // a column range of every channel
   };
+  std::vector<int> by_channels((size_t)n_waves, 0);
   for (int p = 0; p < n_waves; ++p) {
     const pstgf_wave_t &w = waves[p];
     if (w.n_chan == 0 || w.n_E == 0) continue;
@@ -722,7 +732,7 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
     dev[p].ldw = pitch;
     dev[p].E_k = static_cast<double *>(dEk);
     dev[p].energies = static_cast<double *>(dEn);
-    if (!overlap_upload) PSTGF_CUDA(upload_W(p, 0, w_rows));
+    if (!overlap_upload) PSTGF_CUDA(upload_W(p, 0, w.n_poles, false));
   }
   // Two ways to overlap the copy-back with the formation (pstgf_rmat_set_host_pipeline):
   //  signalled  ONE launch forms a whole chunk (as much of R as the device budget allows); its segments (a wave's
@@ -791,20 +801,26 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
   // the SMs the tail of chunk c has left; both wait for the inputs (and the allocations) enqueued on `stream`
   PSTGF_CUDA(cudaEventRecord(res.inputs, res.s));
   for (cudaStream_t c : res.compute) PSTGF_CUDA(cudaStreamWaitEvent(c, res.inputs, 0));
-  // inputs, second part: W in slabs of rows on `stream`, behind the event the launches wait for, so that the
-  // formation starts on the first slab while the others are still on their way
+  // inputs, second part: W in slabs of poles on `stream`, behind the event the launches wait for, so that the
+  // k loops of the first items run on the first slabs while the others are still on their way
   if (overlap_upload) {
     for (int p = 0; p < n_waves; ++p) {
       const pstgf_wave_t &w = waves[p];
       if (!wave_has_items(w)) continue;
-      const long long w_rows = w.w_layout == PSTGF_W_CHANNEL_CONTIGUOUS ? w.n_poles : w.n_chan;
-      const size_t bytes = sizeof(double) * (size_t)dev[p].ldw * (size_t)w_rows;
-      const long long n_slabs = std::max<long long>(1, std::min<long long>({(long long)MAX_UPLOAD_SLABS, w_rows, (long long)(bytes >> 22)}));
+      const size_t bytes = sizeof(double) * (size_t)w.n_chan * (size_t)w.n_poles;
+      // Slabs of poles when the upload takes no more than about two item times (~1.4 us per k-tile of 20 poles,
+      // ~50 GB/s): the first items' k loops then hide it.  Otherwise slabs of channels, if W's rows are channels.
+      const double t_upload = (double)bytes / 50e9, t_item = 1.4e-6 * ((w.n_poles + pstgf::KT - 1) / pstgf::KT);
+      by_channels[(size_t)p] = (w.w_layout == PSTGF_W_POLE_CONTIGUOUS && t_upload > 2.0 * t_item) ? 1 : 0;
+      const long long extent = by_channels[(size_t)p] ? w.n_chan : w.n_poles;
+      // slabs of at least 4 MiB, and at least 512 bytes per row segment when a slab is a column range
+      const long long n_slabs = std::max<long long>(1, std::min<long long>({(long long)MAX_UPLOAD_SLABS, by_channels[(size_t)p] ? extent : extent / 64,
+                                                                            (long long)(bytes >> 22)}));
       unsigned int *vals = flags.upload_values + (size_t)p * (MAX_UPLOAD_SLABS + 1);
       for (long long sl = 0; sl < n_slabs; ++sl) {
-        const long long r0 = w_rows * sl / n_slabs, r1 = w_rows * (sl + 1) / n_slabs;
-        PSTGF_CUDA(upload_W(p, r0, r1));
-        vals[sl] = (unsigned int)r1;
+        const long long k0 = extent * sl / n_slabs, k1 = extent * (sl + 1) / n_slabs;
+        PSTGF_CUDA(upload_W(p, k0, k1, by_channels[(size_t)p] != 0));
+        vals[sl] = (unsigned int)k1;
         PSTGF_CUDA(cudaMemcpyAsync(flags.upload_counters + p, vals + sl, sizeof(unsigned int), cudaMemcpyHostToDevice, res.s));
       }
     }
@@ -813,6 +829,7 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
   std::vector<pstgf_wave_t> sub;
   std::vector<unsigned int *> done, flag;
   std::vector<const unsigned int *> rows_ready;
+  std::vector<int> ready_kind;
   BatchCompletion completion;
   for (size_t c = 0; c < chunks.size(); ++c) {
     const int b = (int)(c % ring);
@@ -822,6 +839,7 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
     done.clear();
     flag.clear();
     rows_ready.clear();
+    ready_kind.clear();
     const size_t f0 = (size_t)b * MAX_CHUNK_SEGMENTS;
     for (const Segment &g : chunks[c]) {
       pstgf_wave_t w = dev[g.wave];
@@ -833,6 +851,7 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
         done.push_back(flags.counters + f0 + (sub.size() - 1));
         flag.push_back(flags.flags_dev + f0 + (sub.size() - 1));
         rows_ready.push_back(overlap_upload ? flags.upload_counters + g.wave : nullptr);
+        ready_kind.push_back(by_channels[(size_t)g.wave]);
       }
     }
     auto copy_back = [&](const Segment &g) -> cudaError_t {
@@ -848,6 +867,7 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
       completion.done = done.data();
       completion.flag = flag.data();
       completion.rows_ready = rows_ready.data();
+      completion.ready_counts_channels = ready_kind.data();
       st = form_batch_impl(sub.data(), (int)sub.size(), wsbuf[b], wsb, cs, &completion);
       if (st != PSTGF_OK) return st;
       launches += tl_launches;

@@ -77,7 +77,7 @@ struct alignas(128) DevWave {
   double *R_out;
   unsigned int *done;      // optional completion counter of this wave (host-buffer call): += 1 per consumer warp and item
   unsigned int *done_flag; // ... and the (host-mapped) word that is set to 1 by the arrival that makes it done_target
-  const unsigned int *rows_ready;   // optional (host-buffer call): rows of the W array uploaded so far, see the load warp
+  const unsigned int *rows_ready;   // optional (host-buffer call): how much of W has been uploaded so far, see the load warp
   long long ldw;
   double inv2a;            // 1/(2a), PAPER.md:108 prefactor
   int n_chan, n_poles, n_E;
@@ -89,6 +89,7 @@ struct alignas(128) DevWave {
   int use_tma;             // W 16-byte aligned and ldw even
   int n_eb_coarse;         // energy blocks [0, n_eb_coarse) use coarse tiles, [n_eb_coarse, n_eb) fine tiles
   unsigned int done_target;
+  int ready_counts_channels;   // what rows_ready counts: 0 poles uploaded, 1 channels (rows of a pole-contiguous W)
   int tr;                  // 1: W is channel-contiguous [n_poles][ldw] (H.DAT record order), map box [KT][TR_PITCH]
 };
 static_assert(sizeof(DevWave) == 256, "DevWave layout");

@@ -74,9 +74,12 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
                : "d"(a), "d"(b));
 }
 
-// Host-buffer call: W may still be on its way up while the launch runs.  The upload stream bumps a counter
-// after every slab of rows (channels of a pole-contiguous W, poles of a channel-contiguous one); the load warp
-// waits here until the rows its next TMA boxes cover have landed.
+// Host-buffer call: W may still be on its way up while the launch runs.  It is uploaded in slabs, the upload
+// stream bumps a counter after every slab, and the load warp waits here until what it is about to load has
+// landed.  Slabs of poles (column ranges of a pole-contiguous W, rows of a channel-contiguous one) let the k loop
+// of the first items run behind the upload -- good when the upload takes about as long as an item; slabs of
+// channels (rows of a pole-contiguous W) let the tiles near the top of the matrix run at full speed while the
+// rest is still coming -- good when the upload takes many item times (the 6.2 GB of the paper-scale wave).
 __device__ __forceinline__ void wait_rows_uploaded(const unsigned int *rows_ready, unsigned int need, unsigned int &seen,
                                                    int lane) {
   if (seen >= need) return;
@@ -467,13 +470,14 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
         const CUtensorMap *map = &w.map;
         const int i_boxes = (nrb + TN / 8 - 1) / (TN / 8);     // I panel: one to four boxes of 32 rows
         const uint32_t tx_bytes = (i_boxes + (kind != 0 ? 1 : 0)) * (w.tr ? TR_BOX_BYTES : BOX_BYTES);
-        // rows of W this item reads (pole-contiguous W: channels; the poles of a channel-contiguous W are waited
-        // for stage by stage below)
+        // host-buffer call: W uploaded so far.  Slabs of channels are waited for here, once per item (the rows and
+        // columns of its tile); slabs of poles stage by stage below.
         const unsigned int *rows_ready = w.rows_ready;
         unsigned int rows_seen = rows_ready ? 0u : 0xffffffffu;
-        if (rows_ready && !w.tr) {
+        if (rows_ready && w.ready_counts_channels) {
           const int last = kind == 0 ? row0 + nrb * 8 : max(row0 + nrb * 8, col0 + nblk * 8);
           wait_rows_uploaded(rows_ready, (unsigned int)min(last, w.n_chan), rows_seen, lane);
+          rows_seen = 0xffffffffu;
         }
         if (w.use_tma) {
           // TMA box coordinates: (pole, channel) for pole-contiguous W, (channel, pole) for the H.DAT order
@@ -481,7 +485,7 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
           const uint32_t box = tr ? TR_BOX_BYTES : BOX_BYTES;
           for (int kt = 0; kt < n_kt; ++kt) {
             const int k0 = kt * KT;
-            if (tr) wait_rows_uploaded(rows_ready, (unsigned int)min(k0 + KT, w.n_poles), rows_seen, lane);
+            wait_rows_uploaded(rows_ready, (unsigned int)min(k0 + KT, w.n_poles), rows_seen, lane);
             mbar_wait(empty0 + 8 * ps.stage, ps.phase ^ 1u);
             if (lane == 0) {
               const uint32_t full = full0 + 8 * ps.stage;
@@ -496,7 +500,7 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
         } else {
           for (int kt = 0; kt < n_kt; ++kt) {
             const int k0 = kt * KT;
-            if (w.tr) wait_rows_uploaded(rows_ready, (unsigned int)min(k0 + KT, w.n_poles), rows_seen, lane);
+            wait_rows_uploaded(rows_ready, (unsigned int)min(k0 + KT, w.n_poles), rows_seen, lane);
             mbar_wait(empty0 + 8 * ps.stage, ps.phase ^ 1u);
             double *sd = reinterpret_cast<double *>(smem + ps.stage * STAGE_BYTES);
             if (w.tr) {
