@@ -269,6 +269,19 @@ def test_single_wave_call_in_a_cuda_graph(rmat, oracle):
     _check(out.cpu().numpy(), R_ref)
 
 
+def test_host_call_with_pageable_memory(rmat, oracle):
+    """Pinned host memory is recommended, not required: plain numpy-backed tensors work (the copies then block)."""
+    from paper_1909_07321_b200 import inputs
+    for w in (inputs.make_wave(88, 96, 20000, 64), inputs.make_wave(89, 40, 100, 9)):   # signalled and chunked routes
+        R = torch.full((w.n_E, w.n_chan, w.n_chan), np.nan, dtype=torch.float64)
+        rmat.pstgf_rmat_form_batch_host([(torch.from_numpy(w.W.copy()), torch.from_numpy(w.E_k.copy()),
+                                          torch.from_numpy(w.energies.copy()), w.a, R)])
+        pick = sorted({0, w.n_E // 2, w.n_E - 1})
+        _check(R.numpy()[pick], oracle.rmat_form(w.W, w.E_k, w.energies[pick], w.a, threads=_threads()))
+        Rn = rmat.pstgf_rmat_form_naive(_dev(w.W), _dev(w.E_k), _dev(w.energies), w.a).cpu().numpy()
+        _check(R.numpy(), Rn)
+
+
 def test_host_call_signalled_pipeline(rmat, oracle):
     """The signalled pipeline on a longer run: ONE launch, pieces copied back as their completion flags come up.
     Small pieces, every energy checked against the term-by-term device kernel, sampled energies against the
