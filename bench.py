@@ -42,8 +42,12 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
-    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5, 6],
-                    help="1-5: BASELINE.json configs[0..4]; 6: the paper-scale wave of PAPER.md:168 (7261 x 106661)")
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5, 6, 7],
+                    help="1-5: BASELINE.json configs[0..4]; 6: the paper-scale wave of PAPER.md:168 (7261 x 106661); "
+                         "7: 256 small waves, n_chan in [8, 32] (PAPER.md:676 shape: many partial waves in one call)")
+    ap.add_argument("--n-E", type=int, default=0, dest="n_E",
+                    help="override the energies per wave (the mesh keeps its range): PSTGF calls RINIT once per "
+                         "(wave, energy), PAPER.md:122-126, so few-energy calls are a workload of their own")
     ap.add_argument("--w-layout", choices=["poles", "channels"], default="poles",
                     help="memory order of W on the device: pole-contiguous [n_chan][n_poles] (default, north_star's) or "
                          "channel-contiguous [n_poles][n_chan], the H.DAT record order of PAPER.md:535")
@@ -54,6 +58,9 @@ def parse_args():
     ap.add_argument("--tail-policy", choices=["auto", "none", "all"], default="auto",
                     help="scheduling knob of the library (pstgf_rmat_set_tail_policy): fine-tile tail sized automatically "
                          "(default), coarse tiles only, fine tiles only; same bits, for measurements")
+    ap.add_argument("--slab-policy", choices=["auto", "none", "32", "64", "128"], default="auto",
+                    help="how the n_E mod 8 energies are cut (pstgf_debug_set_slab_policy): tile edge chosen by the planner "
+                         "(default), left to a partly idle block of 8 (round-1 behaviour), or a forced edge; same bits")
     ap.add_argument("--e2e-chunk-mib", type=int, default=0,
                     help="max_chunk_bytes of pstgf_rmat_form_batch_host in MiB (0 = the library's default)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
@@ -137,7 +144,8 @@ def workload_description(cfg: int, wl) -> dict:
     names = {1: "configs[0] single wave 8x160, n_E 1000", 2: "configs[1] single wave 64x1280, n_E 4096",
              3: "configs[2] 8 waves 256x5120, n_E 2048 shared", 4: "configs[3] ragged 32 waves n_chan U[16,400], n_E 512",
              5: "configs[4] large single wave 512x10240, n_E 256",
-             6: "paper-scale single wave 7261x106661 (PAPER.md:168), n_E 16 [not in BASELINE.json configs]"}
+             6: "paper-scale single wave 7261x106661 (PAPER.md:168), n_E 16 [not in BASELINE.json configs]",
+             7: "256 small waves n_chan U[8,32], n_poles 20 n_chan, n_E 512 [not in BASELINE.json configs]"}
     return {"workload": names[cfg], "config_index": cfg - 1, "seed": wl.seed, "n_waves": len(wl.waves),
             "n_chan": [w.n_chan for w in wl.waves] if len(wl.waves) <= 8 else
             {"min": min(w.n_chan for w in wl.waves), "max": max(w.n_chan for w in wl.waves)},
@@ -209,7 +217,7 @@ def run_reference(args):
     if rank != 0:
         return 0
     from paper_1909_07321_b200 import inputs
-    wl = inputs.make_config(args.config)
+    wl = inputs.make_config(args.config, n_E=args.n_E or None)
     cores = oracle_cores()
     per_e = est_oracle_seconds_per_energy(wl)
     budget = 120.0 / max(1, args.steps + args.warmup)            # whole run within a few minutes
@@ -357,20 +365,22 @@ def run_cuda(args):
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     rmat.load()          # raises if libpstgf_rmat.so is missing
-    rmat.pstgf_rmat_set_tail_policy({"auto": rmat.PSTGF_TAIL_AUTO, "none": rmat.PSTGF_TAIL_NONE,
-                                     "all": rmat.PSTGF_TAIL_ALL}[args.tail_policy])
+    rmat.pstgf_debug_set_tail_policy({"auto": rmat.PSTGF_TAIL_AUTO, "none": rmat.PSTGF_TAIL_NONE,
+                                      "all": rmat.PSTGF_TAIL_ALL}[args.tail_policy])
+    rmat.pstgf_debug_set_slab_policy({"auto": rmat.PSTGF_SLAB_AUTO, "none": rmat.PSTGF_SLAB_NONE, "32": rmat.PSTGF_SLAB_T32,
+                                      "64": rmat.PSTGF_SLAB_T64, "128": rmat.PSTGF_SLAB_T128}[args.slab_policy])
     peaks = measured_peaks()
 
     # Weak scaling over ranks: at N ranks the job is the configuration with an N times
     # finer energy mesh; shard.plan gives each rank its wave-rotated share of the energy blocks (PAPER.md:116,
     # :135-137, Fig. 1), i.e. the configuration's own n_E per wave and rank.  No data-path collective.
     if world == 1:
-        wl = inputs.make_config(args.config)
+        wl = inputs.make_config(args.config, n_E=args.n_E or None)
         n_e_job = wl.n_energies()
     else:
         from paper_1909_07321_b200 import shard
         base = inputs.config_shapes(args.config)
-        wl_job = inputs.make_config(args.config, n_E=world * base[0][2])
+        wl_job = inputs.make_config(args.config, n_E=world * (args.n_E or base[0][2]))
         n_e_job = wl_job.n_energies()
         wl = inputs.Workload(name=wl_job.name, seed=wl_job.seed)
         for p, idx in shard.plan([w.n_E for w in wl_job.waves], rank, world):
@@ -455,6 +465,7 @@ def run_cuda(args):
     # FP64 peak: probe the DMMA pipe (the instruction the kernel issues) right here, burst, best of 5
     probe = None
     if rank == 0:
+        from paper_1909_07321_b200.measure import probe as probe_lib      # libpstgf_probe.so: bench-side, not the product
         sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
         sink = torch.empty(sms * 4 * 256, dtype=torch.float64, device="cuda")
         probe = {}
@@ -463,7 +474,7 @@ def run_cuda(args):
             for _ in range(5):
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 e0.record()
-                fl = rmat.pstgf_fp64_probe(kind, 2000, sms * 2, 256, sink)
+                fl = probe_lib.fp64_probe(kind, 2000, sms * 2, 256, sink)
                 e1.record()
                 torch.cuda.synchronize()
                 best = max(best, fl / (e0.elapsed_time(e1) * 1e-3) / 1e12)

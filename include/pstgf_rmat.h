@@ -21,15 +21,20 @@
  *    (allocate them with any CUDA allocator, e.g. PyTorch).  Any pointer the
  *    device can dereference works, mapped pinned host memory included (R_out
  *    there makes every store a PCIe write: about six times slower than device
- *    memory plus a copy; pstgf_rmat_form_batch_host is the fast host path).  The library
- *    allocates no device memory in the DEVICE-pointer calls (but for the 8 KiB
- *    counter pool of pstgf_rmat_form, once per device); the batch call keeps
- *    its tables in the caller's workspace.
+ *    memory plus a copy; pstgf_rmat_form_batch_host is the fast host path).
+ *  - Device memory owned by the library.  The DEVICE-pointer calls allocate
+ *    none, but for the 8 KiB counter pool of pstgf_rmat_form (once per
+ *    device); the batch call keeps its tables in the caller's workspace.
+ *    pstgf_rmat_form_batch_host stages through a memory pool of its own (one
+ *    per device) and keeps 33 KiB of completion words per calling thread.
+ *    pstgf_rmat_finalize() frees all of it.
  *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default
  *    stream).  DEVICE-pointer calls enqueue work and return without
  *    synchronising; buffers must stay alive until the stream reaches the end
  *    of the enqueued work.  Host structs (pstgf_wave_t arrays) are consumed
- *    before the call returns.
+ *    before the call returns.  pstgf_rmat_form / _form_hdat may be captured
+ *    into a CUDA graph; the batch calls may not (PSTGF_ERR_CAPTURE: their
+ *    tables travel by a copy from the call's own host memory).
  *  - Layout: W is row-major [n_chan][ldw], element (n,k) at W[n*ldw + k],
  *    ldw >= n_poles (k contiguous), unless the wave says
  *    PSTGF_W_CHANNEL_CONTIGUOUS (the H.DAT record order).  R_out is dense row-major
@@ -37,7 +42,8 @@
  *    R_out[e][m][n] bitwise.  R_out must not overlap any input or another
  *    wave's R_out.  Inputs may be shared between waves.
  *  - Sizes: n_E == 0, n_chan == 0 or n_waves == 0 -> PSTGF_OK, nothing
- *    written.  n_poles == 0 -> R_out is zero-filled (empty sum).
+ *    written.  n_poles == 0 -> the sum is empty: R_out is zero-filled (plus
+ *    diag_add on the diagonal, if given).
  *  - An energy equal to a pole is not detected (data lives on the device):
  *    IEEE semantics apply (inf/NaN in that energy's R).  The paper is silent;
  *    callers keep a clearance (the synthetic workloads use 1e-3 Ryd).
@@ -47,7 +53,9 @@
  *    pitch, or accept the slower path); otherwise a slower load path inside the same kernel is
  *    used.  Any n_chan (odd included) is supported.
  *  - Results are deterministic: each R element is produced by exactly one
- *    thread with a fixed k order, whatever CTA picked the work item up.
+ *    thread with a fixed k order, whatever CTA picked the work item up, and
+ *    however the energies of a call are grouped: an energy gives the same bits
+ *    in a call of 1 energy, of 7 or of 4096.
  *  - Errors are returned as pstgf_status_t; nothing is thrown or printed.
  *    Argument errors are detected before anything is enqueued.
  */
@@ -60,7 +68,7 @@
 extern "C" {
 #endif
 
-#define PSTGF_RMAT_VERSION 103 /* major*100 + minor */
+#define PSTGF_RMAT_VERSION 200 /* major*100 + minor; 2.x: pstgf_wave_t grew diag_add (72 bytes) */
 
 typedef enum {
   PSTGF_OK = 0,
@@ -68,7 +76,9 @@ typedef enum {
   PSTGF_ERR_ALIGNMENT = 2,          /* a pointer is not 8-byte aligned */
   PSTGF_ERR_WORKSPACE = 3,          /* workspace NULL, not 256-byte aligned, or smaller than the query says */
   PSTGF_ERR_UNSUPPORTED_DEVICE = 4, /* no CUDA device, or the current device is not compute capability 10.x */
-  PSTGF_ERR_CUDA = 5                /* a CUDA runtime/driver call failed; see pstgf_last_cuda_error() */
+  PSTGF_ERR_CUDA = 5,               /* a CUDA runtime/driver call failed; see pstgf_last_cuda_error() */
+  PSTGF_ERR_TIMEOUT = 6,            /* pstgf_rmat_form_batch_host: the launch gave up waiting for an upload of W; R_out undefined */
+  PSTGF_ERR_CAPTURE = 7             /* the stream is being captured and this call cannot be (see above) */
 } pstgf_status_t;
 
 /*
@@ -87,7 +97,21 @@ typedef struct {
   const double *E_k;      /* [n_poles] */
   const double *energies; /* [n_E] */
   double *R_out;          /* [n_E][n_chan][n_chan] */
+  const double *diag_add; /* optional (NULL = none) [n_E][n_chan]: R_out[e][n][n] = eq. 4 + diag_add[e][n], see below */
 } pstgf_wave_t;
+
+/*
+ * diag_add: a per-(energy, channel) addend for the diagonal of R, applied by
+ * the same epilogue that scales by 1/(2a) and writes R (no second pass over
+ * R): R_out[e][n][n] = (1/2a) sum_k w_nk^2 / (E_k - E_e) + diag_add[e][n];
+ * off-diagonal elements are untouched (bitwise).  This is where a Buttle
+ * correction goes.  PAPER.md lists the DATA of that correction -- records
+ * NBUTD / EBUTD / CBUTD per target angular momentum ("the
+ * coefficients of the Buttle correction", :544; file DBUT for old inner-region
+ * codes, :581-583) -- but NOT its formula (that is in the paper's refs [3],
+ * [17]): the formula is not in PAPER.md, so the caller evaluates it and
+ * supplies the diagonal.
+ */
 
 /*
  * Memory order of W.
@@ -114,7 +138,12 @@ typedef struct {
  *   R_out    [n_E][n_chan][n_chan]
  * One persistent kernel launch (plus a zero-fill when n_poles == 0); work
  * items (energy block, upper-triangle tile) are drawn by the CTAs from an
- * atomic counter.  The counter lives in a pool of 64 slots (8 KiB of device
+ * atomic counter.  PSTGF forms R once per (partial wave, energy) (loop over
+ * E -> RINIT; one energy per processor at :694): a call
+ * with few energies (and the n_E mod 8 energies of any call) is cut into
+ * items in which the CTA's eight compute warps share ONE or TWO energies and
+ * split the tile instead, so n_E = 1 is a first-class
+ * shape.  The counter lives in a pool of 64 slots (8 KiB of device
  * memory per device, allocated by the library at the first call -- the only
  * device allocation of the DEVICE-pointer calls); when 64 launches are in
  * flight at once, or `stream` is being captured into a CUDA graph, items are
@@ -132,22 +161,6 @@ pstgf_status_t pstgf_rmat_form(const double *W, long long ldw, const double *E_k
 pstgf_status_t pstgf_rmat_form_hdat(const double *Wt, long long ldw, const double *E_k,
                                     const double *energies, int n_chan, int n_poles, int n_E,
                                     double a, double *R_out, void *stream);
-
-/*
- * Scheduling knob (process-wide; meant for tests and measurements).  Work
- * items are handed to the persistent CTAs largest first; the END of that list
- * -- about one round of the grid's worth of work -- is cut into finer tiles
- * (32-row instead of 64-row) so that the CTAs run dry together, the device-
- * side counterpart of the paper's concern that no processor be left waiting
- * (PAPER.md:135-137, Fig. 1).  PSTGF_TAIL_AUTO (default) sizes that tail
- * itself, PSTGF_TAIL_NONE uses coarse tiles only, PSTGF_TAIL_ALL fine tiles
- * only.  Every R element has the same operands and summation order under all
- * three policies: results are bitwise identical.
- */
-#define PSTGF_TAIL_AUTO 0
-#define PSTGF_TAIL_NONE 1
-#define PSTGF_TAIL_ALL 2
-pstgf_status_t pstgf_rmat_set_tail_policy(int policy);
 
 /*
  * Bytes of device workspace pstgf_rmat_form_batch needs for these waves
@@ -171,60 +184,107 @@ pstgf_status_t pstgf_rmat_form_batch(const pstgf_wave_t *waves, int n_waves, voi
                                      size_t workspace_bytes, void *stream);
 
 /*
- * The same result as pstgf_rmat_form from a one-thread-per-element kernel
- * that follows eq. 4 term by term ((w_n*w_m)/(E_k-E), k ascending,
- * compensated sum).  Slow; provided so that callers and tests can check every
- * energy of a large run against an independent device evaluation.
- * DEVICE: W, E_k, energies, R_out.  `w_layout` as in pstgf_wave_t.
+ * The same result as the calls above for ONE wave (HOST struct, DEVICE
+ * pointers) from a one-thread-per-element kernel that follows eq. 4 term by
+ * term ((w_n*w_m)/(E_k-E), k ascending, compensated sum, then diag_add).
+ * Slow; provided so that callers and tests can check every energy of a large
+ * run against an independent device evaluation.
  */
-pstgf_status_t pstgf_rmat_form_naive(const double *W, long long ldw, const double *E_k,
-                                     const double *energies, int n_chan, int n_poles, int n_E,
-                                     double a, double *R_out, int w_layout, void *stream);
+pstgf_status_t pstgf_rmat_form_naive(const pstgf_wave_t *wave, void *stream);
 
 /*
  * End-to-end convenience over HOST buffers: `waves` holds HOST pointers
  * (pinned memory recommended; pageable memory works but copies synchronously).
  * Inputs are copied to the device on `stream`, R is formed on streams of the
  * library's own in pieces of whole energy blocks and copied back into the host
- * R_out on another stream while the next pieces are being formed (see
- * pstgf_rmat_set_host_pipeline; device staging for R is bounded by a third
- * of the free device memory, at most 16 GiB, per chunk).  Device memory comes from a stream-ordered pool the
- * library owns (one per device, kept for the life of the process so that
- * repeated calls do not re-grow it).  SYNCHRONISES before returning.
+ * R_out on another stream while the next pieces are being formed.  Device
+ * staging for R is bounded per chunk by a quarter of the device's memory, at
+ * most 16 GiB, and halved (down to one piece) when that allocation fails
+ * because another allocator holds the memory.  Device memory comes from a
+ * stream-ordered pool the library owns (one per device, kept until
+ * pstgf_rmat_finalize so that repeated calls do not re-grow it).
+ * SYNCHRONISES before returning.
  * `max_chunk_bytes` bounds a piece (0 = default: 1/32 of all R in [8, 64] MiB
  * for the signalled pipeline, 1/8 in [16, 256] MiB for the chunked one); a
  * piece always holds at least one energy block.
+ * W is uploaded in slabs behind the launch, which waits for the slab it needs
+ * next; that wait is bounded (2 s): if an upload never arrives the launch
+ * drains and the call returns PSTGF_ERR_TIMEOUT with R_out undefined.
  */
 pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves,
                                           size_t max_chunk_bytes, void *stream);
 
 /*
- * How pstgf_rmat_form_batch_host overlaps formation and copy-back (process-wide knob for tests and
- * measurements).  PSTGF_HOST_PIPELINE_AUTO (default): one launch per device-sized chunk of R; every piece of at
+ * Energy mesh in the units of eq. 4 from the mesh of the namelists: PSTGF's
+ * input meshes are "z-scaled energies in Rydberg, E/z^2" (E0, EINCR:
+ * PAPER.md:431-435; EMESH: PAPER.md:503), while eq. 4 needs E
+ * on the scale of the poles E_k.  HOST arrays: e_out[i] = z*z * e_scaled[i]
+ * for i in [0, n) (one rounding of z*z, one per product); e_out may alias
+ * e_scaled.  z is the scaling charge, finite and > 0 (the paper does not say
+ * what scale a neutral target uses: the caller passes the one its mesh was
+ * written in, e.g. 1).  The origin is not moved: meshes given relative to a
+ * threshold are the caller's to shift.
+ */
+pstgf_status_t pstgf_mesh_from_zscaled(const double *e_scaled, long long n, double z, double *e_out);
+
+/*
+ * Frees everything the library keeps between calls (counter pools, the host
+ * call's memory pools and completion words, planner caches) after waiting for
+ * the devices it used to go idle.  No call of this library may be in flight in
+ * another thread.  The library may be used again afterwards.
+ */
+pstgf_status_t pstgf_rmat_finalize(void);
+
+/* ---- knobs for tests and measurements ------------------------------------------------------------
+ * THREAD-LOCAL: each affects only the calls the calling thread makes afterwards.  None changes a
+ * single bit of any result. */
+
+/*
+ * Work items are handed to the persistent CTAs largest first; the END of that list
+ * -- about one round of the grid's worth of work -- is cut into finer tiles
+ * (32-row instead of 64-row) so that the CTAs run dry together, the device-
+ * side counterpart of the paper's concern that no processor be left waiting
+ * (PAPER.md:135-137, Fig. 1).  PSTGF_TAIL_AUTO (default) sizes that tail
+ * itself, PSTGF_TAIL_NONE uses coarse tiles only, PSTGF_TAIL_ALL fine tiles
+ * only.
+ */
+#define PSTGF_TAIL_AUTO 0
+#define PSTGF_TAIL_NONE 1
+#define PSTGF_TAIL_ALL 2
+pstgf_status_t pstgf_debug_set_tail_policy(int policy);
+
+/*
+ * The n_E mod 8 energies that do not fill a block of 8 are taken two or one at
+ * a time by "slab" items whose eight warps split a square tile.
+ * PSTGF_SLAB_AUTO (default) picks the tile edge (128, 64 or 32) that gives
+ * the grid enough items; PSTGF_SLAB_NONE leaves the remainder to a partly
+ * idle block of 8 (the round-1 behaviour); _T32/_T64/_T128 force an edge.
+ */
+#define PSTGF_SLAB_AUTO 0
+#define PSTGF_SLAB_NONE 1
+#define PSTGF_SLAB_T32 2
+#define PSTGF_SLAB_T64 3
+#define PSTGF_SLAB_T128 4
+pstgf_status_t pstgf_debug_set_slab_policy(int policy);
+
+/*
+ * How pstgf_rmat_form_batch_host overlaps formation and copy-back.
+ * PSTGF_HOST_PIPELINE_AUTO (default): one launch per device-sized chunk of R; every piece of at
  * most max_chunk_bytes has a completion counter the kernel bumps, the arrival that completes a piece raises a
  * flag in mapped host memory, and the calling thread, which polls the flags, enqueues the piece's copy-back
- * while the same launch goes on forming the next ones; W is uploaded in slabs (ranges of poles or of channels) behind the launch, whose
- * load warp waits on a per-wave upload counter (jobs of under about 2 ms of formation take the CHUNKED
- * route anyway).  PSTGF_HOST_PIPELINE_CHUNKED: one launch per piece, copy-back ordered by events.  Same bits
- * either way.
+ * while the same launch goes on forming the next ones; W is uploaded in slabs (ranges of poles or of channels)
+ * behind the launch, whose load warp waits on a per-wave upload counter (jobs of under about 2 ms of formation
+ * take the CHUNKED route anyway).  PSTGF_HOST_PIPELINE_CHUNKED: one launch per piece, copy-back ordered by events.
  */
 #define PSTGF_HOST_PIPELINE_AUTO 0
 #define PSTGF_HOST_PIPELINE_CHUNKED 1
-pstgf_status_t pstgf_rmat_set_host_pipeline(int mode);
+pstgf_status_t pstgf_debug_set_host_pipeline(int mode);
 
-/*
- * Measurement utility (not on the hot path): a register-resident FP64
- * throughput probe that fixes the roofline denominator of the contraction
- * (MEASURED_PEAKS.json has no FP64 entry).  kind 0 = DMMA.8x8x4 (the
- * instruction the SYRK kernel issues, in its register-tile pattern), 1 = DFMA,
- * 2 = DMMA on even warps and DFMA on odd warps.
- * Launches `blocks` CTAs of `threads` threads (multiple of 32, <= 256) that
- * each run `iters` iterations; DEVICE `sink` receives blocks*threads doubles.
- * HOST `flop_out` (may be NULL) receives the FLOPs the launch performs
- * (2 per FMA).  Asynchronous on `stream`; time it with events.
- */
-pstgf_status_t pstgf_fp64_probe(int kind, int iters, int blocks, int threads, double *sink,
-                                double *flop_out, void *stream);
+/* Bound, in ms, on the kernel's wait for an upload slab of W (0 = the default, 2000). */
+pstgf_status_t pstgf_debug_set_upload_timeout_ms(unsigned int ms);
+/* on != 0: the host call uploads W but withholds the "slab uploaded" signals, so the launch must take its
+ * time-out path (a test of PSTGF_ERR_TIMEOUT). */
+pstgf_status_t pstgf_debug_stall_upload(int on);
 
 /* Kernel launches enqueued by this thread's last successful call (for accounting). */
 int pstgf_last_launch_count(void);

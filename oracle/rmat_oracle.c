@@ -25,8 +25,15 @@
  * Pins (tests/test_oracle_pins.py): exact rational brute force, the hand
  * example of tests/golden/eq4_hand_example.txt, the single-pole closed form,
  * symmetry, definiteness, the resolvent identity, exact scalings, block
- * structure, additivity, degenerate poles vs. a library SYRK.  Nothing in
- * this file is "parity unpinned".
+ * structure, additivity, degenerate poles vs. a library SYRK; the leading
+ * dimension (ldw > n_poles) and the diagonal addend have pins of their own.
+ * Nothing in this file is "parity unpinned".
+ *
+ * The optional diagonal addend (diag_add[e][n], added to R_nn after the
+ * division by 2a) is where a caller puts a Buttle correction: PAPER.md lists
+ * that correction's data (records NBUTD/EBUTD/CBUTD, PAPER.md:524-528, :544,
+ * file DBUT :581-583) but not its formula, so the oracle -- like the library
+ * -- takes the diagonal from the caller and only defines where it goes.
  *
  * Build: gcc -O2 -std=c11 -fno-fast-math -ffp-contract=off -fopenmp -fPIC -shared
  * (-ffp-contract=off keeps the compensation from being fused away).
@@ -58,13 +65,15 @@ static double eq4_entry(const double *w_n, const double *w_m, const double *E_k,
 /*
  * R_out[e][n][m] for e in [0,n_E), n,m in [0,n_chan): dense, row-major.
  * W is row-major [n_chan][ldw] with k contiguous (reading R6).
+ * diag_add (may be NULL) is [n_E][n_chan]: R_out[e][n][n] += diag_add[e][n],
+ * one rounded addition after the division by 2a.
  * threads <= 1 runs serially; threads > 1 splits the energy loop only
  * (the arithmetic of each entry is unchanged).  Returns 0, or 1 on bad
  * arguments.
  */
 int oracle_rmat_form(const double *W, long long ldw, const double *E_k,
                      const double *energies, int n_chan, int n_poles, int n_E,
-                     double a, double *R_out, int threads)
+                     double a, const double *diag_add, double *R_out, int threads)
 {
     if (n_chan < 0 || n_poles < 0 || n_E < 0 || ldw < n_poles) return 1;
     if (n_chan == 0 || n_E == 0) return 0;
@@ -81,6 +90,9 @@ int oracle_rmat_form(const double *W, long long ldw, const double *E_k,
             for (int m = 0; m < n_chan; ++m)
                 R[(size_t)n * n_chan + m] =
                     eq4_entry(W + (size_t)n * ldw, W + (size_t)m * ldw, E_k, n_poles, E, a);
+        if (diag_add)
+            for (int n = 0; n < n_chan; ++n)
+                R[(size_t)n * n_chan + n] += diag_add[(size_t)e * n_chan + n];
     }
     return 0;
 }

@@ -37,7 +37,7 @@ def _load():
         lib = ctypes.CDLL(build())
         dp = ctypes.POINTER(ctypes.c_double)
         lib.oracle_rmat_form.argtypes = [dp, ctypes.c_longlong, dp, dp, ctypes.c_int, ctypes.c_int,
-                                         ctypes.c_int, ctypes.c_double, dp, ctypes.c_int]
+                                         ctypes.c_int, ctypes.c_double, dp, dp, ctypes.c_int]
         lib.oracle_rmat_form.restype = ctypes.c_int
         ip = ctypes.POINTER(ctypes.c_int)
         lib.oracle_rmat_entries.argtypes = [dp, ctypes.c_longlong, dp, dp, ctypes.c_int, ctypes.c_int, ctypes.c_int,
@@ -57,23 +57,38 @@ def _dptr(a: np.ndarray):
     return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
 
 
-def rmat_form(W, E_k, energies, a: float, threads: int = 1) -> np.ndarray:
+def rmat_form(W, E_k, energies, a: float, threads: int = 1, diag_add=None) -> np.ndarray:
     """R[e, n, m] of eq. 4 for one partial wave.
 
-    W [n_chan, n_poles] (row-major, any ld via a strided view's base is NOT
-    supported: the array is made contiguous), E_k [n_poles], energies [n_E].
+    W [n_chan, n_poles], E_k [n_poles], energies [n_E].  A float64 W whose rows are contiguous (unit stride
+    along the poles) is passed as it is, with its row stride as the leading dimension ldw >= n_poles (a
+    column slice of a wider array is NOT copied); anything else is made contiguous first.
+    diag_add, if given, is [n_E, n_chan] and is added to the diagonal of each R[e] (see rmat_oracle.c).
     """
-    W = np.ascontiguousarray(W, dtype=np.float64)
+    W = np.asarray(W, dtype=np.float64)
+    if W.ndim != 2:
+        raise ValueError("W must be [n_chan, n_poles]")
+    item = W.itemsize
+    rows_ok = W.shape[1] <= 1 or W.strides[1] == item
+    ld_ok = W.shape[0] <= 1 or (W.strides[0] % item == 0 and W.strides[0] // item >= W.shape[1])
+    if not (rows_ok and ld_ok):
+        W = np.ascontiguousarray(W)
     E_k = np.ascontiguousarray(E_k, dtype=np.float64)
     energies = np.ascontiguousarray(energies, dtype=np.float64)
-    if W.ndim != 2 or E_k.ndim != 1 or energies.ndim != 1 or W.shape[1] != E_k.shape[0]:
+    if E_k.ndim != 1 or energies.ndim != 1 or W.shape[1] != E_k.shape[0]:
         raise ValueError("shape mismatch: W [n_chan, n_poles], E_k [n_poles], energies [n_E]")
     n_chan, n_poles = W.shape
+    ldw = W.strides[0] // item if n_chan > 1 else n_poles
     n_E = energies.shape[0]
+    da = None
+    if diag_add is not None:
+        da = np.ascontiguousarray(diag_add, dtype=np.float64)
+        if da.shape != (n_E, n_chan):
+            raise ValueError("diag_add must be [n_E, n_chan]")
     R = np.zeros((n_E, n_chan, n_chan), dtype=np.float64)
-    # ld >= 1 keeps ctypes happy for n_poles == 0
-    rc = _load().oracle_rmat_form(_dptr(W), max(n_poles, 0), _dptr(E_k), _dptr(energies),
-                                  n_chan, n_poles, n_E, float(a), _dptr(R), int(threads))
+    rc = _load().oracle_rmat_form(_dptr(W), max(ldw, n_poles), _dptr(E_k), _dptr(energies),
+                                  n_chan, n_poles, n_E, float(a), _dptr(da) if da is not None else None,
+                                  _dptr(R), int(threads))
     if rc != 0:
         raise ValueError(f"oracle_rmat_form rejected its arguments (rc={rc})")
     return R

@@ -1,6 +1,8 @@
-"""In-tree nvcc build of libpstgf_rmat.so for sm_100a (no JIT cache: the .so travels with the tree)."""
+"""In-tree nvcc build of libpstgf_rmat.so (the product) and libpstgf_probe.so (the FP64 throughput probe bench.py
+uses) for sm_100a (no JIT cache: the .so files travel with the tree)."""
 from __future__ import annotations
 
+import hashlib
 import os
 import shutil
 import subprocess
@@ -8,9 +10,11 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libpstgf_rmat.so")
-SOURCES = [os.path.join(CSRC, "pstgf_rmat.cu"), os.path.join(CSRC, "fp64_probe.cu")]
+SOURCES = [os.path.join(CSRC, "pstgf_rmat.cu")]
 HEADERS = [os.path.join(CSRC, "rmat_common.h"), os.path.join(CSRC, "rmat_kernel.cuh"),
            os.path.join(os.path.dirname(_HERE), "include", "pstgf_rmat.h")]
+PROBE_LIB = os.path.join(_HERE, "libpstgf_probe.so")
+PROBE_SOURCES = [os.path.join(_HERE, "measure", "fp64_probe.cu")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 
@@ -22,20 +26,45 @@ def nvcc_path() -> str:
     raise RuntimeError("nvcc not found: libpstgf_rmat.so cannot be built")
 
 
-def is_stale() -> bool:
-    if not os.path.exists(LIB):
+def _source_hash(deps: list[str]) -> str:
+    h = hashlib.sha256(" ".join(NVCC_FLAGS).encode())
+    for f in deps:
+        with open(f, "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()
+
+
+def _stale(lib: str, deps: list[str]) -> bool:
+    """A library is current when the hash of its sources (recorded beside it at build time) matches: file times
+    do not survive a copy of the tree to another machine, contents do."""
+    stamp = lib + ".srchash"
+    if not os.path.exists(lib) or not os.path.exists(stamp):
         return True
-    t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(f) > t for f in SOURCES + HEADERS)
+    with open(stamp) as fh:
+        return fh.read().strip() != _source_hash(deps)
+
+
+def is_stale() -> bool:
+    """True when libpstgf_rmat.so is missing or was built from other sources than the ones in the tree."""
+    return _stale(LIB, SOURCES + HEADERS)
+
+
+def _compile(lib: str, sources: list[str], deps: list[str], verbose: bool) -> None:
+    tmp = lib + f".tmp{os.getpid()}"
+    digest = _source_hash(deps)
+    cmd = [nvcc_path(), *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), *sources, "-o", tmp]
+    subprocess.run(cmd, check=True)
+    os.replace(tmp, lib)
+    with open(lib + ".srchash", "w") as fh:
+        fh.write(digest + "\n")
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile csrc/ into libpstgf_rmat.so if it is missing or older than its sources."""
+    """Compile csrc/ into libpstgf_rmat.so (and measure/ into libpstgf_probe.so) if missing or older than the sources."""
     if force or is_stale():
-        tmp = LIB + f".tmp{os.getpid()}"
-        cmd = [nvcc_path(), *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), *SOURCES, "-o", tmp]
-        subprocess.run(cmd, check=True)
-        os.replace(tmp, LIB)
+        _compile(LIB, SOURCES, SOURCES + HEADERS, verbose)
+    if force or _stale(PROBE_LIB, PROBE_SOURCES):
+        _compile(PROBE_LIB, PROBE_SOURCES, PROBE_SOURCES, verbose)
     return LIB
 
 

@@ -46,6 +46,7 @@ typedef CUresult (*encode_tiled_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32
 struct DeviceState {
   int device = -1;
   int sm_count = 0;
+  int l2_bytes = 0;
   bool ok = false;
 };
 
@@ -66,6 +67,9 @@ pstgf_status_t device_state(DeviceState &ds) {
   PSTGF_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
   PSTGF_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   if (major != 10) return PSTGF_ERR_UNSUPPORTED_DEVICE;
+  int l2 = 0;
+  PSTGF_CUDA(cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev));
+  ds.l2_bytes = l2;
   std::call_once(g_encode_once, [] {
     void *fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
@@ -78,9 +82,9 @@ pstgf_status_t device_state(DeviceState &ds) {
     std::lock_guard<std::mutex> lock(g_attr_mutex);
     if (dev < 64 && !g_attr_set[dev]) {
       PSTGF_CUDA(cudaFuncSetAttribute(pstgf::rmat_persistent_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      pstgf::SMEM_BYTES));
+                                      pstgf::SMEM_MAX_OPTIN));
       PSTGF_CUDA(cudaFuncSetAttribute(pstgf::rmat_persistent_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      pstgf::SMEM_BYTES));
+                                      pstgf::SMEM_MAX_OPTIN));
       g_attr_set[dev] = true;
     }
   }
@@ -101,20 +105,28 @@ pstgf_status_t check_wave(const pstgf_wave_t &w) {
   if (w.w_layout != PSTGF_W_POLE_CONTIGUOUS && w.w_layout != PSTGF_W_CHANNEL_CONTIGUOUS) return PSTGF_ERR_INVALID_VALUE;
   const long long ld_min = w.w_layout == PSTGF_W_CHANNEL_CONTIGUOUS ? w.n_chan : w.n_poles;
   if (w.n_poles > 0 && (!w.W || !w.E_k || w.ldw < ld_min)) return PSTGF_ERR_INVALID_VALUE;
-  if (!aligned8(w.W) || !aligned8(w.E_k) || !aligned8(w.energies) || !aligned8(w.R_out)) return PSTGF_ERR_ALIGNMENT;
+  if (!aligned8(w.W) || !aligned8(w.E_k) || !aligned8(w.energies) || !aligned8(w.R_out) || !aligned8(w.diag_add))
+    return PSTGF_ERR_ALIGNMENT;
   return PSTGF_OK;
 }
 
 // ---- planner -------------------------------------------------------------------------------
-std::atomic<int> g_tail_policy{PSTGF_TAIL_AUTO};
+// Knobs for tests and measurements (pstgf_debug_*): thread-local, they affect the calling thread's calls only.
+thread_local int tl_tail_policy = PSTGF_TAIL_AUTO;
+thread_local int tl_slab_policy = PSTGF_SLAB_AUTO;
+thread_local int tl_host_pipeline = PSTGF_HOST_PIPELINE_AUTO;
+thread_local unsigned int tl_upload_timeout_ms = 0;   // 0 = the kernel's default (2 s)
+thread_local int tl_stall_upload = 0;
 
-// Fills everything of DevWave except the tensor map; every energy block starts out coarse.
-void plan_wave(const pstgf_wave_t &w, DevWave &d) {
+// Fills everything of DevWave except the tensor map, the slab section and the tail; every energy block starts out
+// coarse and a remainder of n_E mod 8 energies starts out as a partial classic block.
+void plan_wave(const pstgf_wave_t &w, DevWave &d, int l2_bytes) {
   std::memset(&d, 0, sizeof(d));
   d.W = w.W;
   d.E_k = w.E_k;
   d.energies = w.energies;
   d.R_out = w.R_out;
+  d.diag_add = w.diag_add;
   d.ldw = w.ldw;
   d.inv2a = 1.0 / (2.0 * w.a);
   d.n_chan = w.n_chan;
@@ -126,13 +138,20 @@ void plan_wave(const pstgf_wave_t &w, DevWave &d) {
   d.n_eb = (w.n_E + pstgf::EB - 1) / pstgf::EB;
   d.n_tiles = pstgf::coarse_tiles(w.n_chan);
   d.n_eb_coarse = d.n_eb;
+  d.slab_e0 = w.n_E;
+  d.slab_T = 64;
+  d.slab_nt = (w.n_chan + 63) / 64;
   d.tr = w.w_layout == PSTGF_W_CHANNEL_CONTIGUOUS ? 1 : 0;
   d.use_tma = ((reinterpret_cast<uintptr_t>(w.W) & 15u) == 0 && (w.ldw % 2) == 0 && w.ldw * 8 < (1LL << 40)) ? 1 : 0;
+  // a W of at most half the L2 is loaded with the evict_last policy: R's streaming stores then do not push it out
+  const double w_bytes = 8.0 * (double)w.ldw * (double)(d.tr ? w.n_poles : w.n_chan);
+  d.l2_keep = (l2_bytes > 0 && w_bytes <= 0.5 * (double)l2_bytes) ? 1 : 0;
 }
 
 long long coarse_items(const DevWave &d) { return (long long)d.n_tiles * d.n_eb_coarse; }
+long long slab_items(const DevWave &d) { return (long long)pstgf::slab_tiles(d.slab_nt) * (d.slab_g2 + d.slab_g1); }
 long long fine_items(const DevWave &d) { return (long long)pstgf::fine_tiles(d.n_j) * (d.n_eb - d.n_eb_coarse); }
-long long wave_items(const DevWave &d) { return coarse_items(d) + fine_items(d); }
+long long wave_items(const DevWave &d) { return coarse_items(d) + slab_items(d) + fine_items(d); }
 
 // Relative cost of a wave's items, for the largest-first order of the batch.
 double wave_item_cost(const pstgf_wave_t &w) { return (double)std::min(w.n_chan, pstgf::TM) * w.n_poles; }
@@ -144,6 +163,111 @@ double largest_item_cost(const DevWave &d) {
 }
 double cost_per_energy_block(const DevWave &d) {
   return (double)d.n_kt * ((double)d.n_i * pstgf::COST_DIAG + (double)(d.n_tiles - d.n_i) * pstgf::COST_OFF);
+}
+
+// Makespan of greedy list scheduling (what the atomic counter does) of runs of equal items on `grid` CTAs.
+double simulate_makespan(const std::vector<std::pair<double, int>> &runs, int grid) {
+  std::priority_queue<double, std::vector<double>, std::greater<double>> free_at;
+  for (int b = 0; b < grid; ++b) free_at.push(0.0);
+  double last = 0.0;
+  for (const auto &r : runs)
+    for (int n = 0; n < r.second; ++n) {
+      const double f = free_at.top() + r.first;
+      free_at.pop();
+      free_at.push(f);
+      last = std::max(last, f);
+    }
+  return last;
+}
+
+// ---- slab section: the energies that do not fill a block of 8 ------------------------------------
+// An item's time is set by its busiest warp: blocks per warp and k-step (SlabShape: nr x ncw), times a factor for
+// the quality of the warp's inner loop (fewer DMMAs per fragment load and per scaling multiply in the small
+// shapes; fitted to the B200 sweeps of bench.py --n-E), plus a fixed cost per item (epilogue, ring refill) in
+// units of k-tiles.
+double slab_item_cost(int T, int g, int n_kt) {
+  const pstgf::SlabShape sh = pstgf::slab_shape(T, g);
+  const int blocks = sh.nr * sh.ncw;
+  const double quality = blocks >= 32 ? 1.0 : blocks >= 16 ? 1.03 : blocks >= 8 ? 1.08 : blocks >= 4 ? 1.25 : 1.5;
+  return blocks * quality * ((double)n_kt + 3.0);
+}
+
+std::mutex g_slab_mutex;
+std::map<std::tuple<int, int, int, int>, int> g_slab_cache;   // (n_chan, remainder, n_kt bucket, grid) -> T
+
+// Tile edge of a wave's slab items: the candidate with the smallest simulated makespan of the slab items alone.
+// Large tiles have the better inner loop and the smaller L2 traffic, small tiles give the grid enough items.
+int best_slab_edge(int n_chan, int r, int n_kt, int grid) {
+  const auto key = std::make_tuple(n_chan, r, std::min(n_kt, 64), grid);
+  {
+    std::lock_guard<std::mutex> lock(g_slab_mutex);
+    auto it = g_slab_cache.find(key);
+    if (it != g_slab_cache.end()) return it->second;
+  }
+  int best_T = 32;
+  double best = 0.0;
+  std::vector<std::pair<double, int>> runs;
+  for (int T : {128, 64, 32}) {
+    const int nt = (n_chan + T - 1) / T;
+    const long long tiles = pstgf::slab_tiles(nt);
+    const int g2 = T == 128 ? 0 : r / 2, g1 = T == 128 ? r : r % 2;
+    double m;
+    if (tiles * (g2 + g1) > 16LL * grid) {
+      // plenty of items: the makespan is the work divided by the grid, no need to simulate
+      m = (double)tiles * (g2 * slab_item_cost(T, 2, n_kt) + g1 * slab_item_cost(T, 1, n_kt)) / grid;
+    } else {
+      runs.clear();
+      // group-fastest order inside a tile; all tiles cost the same in this model (edge tiles are cheaper in fact)
+      if (g2 > 0 && g1 > 0) {
+        for (long long t = 0; t < tiles; ++t) {
+          runs.emplace_back(slab_item_cost(T, 2, n_kt), g2);
+          runs.emplace_back(slab_item_cost(T, 1, n_kt), g1);
+        }
+      } else {
+        runs.emplace_back(slab_item_cost(T, g2 > 0 ? 2 : 1, n_kt), (int)(tiles * (g2 + g1)));
+      }
+      m = simulate_makespan(runs, grid);
+    }
+    if (best == 0.0 || m < best * (1.0 - 1e-9)) {
+      best = m;
+      best_T = T;
+    }
+  }
+  std::lock_guard<std::mutex> lock(g_slab_mutex);
+  g_slab_cache[key] = best_T;
+  return best_T;
+}
+
+void plan_slabs(std::vector<DevWave> &ds, int grid) {
+  const int policy = tl_slab_policy;
+  if (policy == PSTGF_SLAB_NONE) return;
+  for (DevWave &d : ds) {
+    const int r = d.n_E % pstgf::EB;
+    if (r == 0) continue;
+    int T = policy == PSTGF_SLAB_T32 ? 32 : policy == PSTGF_SLAB_T64 ? 64 : policy == PSTGF_SLAB_T128 ? 128
+                                                                           : best_slab_edge(d.n_chan, r, d.n_kt, grid);
+    d.n_eb = d.n_E / pstgf::EB;
+    d.n_eb_coarse = d.n_eb;
+    d.slab_e0 = d.n_eb * pstgf::EB;
+    d.slab_T = T;
+    d.slab_nt = (d.n_chan + T - 1) / T;
+    d.slab_g2 = T == 128 ? 0 : r / 2;       // tiles of edge 128 take one energy at a time (8 warps x 16 x 2 blocks)
+    d.slab_g1 = T == 128 ? r : r % 2;
+  }
+}
+
+// Ring geometry of a launch: the classic stage (5 panels of 32 channels) unless a wave has slab tiles of edge 128
+// (8 panels); as many stages as fit, at most MAX_STAGES.
+pstgf::RingGeo ring_geometry(const std::vector<DevWave> &ds) {
+  int bytes = 0;
+  for (const DevWave &d : ds) {
+    const bool big = slab_items(d) > 0 && d.slab_T == 128;
+    bytes = std::max(bytes, pstgf::stage_bytes_for(d.tr != 0, big ? pstgf::BIG_PANELS : pstgf::CLASSIC_PANELS));
+  }
+  pstgf::RingGeo g;
+  g.stage_bytes = bytes;
+  g.n_stages = std::min(pstgf::MAX_STAGES, (pstgf::SMEM_MAX_OPTIN - pstgf::SMEM_RING_OFFSET - pstgf::SMEM_ALIGN_SLACK) / bytes);
+  return g;
 }
 
 // ---- tail size of a single wave by simulation ------------------------------------------------------
@@ -178,21 +302,6 @@ void item_costs(const DevWave &d, int t, std::vector<std::pair<double, int>> &ru
       runs.emplace_back(BLK_DIAG32 * nb * (nb + 1) / 2, t);
     }
   }
-}
-
-// Makespan of greedy list scheduling (what the atomic counter does) of those items on `grid` CTAs.
-double simulate_makespan(const std::vector<std::pair<double, int>> &runs, int grid) {
-  std::priority_queue<double, std::vector<double>, std::greater<double>> free_at;
-  for (int b = 0; b < grid; ++b) free_at.push(0.0);
-  double last = 0.0;
-  for (const auto &r : runs)
-    for (int n = 0; n < r.second; ++n) {
-      const double f = free_at.top() + r.first;
-      free_at.pop();
-      free_at.push(f);
-      last = std::max(last, f);
-    }
-  return last;
 }
 
 std::mutex g_tail_mutex;
@@ -233,16 +342,18 @@ int best_tail_single_wave(const DevWave &d, int grid, double budget) {
 // Tail of the schedule (see rmat_common.h): about one round of the grid's worth of work, taken from the
 // END of the largest-first order, is cut into fine tiles so that list scheduling finishes on small items.
 void plan_tails(std::vector<DevWave> &ds, int grid) {
-  const int policy = g_tail_policy.load();
+  const int policy = tl_tail_policy;
   if (policy == PSTGF_TAIL_NONE) return;
   if (policy == PSTGF_TAIL_ALL) {
     for (DevWave &d : ds) d.n_eb_coarse = 0;
     return;
   }
   double c_max = 0.0;
-  for (const DevWave &d : ds) c_max = std::max(c_max, largest_item_cost(d));
+  for (const DevWave &d : ds)
+    if (d.n_eb > 0) c_max = std::max(c_max, largest_item_cost(d));
   double budget = c_max * grid;
   if (ds.size() == 1) {
+    if (ds[0].n_eb == 0) return;
     const int t = best_tail_single_wave(ds[0], grid, c_max * grid);
     if (t >= 0) {
       ds[0].n_eb_coarse = ds[0].n_eb - t;
@@ -251,6 +362,7 @@ void plan_tails(std::vector<DevWave> &ds, int grid) {
   }
   for (size_t q = ds.size(); q-- > 0 && budget > 0.0;) {
     DevWave &d = ds[q];
+    if (d.n_eb == 0) continue;
     const double per_eb = cost_per_energy_block(d);
     if (largest_item_cost(d) <= 0.45 * c_max) {   // a small wave at the end of the list: its coarse items are fine enough
       budget -= d.n_eb * per_eb;
@@ -291,24 +403,40 @@ pstgf_status_t encode_map(DevWave &d) {
 // A wave with work for the contraction kernel (n_poles == 0 is a zero-fill instead).
 bool wave_has_items(const pstgf_wave_t &w) { return w.n_chan > 0 && w.n_E > 0 && w.n_poles > 0; }
 
+// n_poles == 0: the sum of eq. 4 is empty, R is the diagonal addend alone (zero without one).
+__global__ void diag_only_kernel(const double *__restrict__ diag_add, int n_chan, long long n, double *__restrict__ R_out) {
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;      // over [n_E][n_chan]
+  if (idx >= n) return;
+  const long long e = idx / n_chan;
+  const int c = (int)(idx - e * n_chan);
+  R_out[(size_t)e * n_chan * n_chan + (size_t)c * n_chan + c] = diag_add[idx];
+}
+
 pstgf_status_t zero_fill(const pstgf_wave_t &w, cudaStream_t s) {
   if (w.n_chan > 0 && w.n_E > 0 && w.n_poles == 0) {
     PSTGF_CUDA(cudaMemsetAsync(w.R_out, 0, sizeof(double) * (size_t)w.n_E * w.n_chan * w.n_chan, s));
     ++tl_launches;
+    if (w.diag_add) {
+      const long long n = (long long)w.n_E * w.n_chan;
+      diag_only_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(w.diag_add, w.n_chan, n, w.R_out);
+      PSTGF_CUDA(cudaGetLastError());
+      ++tl_launches;
+    }
   }
   return PSTGF_OK;
 }
 
 // workspace layout of the batch call
 constexpr size_t WS_COUNTER_BYTES = 256;
-size_t ws_item_begin_bytes(int n_waves) { return ((2 * (size_t)n_waves + 1) * sizeof(long long) + 255) & ~(size_t)255; }
+size_t ws_item_begin_bytes(int n_waves) { return ((3 * (size_t)n_waves + 1) * sizeof(long long) + 255) & ~(size_t)255; }
 size_t ws_bytes(int n_waves) { return WS_COUNTER_BYTES + ws_item_begin_bytes(n_waves) + (size_t)n_waves * sizeof(DevWave); }
 
 // ---- work counters of the single-wave call ---------------------------------------------------
 // pstgf_rmat_form has no workspace argument, so its atomic work counter comes from a small pool the library
-// keeps per device (COUNTER_SLOTS x 128 B, allocated at first use).  A slot is handed to one launch at a time:
-// an event recorded behind the launch tells when it is free again (the kernel's last CTA zeroes it).  With no
-// free slot, or under stream capture, the launch falls back to round-robin item assignment.
+// keeps per device (COUNTER_SLOTS x 128 B, allocated at first use, freed by pstgf_rmat_finalize).  A slot is
+// handed to one launch at a time: an event recorded behind the launch tells when it is free again (the kernel's
+// last CTA zeroes it).  With no free slot, or under stream capture, the launch falls back to round-robin item
+// assignment.
 constexpr int COUNTER_SLOTS = 64;
 struct CounterPool {
   unsigned long long *base = nullptr;
@@ -319,14 +447,19 @@ struct CounterPool {
 std::mutex g_counter_mutex;
 CounterPool g_counters[64];
 
+bool stream_is_capturing(cudaStream_t s) {
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(s, &cap) != cudaSuccess) {
+    (void)cudaGetLastError();
+    return true;      // cannot tell: treat as capturing (the safe side)
+  }
+  return cap != cudaStreamCaptureStatusNone;
+}
+
 // Called with g_counter_mutex held.  Returns the slot or -1.
 int acquire_counter(int dev, cudaStream_t s, unsigned long long **out) {
   if (dev < 0 || dev >= 64) return -1;
-  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
-  if (cudaStreamIsCapturing(s, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone) {
-    (void)cudaGetLastError();
-    return -1;
-  }
+  if (stream_is_capturing(s)) return -1;
   CounterPool &cp = g_counters[dev];
   if (!cp.base) {
     void *p = nullptr;
@@ -365,9 +498,15 @@ int acquire_counter(int dev, cudaStream_t s, unsigned long long **out) {
 
 extern "C" {
 
-pstgf_status_t pstgf_rmat_set_tail_policy(int policy) {
+pstgf_status_t pstgf_debug_set_tail_policy(int policy) {
   if (policy != PSTGF_TAIL_AUTO && policy != PSTGF_TAIL_NONE && policy != PSTGF_TAIL_ALL) return PSTGF_ERR_INVALID_VALUE;
-  g_tail_policy.store(policy);
+  tl_tail_policy = policy;
+  return PSTGF_OK;
+}
+
+pstgf_status_t pstgf_debug_set_slab_policy(int policy) {
+  if (policy < PSTGF_SLAB_AUTO || policy > PSTGF_SLAB_T128) return PSTGF_ERR_INVALID_VALUE;
+  tl_slab_policy = policy;
   return PSTGF_OK;
 }
 
@@ -383,18 +522,20 @@ static pstgf_status_t form_single(const pstgf_wave_t &w, void *stream) {
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   if (n_poles == 0) return zero_fill(w, s);
   std::vector<DevWave> d(1);
-  plan_wave(w, d[0]);
+  plan_wave(w, d[0], ds.l2_bytes);
+  plan_slabs(d, ds.sm_count);
   plan_tails(d, ds.sm_count);
   st = encode_map(d[0]);
   if (st != PSTGF_OK) return st;
   const long long n_items = wave_items(d[0]);
   const int grid = (int)std::min<long long>(ds.sm_count, n_items);
+  const pstgf::RingGeo geo = ring_geometry(d);
   {
     std::lock_guard<std::mutex> lock(g_counter_mutex);
     unsigned long long *counter = nullptr;
     const int slot = acquire_counter(ds.device, s, &counter);
-    pstgf::rmat_persistent_kernel<false><<<grid, pstgf::NUM_THREADS, pstgf::SMEM_BYTES, s>>>(d[0], nullptr, nullptr, 1,
-                                                                                           n_items, counter);
+    pstgf::rmat_persistent_kernel<false><<<grid, pstgf::NUM_THREADS, pstgf::smem_bytes_for(geo), s>>>(
+        d[0], nullptr, nullptr, 1, n_items, counter, geo);
     PSTGF_CUDA(cudaGetLastError());
     if (slot >= 0) {
       CounterPool &cp = g_counters[ds.device];
@@ -408,13 +549,13 @@ static pstgf_status_t form_single(const pstgf_wave_t &w, void *stream) {
 
 pstgf_status_t pstgf_rmat_form(const double *W, long long ldw, const double *E_k, const double *energies, int n_chan,
                                int n_poles, int n_E, double a, double *R_out, void *stream) {
-  pstgf_wave_t w{n_chan, n_poles, n_E, PSTGF_W_POLE_CONTIGUOUS, ldw, a, W, E_k, energies, R_out};
+  pstgf_wave_t w{n_chan, n_poles, n_E, PSTGF_W_POLE_CONTIGUOUS, ldw, a, W, E_k, energies, R_out, nullptr};
   return form_single(w, stream);
 }
 
 pstgf_status_t pstgf_rmat_form_hdat(const double *Wt, long long ldw, const double *E_k, const double *energies,
                                     int n_chan, int n_poles, int n_E, double a, double *R_out, void *stream) {
-  pstgf_wave_t w{n_chan, n_poles, n_E, PSTGF_W_CHANNEL_CONTIGUOUS, ldw, a, Wt, E_k, energies, R_out};
+  pstgf_wave_t w{n_chan, n_poles, n_E, PSTGF_W_CHANNEL_CONTIGUOUS, ldw, a, Wt, E_k, energies, R_out, nullptr};
   return form_single(w, stream);
 }
 
@@ -429,6 +570,7 @@ struct BatchCompletion {
   unsigned int *const *flag = nullptr;   // in: per input wave, a zeroed host-mapped word (device-visible address)
   const unsigned int *const *rows_ready = nullptr;   // in, optional: per input wave, the upload counter of its W
   const int *ready_counts_channels = nullptr;        // ... and what it counts (DevWave::ready_counts_channels)
+  unsigned int *abort_flag = nullptr;                // in: host-mapped word a load warp sets when an upload wait times out
   std::vector<int> order;                // out: input wave indices in the order the launch completes them
   std::vector<long long> items;          // out: items of each input wave (arrivals = items * EB)
 };
@@ -449,6 +591,9 @@ static pstgf_status_t form_batch_impl(const pstgf_wave_t *waves, int n_waves, vo
   pstgf_status_t st = device_state(dstate);
   if (st != PSTGF_OK) return st;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
+  // the tables go to the workspace by a copy from this call's own host memory: a captured graph would replay a
+  // copy from memory that is long gone, so the batch call refuses to be captured
+  if (stream_is_capturing(s)) return PSTGF_ERR_CAPTURE;
   int launches = 0;
   // waves with work, most expensive items first (largest-first list scheduling)
   std::vector<int> order;
@@ -464,15 +609,16 @@ static pstgf_status_t form_batch_impl(const pstgf_wave_t *waves, int n_waves, vo
   std::stable_sort(order.begin(), order.end(),
                    [&](int x, int y) { return wave_item_cost(waves[x]) > wave_item_cost(waves[y]); });
   const int nw = (int)order.size();
-  // host image of the workspace: [counter | item_begin[2 nw + 1] | DevWave[nw]]; item sections are the coarse
-  // items of every wave (largest first), then the fine items of every wave
+  // host image of the workspace: [counter | item_begin[3 nw + 1] | DevWave[nw]]; item sections are the coarse
+  // items of every wave (largest first), then the slab items of every wave, then the fine items of every wave
   const size_t off_begin = WS_COUNTER_BYTES, off_waves = WS_COUNTER_BYTES + ws_item_begin_bytes(n_waves);
   std::vector<unsigned char> img(off_waves + (size_t)nw * sizeof(DevWave), 0);
   long long *item_begin = reinterpret_cast<long long *>(img.data() + off_begin);
   std::vector<DevWave> ds((size_t)nw);
   for (int q = 0; q < nw; ++q) {
-    plan_wave(waves[order[q]], ds[q]);
+    plan_wave(waves[order[q]], ds[q], dstate.l2_bytes);
   }
+  plan_slabs(ds, dstate.sm_count);
   plan_tails(ds, dstate.sm_count);
   if (completion && completion->done)
     for (int q = 0; q < nw; ++q) {
@@ -482,15 +628,19 @@ static pstgf_status_t form_batch_impl(const pstgf_wave_t *waves, int n_waves, vo
       if (completion->rows_ready) {
         ds[q].rows_ready = completion->rows_ready[order[q]];
         ds[q].ready_counts_channels = completion->ready_counts_channels[order[q]];
+        ds[q].abort_flag = completion->abort_flag;
+        ds[q].wait_timeout_ms = tl_upload_timeout_ms;
       }
     }
   if (completion) {
-    // all coarse items come before all fine items: waves with a fine tail finish last
+    // coarse items, then slab items, then fine items: a wave is complete when its last section is
     completion->items.assign((size_t)n_waves, 0);
     completion->order.clear();
-    for (int pass = 0; pass < 2; ++pass)
-      for (int q = 0; q < nw; ++q)
-        if ((ds[q].n_eb_coarse < ds[q].n_eb) == (pass == 1)) completion->order.push_back(order[q]);
+    for (int pass = 0; pass < 3; ++pass)
+      for (int q = 0; q < nw; ++q) {
+        const int last = fine_items(ds[q]) > 0 ? 2 : slab_items(ds[q]) > 0 ? 1 : 0;
+        if (last == pass) completion->order.push_back(order[q]);
+      }
     for (int q = 0; q < nw; ++q) completion->items[(size_t)order[q]] = wave_items(ds[q]);
   }
   long long total = 0;
@@ -503,17 +653,22 @@ static pstgf_status_t form_batch_impl(const pstgf_wave_t *waves, int n_waves, vo
   }
   for (int q = 0; q < nw; ++q) {
     item_begin[nw + q] = total;
+    total += slab_items(ds[q]);
+  }
+  for (int q = 0; q < nw; ++q) {
+    item_begin[2 * nw + q] = total;
     total += fine_items(ds[q]);
   }
-  item_begin[2 * nw] = total;
+  item_begin[3 * nw] = total;
   unsigned char *ws = static_cast<unsigned char *>(workspace);
   PSTGF_CUDA(cudaMemcpyAsync(ws, img.data(), img.size(), cudaMemcpyHostToDevice, s));
   const int grid = (int)std::min<long long>(dstate.sm_count, total);
+  const pstgf::RingGeo geo = ring_geometry(ds);
   DevWave dummy;
   std::memset(&dummy, 0, sizeof(dummy));
-  pstgf::rmat_persistent_kernel<true><<<grid, pstgf::NUM_THREADS, pstgf::SMEM_BYTES, s>>>(
+  pstgf::rmat_persistent_kernel<true><<<grid, pstgf::NUM_THREADS, pstgf::smem_bytes_for(geo), s>>>(
       dummy, reinterpret_cast<const DevWave *>(ws + off_waves), reinterpret_cast<const long long *>(ws + off_begin), nw,
-      total, reinterpret_cast<unsigned long long *>(ws));
+      total, reinterpret_cast<unsigned long long *>(ws), geo);
   PSTGF_CUDA(cudaGetLastError());
   tl_launches = launches + 1;
   return PSTGF_OK;
@@ -524,26 +679,35 @@ pstgf_status_t pstgf_rmat_form_batch(const pstgf_wave_t *waves, int n_waves, voi
   return form_batch_impl(waves, n_waves, workspace, workspace_bytes, stream, nullptr);
 }
 
-pstgf_status_t pstgf_rmat_form_naive(const double *W, long long ldw, const double *E_k, const double *energies,
-                                     int n_chan, int n_poles, int n_E, double a, double *R_out, int w_layout,
-                                     void *stream) {
+pstgf_status_t pstgf_rmat_form_naive(const pstgf_wave_t *wave, void *stream) {
   tl_launches = 0;
-  pstgf_wave_t w{n_chan, n_poles, n_E, w_layout, ldw, a, W, E_k, energies, R_out};
+  if (!wave) return PSTGF_ERR_INVALID_VALUE;
+  const pstgf_wave_t &w = *wave;
   pstgf_status_t st = check_wave(w);
   if (st != PSTGF_OK) return st;
-  if (n_chan == 0 || n_E == 0) return PSTGF_OK;
+  if (w.n_chan == 0 || w.n_E == 0) return PSTGF_OK;
   DeviceState ds;
   st = device_state(ds);
   if (st != PSTGF_OK) return st;
-  const long long n_elems = (long long)n_E * n_chan * n_chan;
+  const long long n_elems = (long long)w.n_E * w.n_chan * w.n_chan;
   const int threads = 128;
   const long long blocks = (n_elems + threads - 1) / threads;
   if (blocks > 0x7fffffffLL) return PSTGF_ERR_INVALID_VALUE;
+  const bool tr = w.w_layout == PSTGF_W_CHANNEL_CONTIGUOUS;
   pstgf::rmat_naive_kernel<<<(unsigned)blocks, threads, 0, static_cast<cudaStream_t>(stream)>>>(
-      W, w_layout == PSTGF_W_CHANNEL_CONTIGUOUS ? 1LL : ldw, w_layout == PSTGF_W_CHANNEL_CONTIGUOUS ? ldw : 1LL, E_k, energies,
-      n_chan, n_poles, n_elems, a, R_out);
+      w.W, tr ? 1LL : w.ldw, tr ? w.ldw : 1LL, w.E_k, w.energies, w.n_chan, w.n_poles, n_elems, w.a, w.diag_add, w.R_out);
   PSTGF_CUDA(cudaGetLastError());
   tl_launches = 1;
+  return PSTGF_OK;
+}
+
+/* the mesh of the namelists is in z-scaled Rydberg, E/z^2; eq. 4 wants E on the scale of the poles. */
+pstgf_status_t pstgf_mesh_from_zscaled(const double *e_scaled, long long n, double z, double *e_out) {
+  if (n < 0 || !std::isfinite(z) || !(z > 0.0)) return PSTGF_ERR_INVALID_VALUE;
+  if (n == 0) return PSTGF_OK;
+  if (!e_scaled || !e_out) return PSTGF_ERR_INVALID_VALUE;
+  const double z2 = z * z;
+  for (long long i = 0; i < n; ++i) e_out[i] = e_scaled[i] * z2;
   return PSTGF_OK;
 }
 
@@ -552,9 +716,9 @@ namespace {
 constexpr int HOST_RING = 3;          // R staging buffers in flight
 constexpr int HOST_COMPUTE_STREAMS = 2;
 
-// Device memory of the host call comes from a pool the library owns (one per device, kept for the life of
-// the process, release threshold = never): the default pool hands its memory back at every synchronise,
-// and re-growing it costs tens of milliseconds per call.
+// Device memory of the host call comes from a pool the library owns (one per device, release threshold =
+// never, freed by pstgf_rmat_finalize): the default pool hands its memory back at every synchronise, and
+// re-growing it costs tens of milliseconds per call.
 std::mutex g_pool_mutex;
 cudaMemPool_t g_pool[64] = {nullptr};
 
@@ -581,50 +745,65 @@ cudaError_t host_call_pool(int dev, cudaMemPool_t *out) {
 }
 
 constexpr size_t MAX_CHUNK_SEGMENTS = 4096;
-std::atomic<int> g_host_pipeline{PSTGF_HOST_PIPELINE_AUTO};
 
 // Completion state of the signalled pipeline, per device and host thread, allocated at the thread's first host
-// call and kept: 2 x MAX_CHUNK_SEGMENTS device counters and as many flag words in mapped pinned host memory.
+// call: 2 x MAX_CHUNK_SEGMENTS device counters and as many flag words in mapped pinned host memory, plus one
+// abort word.  The blocks are owned by a registry so that pstgf_rmat_finalize can free them whatever thread made
+// them; a thread notices through the generation number that its cached block is gone.
 constexpr size_t MAX_UPLOAD_WAVES = 1024, MAX_UPLOAD_SLABS = 16;
 struct HostFlags {
   unsigned int *counters = nullptr;            // device
   volatile unsigned int *flags_host = nullptr; // host view
-  unsigned int *flags_dev = nullptr;           // device view of the same words
+  unsigned int *flags_dev = nullptr;           // device view of the same words; word [2 MAX_CHUNK_SEGMENTS] is the abort flag
   unsigned int *upload_counters = nullptr;     // device: rows of each wave's W uploaded so far
   unsigned int *upload_values = nullptr;       // pinned host: the values the upload stream copies into them
+  int device = -1;
 };
+std::mutex g_flags_mutex;
+std::vector<HostFlags *> g_flags_registry;
+std::atomic<unsigned long long> g_flags_generation{1};
+
+void free_host_flags(HostFlags *f) {
+  if (f->counters) cudaFree(f->counters);
+  if (f->flags_host) cudaFreeHost(const_cast<unsigned int *>(f->flags_host));
+  if (f->upload_counters) cudaFree(f->upload_counters);
+  if (f->upload_values) cudaFreeHost(f->upload_values);
+  delete f;
+}
+
 cudaError_t host_call_flags(int dev, HostFlags *out) {
-  static thread_local HostFlags cache[64];
+  static thread_local HostFlags *cache[64] = {nullptr};
+  static thread_local unsigned long long cache_generation = 0;
   if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
-  HostFlags &f = cache[dev];
-  if (!f.counters) {
-    void *c = nullptr, *h = nullptr, *d = nullptr;
-    const size_t bytes = 2 * MAX_CHUNK_SEGMENTS * sizeof(unsigned int);
-    cudaError_t e = cudaMalloc(&c, bytes);
-    if (e != cudaSuccess) return e;
-    e = cudaHostAlloc(&h, bytes, cudaHostAllocMapped);
-    if (e == cudaSuccess) e = cudaHostGetDevicePointer(&d, h, 0);
-    if (e != cudaSuccess) {
-      cudaFree(c);
-      if (h) cudaFreeHost(h);
-      return e;
-    }
-    void *uc = nullptr, *uv = nullptr;
-    e = cudaMalloc(&uc, MAX_UPLOAD_WAVES * sizeof(unsigned int));
-    if (e == cudaSuccess) e = cudaHostAlloc(&uv, MAX_UPLOAD_WAVES * (MAX_UPLOAD_SLABS + 1) * sizeof(unsigned int), cudaHostAllocDefault);
-    if (e != cudaSuccess) {
-      cudaFree(c);
-      cudaFreeHost(h);
-      if (uc) cudaFree(uc);
-      return e;
-    }
-    f.counters = static_cast<unsigned int *>(c);
-    f.flags_host = static_cast<volatile unsigned int *>(h);
-    f.flags_dev = static_cast<unsigned int *>(d);
-    f.upload_counters = static_cast<unsigned int *>(uc);
-    f.upload_values = static_cast<unsigned int *>(uv);
+  const unsigned long long gen = g_flags_generation.load();
+  if (cache_generation != gen) {
+    for (HostFlags *&c : cache) c = nullptr;      // freed by pstgf_rmat_finalize
+    cache_generation = gen;
   }
-  *out = f;
+  if (!cache[dev]) {
+    HostFlags *f = new HostFlags;
+    f->device = dev;
+    void *c = nullptr, *h = nullptr, *d = nullptr, *uc = nullptr, *uv = nullptr;
+    const size_t bytes = (2 * MAX_CHUNK_SEGMENTS + 1) * sizeof(unsigned int);
+    cudaError_t e = cudaMalloc(&c, bytes);
+    if (e == cudaSuccess) e = cudaHostAlloc(&h, bytes, cudaHostAllocMapped);
+    if (e == cudaSuccess) e = cudaHostGetDevicePointer(&d, h, 0);
+    if (e == cudaSuccess) e = cudaMalloc(&uc, MAX_UPLOAD_WAVES * sizeof(unsigned int));
+    if (e == cudaSuccess) e = cudaHostAlloc(&uv, MAX_UPLOAD_WAVES * (MAX_UPLOAD_SLABS + 1) * sizeof(unsigned int), cudaHostAllocDefault);
+    f->counters = static_cast<unsigned int *>(c);
+    f->flags_host = static_cast<volatile unsigned int *>(h);
+    f->flags_dev = static_cast<unsigned int *>(d);
+    f->upload_counters = static_cast<unsigned int *>(uc);
+    f->upload_values = static_cast<unsigned int *>(uv);
+    if (e != cudaSuccess) {
+      free_host_flags(f);
+      return e;
+    }
+    std::lock_guard<std::mutex> lock(g_flags_mutex);
+    g_flags_registry.push_back(f);
+    cache[dev] = f;
+  }
+  *out = *cache[dev];
   return cudaSuccess;
 }
 
@@ -664,12 +843,13 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
   DeviceState ds;
   pstgf_status_t st = device_state(ds);
   if (st != PSTGF_OK) return st;
+  if (stream_is_capturing(static_cast<cudaStream_t>(stream))) return PSTGF_ERR_CAPTURE;   // the call synchronises
   // Pipeline choice: the signalled single launch, unless the knob asks for one launch per piece or the whole
   // job is a matter of a millisecond or two (then the naps of the flag polling cost more than launches do).
   double est_flop = 0.0;
   for (int p = 0; p < n_waves; ++p)
     if (wave_has_items(waves[p])) est_flop += (double)waves[p].n_E * waves[p].n_chan * (double)waves[p].n_chan * waves[p].n_poles;
-  const bool signalled = g_host_pipeline.load() == PSTGF_HOST_PIPELINE_AUTO && est_flop / 33e12 >= 2e-3;
+  const bool signalled = tl_host_pipeline == PSTGF_HOST_PIPELINE_AUTO && est_flop / 33e12 >= 2e-3;
   // copy-back granularity (a piece): 1/32 of R in [8, 64] MiB when pieces are free (signalled), 1/8 of R in
   // [16, 256] MiB when each piece is a launch
   size_t cap = max_chunk_bytes;
@@ -692,12 +872,14 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
     if (e == cudaSuccess) res.allocs.push_back(*out);
     return e;
   };
-  // inputs, first part: allocations and the small arrays (poles, energies).  W follows further down: in the
-  // signalled pipeline it is uploaded in slabs of poles WHILE the launch runs, each slab followed by an update of
-  // the wave's upload counter that the kernel's load warp waits on stage by stage.
+  // inputs, first part: allocations and the small arrays (poles, energies, diagonal addends).  W follows further
+  // down: in the signalled pipeline it is uploaded in slabs of poles WHILE the launch runs, each slab followed by an
+  // update of the wave's upload counter that the kernel's load warp waits on stage by stage.
   HostFlags flags;
   if (signalled) PSTGF_CUDA(host_call_flags(ds.device, &flags));
   const bool overlap_upload = signalled && (size_t)n_waves <= MAX_UPLOAD_WAVES;
+  volatile unsigned int *abort_host = signalled ? flags.flags_host + 2 * MAX_CHUNK_SEGMENTS : nullptr;
+  if (signalled) *abort_host = 0u;
   if (overlap_upload) PSTGF_CUDA(cudaMemsetAsync(flags.upload_counters, 0, sizeof(unsigned int) * (size_t)n_waves, res.s));
   std::vector<pstgf_wave_t> dev(waves, waves + n_waves);
   // poles [k0, k1) of all channels, or (by_channels, pole-contiguous W only) channels [k0, k1) with all their poles
@@ -716,7 +898,11 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
     const pstgf_wave_t &w = waves[p];
     if (w.n_chan == 0 || w.n_E == 0) continue;
     if (w.n_poles == 0) {
-      std::memset(w.R_out, 0, sizeof(double) * (size_t)w.n_E * w.n_chan * w.n_chan);
+      const size_t cc = (size_t)w.n_chan * w.n_chan;
+      std::memset(w.R_out, 0, sizeof(double) * (size_t)w.n_E * cc);
+      if (w.diag_add)
+        for (int e = 0; e < w.n_E; ++e)
+          for (int n = 0; n < w.n_chan; ++n) w.R_out[(size_t)e * cc + (size_t)n * w.n_chan + n] = w.diag_add[(size_t)e * w.n_chan + n];
       continue;
     }
     const bool tr = w.w_layout == PSTGF_W_CHANNEL_CONTIGUOUS;
@@ -728,13 +914,19 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
     PSTGF_CUDA(dev_alloc(sizeof(double) * (size_t)w.n_E, &dEn));
     PSTGF_CUDA(cudaMemcpyAsync(dEk, w.E_k, sizeof(double) * (size_t)w.n_poles, cudaMemcpyHostToDevice, res.s));
     PSTGF_CUDA(cudaMemcpyAsync(dEn, w.energies, sizeof(double) * (size_t)w.n_E, cudaMemcpyHostToDevice, res.s));
+    if (w.diag_add) {
+      void *dDa;
+      PSTGF_CUDA(dev_alloc(sizeof(double) * (size_t)w.n_E * w.n_chan, &dDa));
+      PSTGF_CUDA(cudaMemcpyAsync(dDa, w.diag_add, sizeof(double) * (size_t)w.n_E * w.n_chan, cudaMemcpyHostToDevice, res.s));
+      dev[p].diag_add = static_cast<double *>(dDa);
+    }
     dev[p].W = static_cast<double *>(dW);
     dev[p].ldw = pitch;
     dev[p].E_k = static_cast<double *>(dEk);
     dev[p].energies = static_cast<double *>(dEn);
     if (!overlap_upload) PSTGF_CUDA(upload_W(p, 0, w.n_poles, false));
   }
-  // Two ways to overlap the copy-back with the formation (pstgf_rmat_set_host_pipeline):
+  // Two ways to overlap the copy-back with the formation (pstgf_debug_set_host_pipeline):
   //  signalled  ONE launch forms a whole chunk (as much of R as the device budget allows); its segments (a wave's
   //             energy range of at most `cap` bytes) are the waves of that launch, each with a completion
   //             counter; the warp whose arrival completes a segment raises a flag in mapped host memory, and
@@ -744,8 +936,9 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
   //  chunked    one launch per chunk of at most `cap` bytes, copy-back ordered by events.
   size_t chunk_cap = cap;
   if (signalled) {
-    // device budget of a chunk: a quarter of the device's memory, at most 16 GiB (two chunks may be in flight);
-    // queried once per device -- cudaMemGetInfo on every call showed up as occasional stalls of tens of ms
+    // device budget of a chunk: a quarter of the device's memory, at most 16 GiB (two chunks may be in flight),
+    // halved below when the allocation fails (another allocator holding the memory); the total is queried once
+    // per device -- cudaMemGetInfo on every call showed up as occasional stalls of tens of ms
     static std::atomic<size_t> budget[64];
     size_t bud = ds.device < 64 ? budget[ds.device].load() : 0;
     if (!bud) {
@@ -759,43 +952,72 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
   // chunks of (wave, energy range) segments: a segment holds at most `cap` bytes of R (at least one energy
   // block), a chunk at most `chunk_cap` bytes and MAX_CHUNK_SEGMENTS segments
   std::vector<std::vector<Segment>> chunks;
-  size_t max_chunk = 0, cur = 0;
-  size_t max_segs = 1;
-  chunks.emplace_back();
-  for (int p = 0; p < n_waves; ++p) {
-    const pstgf_wave_t &w = waves[p];
-    if (!wave_has_items(w)) continue;
-    const size_t per_e = sizeof(double) * (size_t)w.n_chan * w.n_chan;
-    int e0 = 0;
-    while (e0 < w.n_E) {
-      size_t room = chunk_cap > cur ? chunk_cap - cur : 0;
-      if (signalled) room = std::min(room, cap);
-      int ne = (int)std::min<size_t>((size_t)(w.n_E - e0), room / per_e);
-      if (ne < w.n_E - e0) ne -= ne % pstgf::EB;      // split only at energy-block boundaries
-      if (signalled && ne <= 0 && chunk_cap > cur && chunk_cap - cur >= per_e * (size_t)pstgf::EB) ne = std::min(pstgf::EB, w.n_E - e0);
-      if (ne <= 0 || chunks.back().size() >= MAX_CHUNK_SEGMENTS) {
-        if (cur > 0) {                               // close the chunk and retry in an empty one
-          chunks.emplace_back();
-          cur = 0;
-          continue;
+  size_t max_chunk = 0, max_segs = 1;
+  auto plan_chunks = [&]() {
+    chunks.clear();
+    max_chunk = 0;
+    max_segs = 1;
+    size_t cur = 0;
+    chunks.emplace_back();
+    for (int p = 0; p < n_waves; ++p) {
+      const pstgf_wave_t &w = waves[p];
+      if (!wave_has_items(w)) continue;
+      const size_t per_e = sizeof(double) * (size_t)w.n_chan * w.n_chan;
+      int e0 = 0;
+      while (e0 < w.n_E) {
+        size_t room = chunk_cap > cur ? chunk_cap - cur : 0;
+        if (signalled) room = std::min(room, cap);
+        int ne = (int)std::min<size_t>((size_t)(w.n_E - e0), room / per_e);
+        if (ne < w.n_E - e0) ne -= ne % pstgf::EB;      // split only at energy-block boundaries
+        if (signalled && ne <= 0 && chunk_cap > cur && chunk_cap - cur >= per_e * (size_t)pstgf::EB) ne = std::min(pstgf::EB, w.n_E - e0);
+        if (ne <= 0 || chunks.back().size() >= MAX_CHUNK_SEGMENTS) {
+          if (cur > 0) {                               // close the chunk and retry in an empty one
+            chunks.emplace_back();
+            cur = 0;
+            continue;
+          }
+          ne = std::min(pstgf::EB, w.n_E - e0);          // one block does not fit the cap: take it anyway
         }
-        ne = std::min(pstgf::EB, w.n_E - e0);          // one block does not fit the cap: take it anyway
+        chunks.back().push_back(Segment{p, e0, ne, cur});
+        cur += per_e * (size_t)ne;
+        max_chunk = std::max(max_chunk, cur);
+        max_segs = std::max(max_segs, chunks.back().size());
+        e0 += ne;
       }
-      chunks.back().push_back(Segment{p, e0, ne, cur});
-      cur += per_e * (size_t)ne;
-      max_chunk = std::max(max_chunk, cur);
-      max_segs = std::max(max_segs, chunks.back().size());
-      e0 += ne;
     }
+    if (chunks.back().empty()) chunks.pop_back();
+  };
+  plan_chunks();
+  if (chunks.empty()) {
+    PSTGF_CUDA(cudaStreamSynchronize(res.s));
+    return PSTGF_OK;
   }
-  if (chunks.back().empty()) chunks.pop_back();
-  if (chunks.empty()) return PSTGF_OK;
-  const int ring = (int)std::min<size_t>(signalled ? 2 : HOST_RING, chunks.size());
-  void *rbuf[HOST_RING], *wsbuf[HOST_RING];
-  const size_t wsb = ws_bytes((int)max_segs);
-  for (int b = 0; b < ring; ++b) {
-    PSTGF_CUDA(dev_alloc(max_chunk, &rbuf[b]));
-    PSTGF_CUDA(dev_alloc(wsb, &wsbuf[b]));
+  int ring = 0;
+  void *rbuf[HOST_RING] = {nullptr}, *wsbuf[HOST_RING] = {nullptr};
+  size_t wsb = 0;
+  for (int attempt = 0;; ++attempt) {
+    ring = (int)std::min<size_t>(signalled ? 2 : HOST_RING, chunks.size());
+    wsb = ws_bytes((int)max_segs);
+    cudaError_t e = cudaSuccess;
+    int got = 0;
+    for (; got < ring && e == cudaSuccess; ++got) {
+      e = dev_alloc(max_chunk, &rbuf[got]);
+      if (e == cudaSuccess) e = dev_alloc(wsb, &wsbuf[got]);
+    }
+    if (e == cudaSuccess) break;
+    (void)cudaGetLastError();
+    // out of device memory: give back what this attempt took and retry with chunks of half the size
+    // (down to one energy block per chunk)
+    if (e != cudaErrorMemoryAllocation || attempt >= 8 || max_chunk <= cap) return cuda_fail(e);
+    for (int b = 0; b < got; ++b)
+      for (void *ptr : {rbuf[b], wsbuf[b]})
+        if (ptr) {
+          cudaFreeAsync(ptr, res.s);
+          res.allocs.erase(std::remove(res.allocs.begin(), res.allocs.end(), ptr), res.allocs.end());
+        }
+    for (int b = 0; b < HOST_RING; ++b) rbuf[b] = wsbuf[b] = nullptr;
+    chunk_cap = std::max<size_t>(cap, max_chunk / 2);
+    plan_chunks();
   }
   // the formation kernels run on two streams of the library's own, so that the first CTAs of chunk c+1 start on
   // the SMs the tail of chunk c has left; both wait for the inputs (and the allocations) enqueued on `stream`
@@ -821,7 +1043,8 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
         const long long k0 = extent * sl / n_slabs, k1 = extent * (sl + 1) / n_slabs;
         PSTGF_CUDA(upload_W(p, k0, k1, by_channels[(size_t)p] != 0));
         vals[sl] = (unsigned int)k1;
-        PSTGF_CUDA(cudaMemcpyAsync(flags.upload_counters + p, vals + sl, sizeof(unsigned int), cudaMemcpyHostToDevice, res.s));
+        if (!tl_stall_upload)     // (pstgf_debug_stall_upload: the signal is withheld and the launch must time out)
+          PSTGF_CUDA(cudaMemcpyAsync(flags.upload_counters + p, vals + sl, sizeof(unsigned int), cudaMemcpyHostToDevice, res.s));
       }
     }
   }
@@ -844,6 +1067,7 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
     for (const Segment &g : chunks[c]) {
       pstgf_wave_t w = dev[g.wave];
       w.energies = dev[g.wave].energies + g.e0;
+      if (w.diag_add) w.diag_add = dev[g.wave].diag_add + (size_t)g.e0 * w.n_chan;
       w.n_E = g.ne;
       w.R_out = reinterpret_cast<double *>(static_cast<unsigned char *>(rbuf[b]) + g.off);
       sub.push_back(w);
@@ -868,6 +1092,7 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
       completion.flag = flag.data();
       completion.rows_ready = rows_ready.data();
       completion.ready_counts_channels = ready_kind.data();
+      completion.abort_flag = flags.flags_dev + 2 * MAX_CHUNK_SEGMENTS;
       st = form_batch_impl(sub.data(), (int)sub.size(), wsbuf[b], wsb, cs, &completion);
       if (st != PSTGF_OK) return st;
       launches += tl_launches;
@@ -878,13 +1103,20 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
         while (flags.flags_host[f0 + (size_t)q] == 0u) {
           if (++polls < 2000) continue;
           std::this_thread::sleep_for(std::chrono::microseconds(20));
-          if ((polls & 0x3ffULL) == 0) {                // every ~1000 naps: has the launch died?
-            const cudaError_t e = cudaStreamQuery(cs);
+          if ((polls & 0xffULL) == 0) {                 // every ~250 naps: has the launch, or the upload, died?
+            cudaError_t e = cudaStreamQuery(cs);
             if (e != cudaSuccess && e != cudaErrorNotReady) return cuda_fail(e);
             if (e == cudaSuccess && flags.flags_host[f0 + (size_t)q] == 0u) return cuda_fail(cudaErrorUnknown);
+            e = cudaStreamQuery(res.s);
+            if (e != cudaSuccess && e != cudaErrorNotReady) return cuda_fail(e);
           }
         }
+        if (*abort_host != 0u) break;                    // the launch is draining: its R is not worth copying
         PSTGF_CUDA(copy_back(chunks[c][(size_t)q]));
+      }
+      if (*abort_host != 0u) {
+        PSTGF_CUDA(cudaStreamSynchronize(cs));
+        return PSTGF_ERR_TIMEOUT;
       }
     } else {
       st = pstgf_rmat_form_batch(sub.data(), (int)sub.size(), wsbuf[b], wsb, cs);
@@ -899,14 +1131,77 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
   PSTGF_CUDA(cudaStreamSynchronize(res.copy));
   for (cudaStream_t c : res.compute) PSTGF_CUDA(cudaStreamSynchronize(c));
   PSTGF_CUDA(cudaStreamSynchronize(res.s));
+  if (signalled && *abort_host != 0u) return PSTGF_ERR_TIMEOUT;
   tl_launches = launches;
   return PSTGF_OK;
 }
 
-pstgf_status_t pstgf_rmat_set_host_pipeline(int mode) {
+pstgf_status_t pstgf_debug_set_host_pipeline(int mode) {
   if (mode != PSTGF_HOST_PIPELINE_AUTO && mode != PSTGF_HOST_PIPELINE_CHUNKED) return PSTGF_ERR_INVALID_VALUE;
-  g_host_pipeline.store(mode);
+  tl_host_pipeline = mode;
   return PSTGF_OK;
+}
+
+pstgf_status_t pstgf_debug_set_upload_timeout_ms(unsigned int ms) {
+  tl_upload_timeout_ms = ms;
+  return PSTGF_OK;
+}
+
+pstgf_status_t pstgf_debug_stall_upload(int on) {
+  tl_stall_upload = on ? 1 : 0;
+  return PSTGF_OK;
+}
+
+// Frees what the library keeps between calls: the counter pools of pstgf_rmat_form, the memory pools and the
+// completion blocks of pstgf_rmat_form_batch_host, the planner caches.  Waits for each device to go idle first.
+pstgf_status_t pstgf_rmat_finalize(void) {
+  int prev = 0;
+  const bool have_dev = cudaGetDevice(&prev) == cudaSuccess;
+  if (!have_dev) (void)cudaGetLastError();
+  pstgf_status_t result = PSTGF_OK;
+  auto on_device = [&](int dev) -> bool {
+    if (cudaSetDevice(dev) != cudaSuccess || cudaDeviceSynchronize() != cudaSuccess) {
+      tl_cuda_error = (int)cudaGetLastError();
+      result = PSTGF_ERR_CUDA;
+      return false;
+    }
+    return true;
+  };
+  {
+    std::lock_guard<std::mutex> lock(g_counter_mutex);
+    for (int dev = 0; dev < 64; ++dev) {
+      CounterPool &cp = g_counters[dev];
+      if (!cp.base || !on_device(dev)) continue;
+      for (int i = 0; i < COUNTER_SLOTS; ++i) cudaEventDestroy(cp.ev[i]);
+      cudaFree(cp.base);
+      cp = CounterPool();
+    }
+  }
+  {
+    std::lock_guard<std::mutex> lock(g_flags_mutex);
+    for (HostFlags *f : g_flags_registry)
+      if (on_device(f->device)) free_host_flags(f);
+    g_flags_registry.clear();
+    g_flags_generation.fetch_add(1);
+  }
+  {
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
+    for (int dev = 0; dev < 64; ++dev) {
+      if (!g_pool[dev] || !on_device(dev)) continue;
+      cudaMemPoolDestroy(g_pool[dev]);
+      g_pool[dev] = nullptr;
+    }
+  }
+  {
+    std::lock_guard<std::mutex> lock(g_tail_mutex);
+    g_tail_cache.clear();
+  }
+  {
+    std::lock_guard<std::mutex> lock(g_slab_mutex);
+    g_slab_cache.clear();
+  }
+  if (have_dev) cudaSetDevice(prev);
+  return result;
 }
 
 int pstgf_last_launch_count(void) { return tl_launches; }
@@ -919,6 +1214,8 @@ const char *pstgf_status_string(pstgf_status_t status) {
     case PSTGF_ERR_WORKSPACE: return "PSTGF_ERR_WORKSPACE: workspace null, not 256-byte aligned, or too small";
     case PSTGF_ERR_UNSUPPORTED_DEVICE: return "PSTGF_ERR_UNSUPPORTED_DEVICE: needs a CUDA device of compute capability 10.x";
     case PSTGF_ERR_CUDA: return "PSTGF_ERR_CUDA: a CUDA call failed, see pstgf_last_cuda_error()";
+    case PSTGF_ERR_TIMEOUT: return "PSTGF_ERR_TIMEOUT: the launch gave up waiting for an upload of W; R_out is undefined";
+    case PSTGF_ERR_CAPTURE: return "PSTGF_ERR_CAPTURE: this call cannot be captured into a CUDA graph";
   }
   return "unknown pstgf_status_t";
 }

@@ -20,6 +20,12 @@
 //                tile * n_eb_section + eb (energy-fastest: CTAs running side by side share one W tile
 //                in L2).  An R element has the same operands and k order in both tilings (bitwise
 //                the same result).
+//   slab tiles   the energies that do not fill a block of 8 (n_E mod 8, and every energy of a call with
+//                n_E < 8: PSTGF calls RINIT once per (wave, energy)) are taken in groups
+//                of g = 2 or 1 energies, and the eight consumer warps split the TILE instead of the energy
+//                block: square tiles S(i, j), j >= i, of edge T = 128, 64 or 32 chosen by the planner so that
+//                there are enough items for the grid; the 8 / g warps of one energy each take a slab of the
+//                tile (SlabShape below).  Same operands, same k order: same bits as inside a block of 8.
 // Only tiles on or above the diagonal exist ("half of the symmetric R-matrix"),
 // the mirror is written by the epilogue ("symmetrised").
 #pragma once
@@ -30,42 +36,68 @@ namespace pstgf {
 
 constexpr int TM = 64;      // DIAG / OFF tile rows
 constexpr int TN = 32;      // OFF tile columns: J panel; also the TMA box height
-constexpr int TW = 128;     // WIDE tile rows (the I panel region of a stage holds this many rows)
+constexpr int TW = 128;     // WIDE tile rows (the I panel region of a classic stage holds this many rows)
 constexpr int TWN = 16;     // WIDE tile columns
 constexpr int KT = 20;      // poles per pipeline stage; row pitch 20 doubles == 4 (mod 16) -> conflict-free LDS.64
 constexpr int EB = 8;       // energies per item == consumer warps per CTA
-constexpr int STAGES = 7;   // smem ring depth
+constexpr int MAX_STAGES = 7;   // smem ring depth (fewer when a launch needs the larger stage of 128-row slab tiles)
 constexpr int PRODUCER_WARPS = 4;                    // one warpgroup: 1 load warp + 3 pole-scaling warps
 constexpr int NUM_THREADS = (EB + PRODUCER_WARPS) * 32;   // 8 consumer warps + the producer warpgroup
 constexpr int PRODUCER_REGS = 56;                    // setmaxnreg targets: 8*224 + 4*56 = 12*168, the launch allocation
 constexpr int CONSUMER_REGS = 224;
 constexpr int BOX_BYTES = TN * KT * 8;               // one TMA box: 32 rows x 20 poles
-constexpr int WI_BYTES = TW * KT * 8;                // I panel region: four boxes
-constexpr int WJ_BYTES = TN * KT * 8;
-constexpr int D_BYTES = EB * KT * 8;                 // d_e[k] = 1/(E_k - E_e) for the stage
-// Channel-contiguous W (the H.DAT record order) is staged pole-major: five panels
-// [KT poles][TR_PITCH channels] (I rows 0..31, 32..63, 64..95, 96..127, J), each one TMA box of 36 channels x 20 poles
+constexpr int D_DOUBLES = EB * KT;                   // d_e[k] = 1/(E_k - E_e) for the stage: first thing in a stage
+constexpr int D_BYTES = D_DOUBLES * 8;               // 1280 = 10 x 128: the panels behind it keep their bank pattern
+// Channel-contiguous W (the H.DAT record order) is staged pole-major: panels
+// [KT poles][TR_PITCH channels], each one TMA box of 36 channels x 20 poles
 // (32 used + 4 spare: the row pitch 36 == 4 (mod 16) doubles keeps the LDS.64 fragment loads conflict-free).
 constexpr int TR_PITCH = TN + 4;
 constexpr int TR_BOX_BYTES = KT * TR_PITCH * 8;      // 5760
-constexpr int STAGE_BYTES_ROWMAJOR = WI_BYTES + WJ_BYTES + D_BYTES;   // 26880
-constexpr int STAGE_BYTES_TR = 5 * TR_BOX_BYTES + D_BYTES;            // 30080
-constexpr int STAGE_BYTES = STAGE_BYTES_TR > STAGE_BYTES_ROWMAJOR ? STAGE_BYTES_TR : STAGE_BYTES_ROWMAJOR;
+constexpr int TR_BOX_DOUBLES = KT * TR_PITCH;
 
-// Offsets (in doubles) inside a stage, per layout.  i_off / j_off are additive in (row, k): the offset of
-// element (8 bi + g, 4 ks + q) is off(g, q) + off(8 bi, 4 ks).
+// A stage is [d 8 x 20 | panels of 32 channels x 20 poles].  Classic items use panels 0..3 for the I rows and
+// panel 4 for the J rows; slab items of edge T use panels [0, T/32) for the I rows and [T/32, 2 T/32) for J.
+// Offsets (in doubles) of element (row r, pole k) of the panel region; additive in (r, k) for 8-aligned r:
+// off(8 b + g, 4 s + q) = off(g, q) + off(8 b, 4 s).
 template <bool TR>
 struct StageLayout {
-  static constexpr int J_BASE = TR ? 4 * KT * TR_PITCH : TW * KT;
-  static constexpr int D_BASE = TR ? 5 * KT * TR_PITCH : (TW + TN) * KT;
-  __host__ __device__ static constexpr int i_off(int r, int k) {
-    return TR ? (r >> 5) * KT * TR_PITCH + k * TR_PITCH + (r & 31) : r * KT + k;
+  static constexpr int PANEL = TR ? TR_BOX_DOUBLES : TN * KT;       // doubles per panel of 32 channels
+  static constexpr int PANEL_BYTES = PANEL * 8;
+  static constexpr int W_BASE = D_DOUBLES;                          // panels start behind d
+  static constexpr int J_CLASSIC = W_BASE + (TW / TN) * PANEL;      // classic items: J panel behind four I panels
+  __host__ __device__ static constexpr int off(int r, int k) {
+    return TR ? (r >> 5) * TR_BOX_DOUBLES + k * TR_PITCH + (r & 31) : r * KT + k;
   }
-  __host__ __device__ static constexpr int j_off(int c, int k) { return TR ? k * TR_PITCH + c : c * KT + k; }
 };
-constexpr int SMEM_BARRIER_OFFSET = STAGES * STAGE_BYTES;
-constexpr int SMEM_ITEM_OFFSET = SMEM_BARRIER_OFFSET + (2 * STAGES + 4) * 8;
-constexpr int SMEM_BYTES = SMEM_ITEM_OFFSET + 2 * 96 + 128;  // two ItemInfo slots + alignment slack
+constexpr int stage_bytes_for(bool tr, int panels) { return D_BYTES + panels * (tr ? TR_BOX_BYTES : BOX_BYTES); }
+constexpr int CLASSIC_PANELS = TW / TN + 1;          // 5
+constexpr int BIG_PANELS = 2 * (TW / TN);            // 8: slab tiles of edge 128
+
+// Shared memory of a CTA: [mbarriers | two ItemInfo slots | ring of n_stages stages]; the ring geometry is a launch
+// parameter (RingGeo) because slab tiles of edge 128 need 8 panels per stage instead of 5.
+constexpr int SMEM_BARRIER_OFFSET = 0;               // (2 MAX_STAGES + 4) x 8 B
+constexpr int SMEM_ITEM_OFFSET = 256;                // 2 x 128 B
+constexpr int SMEM_RING_OFFSET = 512;
+constexpr int SMEM_ALIGN_SLACK = 128;
+constexpr int SMEM_MAX_OPTIN = 232448;               // 227 KB
+struct RingGeo {
+  int stage_bytes;
+  int n_stages;
+};
+constexpr int smem_bytes_for(RingGeo g) { return SMEM_RING_OFFSET + g.n_stages * g.stage_bytes + SMEM_ALIGN_SLACK; }
+
+// How the 8 / g consumer warps of one energy share a slab tile of edge T: a grid of wr x wc warps, each
+// computing NR row blocks x NCW column blocks of 8 x 8 (predicated on the diagonal and at the matrix edge).
+struct SlabShape {
+  int wc;    // warps across the columns
+  int nr;    // row blocks per warp: 16, 8, 4 or 2
+  int ncw;   // column blocks per warp: 2 or 1
+};
+__host__ __device__ inline SlabShape slab_shape(int T, int g) {
+  if (T == 128) return SlabShape{8, 16, 2};                 // g = 1 only: 8 warps x (16 x 2 blocks), the WIDE register tile
+  if (T == 64) return g == 1 ? SlabShape{4, 4, 2} : SlabShape{4, 8, 2};
+  return g == 1 ? SlabShape{4, 2, 1} : SlabShape{2, 2, 2};  // T == 32
+}
 
 // One partial wave as the kernel sees it.  Built on the host, lives in kernel parameter
 // space (single-wave call) or in the caller's workspace (batch call).
@@ -75,24 +107,32 @@ struct alignas(128) DevWave {
   const double *E_k;
   const double *energies;
   double *R_out;
+  const double *diag_add;  // optional [n_E][n_chan]: added to R_nn after the 1/(2a) scale (Buttle-type correction)
   unsigned int *done;      // optional completion counter of this wave (host-buffer call): += 1 per consumer warp and item
   unsigned int *done_flag; // ... and the (host-mapped) word that is set to 1 by the arrival that makes it done_target
   const unsigned int *rows_ready;   // optional (host-buffer call): how much of W has been uploaded so far, see the load warp
+  unsigned int *abort_flag;         // host-buffer call: set to 1 by a load warp whose wait for an upload timed out
   long long ldw;
   double inv2a;            // 1/(2a), PAPER.md:108 prefactor
   int n_chan, n_poles, n_E;
   int n_kt;                // ceil(n_poles / KT)
   int n_i;                 // ceil(n_chan / TM): DIAG tiles
   int n_j;                 // ceil(n_chan / TN)
-  int n_eb;                // ceil(n_E / EB)
+  int n_eb;                // energy blocks of 8 handled by classic items (n_E / 8, or ceil when the remainder is not slabbed)
   int n_tiles;             // coarse tiles: n_i DIAG + WIDE + OFF
   int use_tma;             // W 16-byte aligned and ldw even
   int n_eb_coarse;         // energy blocks [0, n_eb_coarse) use coarse tiles, [n_eb_coarse, n_eb) fine tiles
   unsigned int done_target;
   int ready_counts_channels;   // what rows_ready counts: 0 poles uploaded, 1 channels (rows of a pole-contiguous W)
   int tr;                  // 1: W is channel-contiguous [n_poles][ldw] (H.DAT record order), map box [KT][TR_PITCH]
+  int slab_e0;             // first energy handled by slab items (8 n_eb, or n_E when there are none)
+  int slab_g2, slab_g1;    // groups of two energies, then groups of one
+  int slab_T;              // tile edge of the slab items: 128, 64 or 32
+  int slab_nt;             // ceil(n_chan / slab_T): slab tiles = slab_nt (slab_nt + 1) / 2
+  int l2_keep;             // W fits half of L2: load it with the evict_last policy so that R's stores do not push it out
+  unsigned int wait_timeout_ms;   // bound on a load warp's wait for an upload slab (0 = 2000)
 };
-static_assert(sizeof(DevWave) == 256, "DevWave layout");
+static_assert(sizeof(DevWave) == 384, "DevWave layout (alignas 128; the batch workspace holds an array of these)");
 
 // Host-side tile arithmetic (also used by the kernel's decoder).
 // WIDE tiles of row pair p: columns from 128 (p + 1) to the end, 16 at a time.
@@ -113,6 +153,8 @@ __host__ __device__ inline int coarse_tiles(int n_chan) {
 }
 // Fine tiling: n_j row/column panels of 32; OFF32 tiles first (n_j (n_j - 1) / 2), then DIAG32 (n_j).
 __host__ __device__ inline int fine_tiles(int n_j) { return n_j * (n_j - 1) / 2 + n_j; }
+// Slab tiling: nt row/column panels of T; tiles row by row over the upper triangle, (0,0), (0,1), ..., (1,1), ...
+__host__ __device__ inline int slab_tiles(int nt) { return nt * (nt + 1) / 2; }
 
 // Relative cost of one item in DMMA.8x8x4 per k-step of 4 and energy: coarse DIAG 36, coarse OFF 32,
 // fine OFF 16, fine DIAG 10 (full-size tiles; ragged edge tiles are cheaper).

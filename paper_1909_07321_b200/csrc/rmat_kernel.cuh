@@ -4,36 +4,40 @@
 // registers to the consumers (setmaxnreg).  Warp 8 takes work items (atomic counter: in the workspace
 // for the batch call, in a pool slot for the single-wave call), publishes them and issues the TMA loads of the W
 // panels; warps 9..11 build the pole scaling d_e[k] = 1/(E_k - E_e) of every
-// stage in shared memory (S1; the denominator of eq. 4).  Warps 0..7 are consumers, one energy of the
-// item's block each: they contract acc[n][m] += W[n][k] * (W[m][k] * d_e[k]) on the FP64 tensor
-// pipe (mma.sync m8n8k4 -> DMMA.8x8x4) over upper-triangle tiles only (S3) and
-// write R and its mirror scaled by 1/(2a) (S4).  Producer and consumers are
-// coupled by an mbarrier full/empty ring that runs on across item boundaries, so the next
-// item's first stages land while the epilogue of the current one is being stored.
+// stage in shared memory (S1; the denominator of eq. 4).  Warps 0..7 are consumers.  On a classic
+// item each takes one energy of the item's block of 8; on a slab item (the energies that do not fill a block of
+// 8, taken two or one at a time) the warps of one energy split the tile between them.  Either way they contract
+// acc[n][m] += W[n][k] * (W[m][k] * d_e[k]) on the FP64 tensor pipe (mma.sync m8n8k4 -> DMMA.8x8x4) over
+// upper-triangle tiles only (S3) and write R and its mirror scaled by 1/(2a) (S4).
+// Producer and consumers are coupled by an mbarrier full/empty ring that runs on across item boundaries, so the
+// next item's first stages land while the epilogue of the current one is being stored.
 #pragma once
 #include "rmat_common.h"
 
 namespace pstgf {
 
 struct alignas(16) ItemInfo {   // handed from the load warp to the pole-scaling and consumer warps through smem
-  double *R;             // R_out of the block's first energy
-  unsigned int *done;    // completion counter of the item's wave, or null
-  unsigned int *done_flag;   // host-mapped word set to 1 when the counter reaches done_target
-  unsigned int done_target;
-  const double *E_k;     // the wave's poles
-  const double *energies;// the block's first energy
+  double *R;               // R_out of the item's first energy
+  const double *diag_add;  // the wave's diagonal addend at the item's first energy, or null
+  unsigned int *done;      // completion counter of the item's wave, or null
+  unsigned int *done_flag; // host-mapped word set to 1 when the counter reaches done_target
+  const double *E_k;       // the wave's poles
+  const double *energies;  // the item's first energy
   double inv2a;
+  unsigned int done_target;
   int n_chan;
   int n_poles;
-  int n_valid_e;         // energies in this block (1..EB)
+  int n_valid_e;           // energies of this item (1..EB; slab items: 2 or 1)
   int row0, col0;
-  short kind;            // 0 DIAG, 1 OFF / WIDE (rectangular, strictly above the diagonal), -1 stop
-  unsigned char nrb;     // rectangular tiles: 8-row blocks of the I panel (16 WIDE, 8 OFF, 4 fine OFF32)
-  unsigned char tr;      // stage layout: 0 row-major panels, 1 pole-major panels (channel-contiguous W)
-  int nblk;              // DIAG: valid 8x8 block rows/cols; rectangular tiles: valid 8-wide column blocks
+  int nblk;                // DIAG: valid 8x8 block rows/cols; rectangular tiles: valid 8-wide column blocks
   int n_kt;
+  short kind;              // 0 on the diagonal (DIAG / slab S(i,i)), 1 strictly above it, -1 stop
+  unsigned char nrb;       // classic rectangular tiles: 8-row blocks of the I panel (16 WIDE, 8 OFF, 4 fine OFF32)
+  unsigned char tr;        // stage layout: 0 row-major panels, 1 pole-major panels (channel-contiguous W)
+  unsigned char slab_T;    // 0: classic item (one energy per warp); else the edge of the slab tile (32, 64, 128)
+  unsigned char slab_g;    // slab items: energies in the group (2 or 1)
 };
-static_assert(sizeof(ItemInfo) == 96, "ItemInfo slot (SMEM_BYTES reserves 2 x 96)");
+static_assert(sizeof(ItemInfo) <= 128, "ItemInfo slot (SMEM_ITEM_OFFSET reserves 2 x 128)");
 
 // ---- PTX wrappers ------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p) {
@@ -67,6 +71,29 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map
       ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(bar)
       : "memory");
 }
+// The same with an L2 cache policy (evict_last for a W that fits half of L2: R's streaming stores then leave it alone).
+__device__ __forceinline__ void tma_load_2d_hint(uint32_t dst, const CUtensorMap *map, int c0, int c1, uint32_t bar,
+                                                 uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;"
+      ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(bar), "l"(policy)
+      : "memory");
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_last() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+// A tensor map that lives in global memory (the batch call's workspace, rewritten by every call) must be
+// acquired by the CTA before its first use by the TMA unit, or a stale cached copy may be used.
+__device__ __forceinline__ void tensormap_acquire(const CUtensorMap *map) {
+  asm volatile("fence.proxy.tensormap::generic.acquire.gpu [%0], 128;" ::"l"(reinterpret_cast<uint64_t>(map)) : "memory");
+}
+__device__ __forceinline__ unsigned long long global_timer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+  return t;
+}
 // D(8x8) += A(8x4) * B(4x8), FP64.  Lane l holds A[l/4][l%4], B[l%4][l/4], D[l/4][2*(l%4)+{0,1}].
 __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
@@ -80,14 +107,30 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
 // of the first items run behind the upload -- good when the upload takes about as long as an item; slabs of
 // channels (rows of a pole-contiguous W) let the tiles near the top of the matrix run at full speed while the
 // rest is still coming -- good when the upload takes many item times (the 6.2 GB of the paper-scale wave).
+// The wait is bounded: after timeout_ns without the counter reaching `need` (a failed or serialised upload) the
+// warp raises the launch's abort flag and stops waiting; every other load warp sees the flag at its next wait, the
+// launch drains, and the host turns the flag into PSTGF_ERR_TIMEOUT (the R of that call is then undefined).
 __device__ __forceinline__ void wait_rows_uploaded(const unsigned int *rows_ready, unsigned int need, unsigned int &seen,
-                                                   int lane) {
+                                                   unsigned int *abort_flag, unsigned long long timeout_ns, int lane) {
   if (seen >= need) return;
   if (lane == 0) {
     unsigned int v;
+    const unsigned long long t0 = global_timer_ns();
     for (;;) {
       asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(rows_ready) : "memory");
       if (v >= need) break;
+      if (abort_flag != nullptr) {
+        unsigned int ab;
+        asm volatile("ld.relaxed.sys.global.u32 %0, [%1];" : "=r"(ab) : "l"(abort_flag) : "memory");
+        if (ab == 0u && global_timer_ns() - t0 > timeout_ns) {
+          atomicExch_system(abort_flag, 1u);
+          ab = 1u;
+        }
+        if (ab != 0u) {
+          v = 0xffffffffu;
+          break;
+        }
+      }
       __nanosleep(500);
     }
     seen = v;
@@ -96,11 +139,20 @@ __device__ __forceinline__ void wait_rows_uploaded(const unsigned int *rows_read
   seen = __shfl_sync(0xffffffffu, seen, 0);
 }
 
-struct PipeState {
+// Position in the shared-memory ring, with the ring's geometry (a launch parameter: RingGeo).
+struct Pipe {
+  const unsigned char *ring;
+  uint32_t full0, empty0;
+  int stage_bytes, n_stages;
   uint32_t stage = 0, phase = 0;
   __device__ __forceinline__ void advance() {
-    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+    if (++stage == (uint32_t)n_stages) { stage = 0; phase ^= 1u; }
   }
+  __device__ __forceinline__ const double *stage_ptr() const {
+    return reinterpret_cast<const double *>(ring + (size_t)stage * stage_bytes);
+  }
+  __device__ __forceinline__ uint32_t full() const { return full0 + 8 * stage; }
+  __device__ __forceinline__ uint32_t empty() const { return empty0 + 8 * stage; }
 };
 
 // ---- consumers ---------------------------------------------------------------------------
@@ -111,18 +163,19 @@ struct PipeState {
 // host memory, every store a PCIe write -- it showed as a few wrong rows per launch.  A CTA-scope fence executed
 // by the whole warp before the release closes it: the warp's loads have been performed when the fence retires
 // (costs 0.5 % on config 5; releasing one stage late instead was measured and is no cheaper).
-__device__ __forceinline__ void release_stage(uint32_t empty0, uint32_t stage, int lane) {
+__device__ __forceinline__ void release_stage(const Pipe &ps, int lane) {
   __threadfence_block();
   __syncwarp();
-  if (lane == 0) mbar_arrive(empty0 + 8 * stage);
+  if (lane == 0) mbar_arrive(ps.empty());
 }
 
-// Warps whose energy slot lies beyond n_E only keep the ring moving.
-__device__ __forceinline__ void consume_idle(int n_kt, PipeState &ps, uint32_t full0, uint32_t empty0, int lane) {
+// Warps with nothing to compute in an item (an energy slot beyond n_E, a slab below the diagonal) only keep the
+// ring moving.
+__device__ __forceinline__ void consume_idle(int n_kt, Pipe &ps, int lane) {
   for (int kt = 0; kt < n_kt; ++kt) {
-    mbar_wait(full0 + 8 * ps.stage, ps.phase);
+    mbar_wait(ps.full(), ps.phase);
     __syncwarp();
-    if (lane == 0) mbar_arrive(empty0 + 8 * ps.stage);
+    if (lane == 0) mbar_arrive(ps.empty());
     ps.advance();
   }
 }
@@ -131,35 +184,34 @@ __device__ __forceinline__ void consume_idle(int n_kt, PipeState &ps, uint32_t f
 // fine OFF32 32 x 32 (NRB = 4); NRB x NCB DMMA blocks, all needed (column blocks >= nblk lie beyond n_chan and
 // are skipped).  One scaled B fragment feeds NRB DMMAs: the WIDE shape halves the DMULs per DMMA of OFF.
 template <int NCB, int NRB, bool TR>
-__device__ __forceinline__ void consume_off(const ItemInfo &it, const unsigned char *smem, PipeState &ps,
-                                            uint32_t full0, uint32_t empty0, int warp, int lane) {
+__device__ __forceinline__ void consume_off(const ItemInfo &it, Pipe &ps, int warp, int lane) {
   double acc[NRB][NCB][2];
 #pragma unroll
   for (int bi = 0; bi < NRB; ++bi)
 #pragma unroll
     for (int bj = 0; bj < NCB; ++bj) acc[bi][bj][0] = acc[bi][bj][1] = 0.0;
   const int g = lane >> 2, q = lane & 3;
+  using L = StageLayout<TR>;
   for (int kt = 0; kt < it.n_kt; ++kt) {
-    mbar_wait(full0 + 8 * ps.stage, ps.phase);
-    using L = StageLayout<TR>;
-    const double *st = reinterpret_cast<const double *>(smem + ps.stage * STAGE_BYTES);
-    const double *wi = st + L::i_off(g, q);
-    const double *wj = st + L::J_BASE + L::j_off(g, q);
-    const double *dd = st + L::D_BASE + warp * KT + q;
+    mbar_wait(ps.full(), ps.phase);
+    const double *st = ps.stage_ptr();
+    const double *wi = st + L::W_BASE + L::off(g, q);
+    const double *wj = st + L::J_CLASSIC + L::off(g, q);
+    const double *dd = st + warp * KT + q;
 #pragma unroll
     for (int ks = 0; ks < KT / 4; ++ks) {
       const double dv = dd[ks * 4];
       double a[NRB];
 #pragma unroll
-      for (int bi = 0; bi < NRB; ++bi) a[bi] = wi[L::i_off(bi * 8, ks * 4)];
+      for (int bi = 0; bi < NRB; ++bi) a[bi] = wi[L::off(bi * 8, ks * 4)];
 #pragma unroll
       for (int bj = 0; bj < NCB; ++bj) {
-        const double b = wj[L::j_off(bj * 8, ks * 4)] * dv;   // pole scaling folded into the B fragment
+        const double b = wj[L::off(bj * 8, ks * 4)] * dv;   // pole scaling folded into the B fragment
 #pragma unroll
         for (int bi = 0; bi < NRB; ++bi) dmma884(acc[bi][bj][0], acc[bi][bj][1], a[bi], b);
       }
     }
-    release_stage(empty0, ps.stage, lane);
+    release_stage(ps, lane);
     ps.advance();
   }
   // epilogue: R[r][c] and the mirror R[c][r]; rows are always inside the matrix for OFF tiles
@@ -181,26 +233,26 @@ __device__ __forceinline__ void consume_off(const ItemInfo &it, const unsigned c
 
 // DIAG tile: 64 x 64 block on the diagonal; only 8x8 blocks (bi <= bj) are computed, and in
 // blocks on the diagonal only elements c >= r are stored (with their mirror), so that
-// R[n][m] == R[m][n] bitwise.
+// R[n][m] == R[m][n] bitwise.  The optional diagonal addend (pstgf_wave_t.diag_add) goes onto R[n][n] here,
+// after the 1/(2a) scale.
 template <int NB, bool TR>
-__device__ __forceinline__ void consume_diag(const ItemInfo &it, const unsigned char *smem, PipeState &ps,
-                                             uint32_t full0, uint32_t empty0, int warp, int lane) {
+__device__ __forceinline__ void consume_diag(const ItemInfo &it, Pipe &ps, int warp, int lane) {
   double acc[NB * (NB + 1) / 2][2];
 #pragma unroll
   for (int t = 0; t < NB * (NB + 1) / 2; ++t) acc[t][0] = acc[t][1] = 0.0;
   const int g = lane >> 2, q = lane & 3;
+  using L = StageLayout<TR>;
   for (int kt = 0; kt < it.n_kt; ++kt) {
-    mbar_wait(full0 + 8 * ps.stage, ps.phase);
-    using L = StageLayout<TR>;
-    const double *st = reinterpret_cast<const double *>(smem + ps.stage * STAGE_BYTES);
-    const double *wi = st + L::i_off(g, q);
-    const double *dd = st + L::D_BASE + warp * KT + q;
+    mbar_wait(ps.full(), ps.phase);
+    const double *st = ps.stage_ptr();
+    const double *wi = st + L::W_BASE + L::off(g, q);
+    const double *dd = st + warp * KT + q;
 #pragma unroll
     for (int ks = 0; ks < KT / 4; ++ks) {
       const double dv = dd[ks * 4];
       double a[NB];
 #pragma unroll
-      for (int bi = 0; bi < NB; ++bi) a[bi] = wi[L::i_off(bi * 8, ks * 4)];
+      for (int bi = 0; bi < NB; ++bi) a[bi] = wi[L::off(bi * 8, ks * 4)];
 #pragma unroll
       for (int bj = 0; bj < NB; ++bj) {
         const double b = a[bj] * dv;
@@ -208,11 +260,12 @@ __device__ __forceinline__ void consume_diag(const ItemInfo &it, const unsigned 
         for (int bi = 0; bi <= bj; ++bi) dmma884(acc[bj * (bj + 1) / 2 + bi][0], acc[bj * (bj + 1) / 2 + bi][1], a[bi], b);
       }
     }
-    release_stage(empty0, ps.stage, lane);
+    release_stage(ps, lane);
     ps.advance();
   }
   const int C = it.n_chan;
   double *R = it.R + (size_t)warp * C * C;
+  const double *da = it.diag_add ? it.diag_add + (size_t)warp * C : nullptr;
   const double s = it.inv2a;
 #pragma unroll
   for (int bj = 0; bj < NB; ++bj) {
@@ -220,15 +273,108 @@ __device__ __forceinline__ void consume_diag(const ItemInfo &it, const unsigned 
 #pragma unroll
     for (int bi = 0; bi <= bj; ++bi) {
       const int r = it.row0 + bi * 8 + g;
-      const double v0 = acc[bj * (bj + 1) / 2 + bi][0] * s, v1 = acc[bj * (bj + 1) / 2 + bi][1] * s;
+      double v0 = acc[bj * (bj + 1) / 2 + bi][0] * s, v1 = acc[bj * (bj + 1) / 2 + bi][1] * s;
       if (r < C) {
         if (c < C && c >= r) {
+          if (bi == bj && c == r && da) v0 += __ldg(da + r);
           __stcs(R + (size_t)r * C + c, v0);
           if (c > r) __stcs(R + (size_t)c * C + r, v0);
         }
         if (c + 1 < C && c + 1 >= r) {
+          if (bi == bj && c + 1 == r && da) v1 += __ldg(da + r);
           __stcs(R + (size_t)r * C + c + 1, v1);
           if (c + 1 > r) __stcs(R + (size_t)(c + 1) * C + r, v1);
+        }
+      }
+    }
+  }
+}
+
+// Slab item: a square tile S(i, j) of edge T for a group of g = 2 or 1 energies.  The 8 / g warps of one energy
+// form a grid of wr x wc warps over the tile (SlabShape); this warp computes row blocks [rb0, rb0 + NR) x column
+// blocks [cb0, cb0 + NCW) of 8 x 8.  The DMMA loop has no predicates: a warp whose slab is cut by the diagonal or by
+// the edge of the matrix computes all of its register tile and stores only what is wanted (nrc[c] row blocks of
+// column c: a prefix, because rows ascend); a warp with nothing wanted only keeps the ring moving.  A = rows of
+// the I panels, B = scaled rows of the J panels (the I panels on a diagonal tile): the same operands and k order
+// as a classic item gives the element, hence the same bits.
+template <int NR, int NCW, bool TR>
+__device__ __forceinline__ void consume_slab(const ItemInfo &it, Pipe &ps, int warp, int lane, int wc) {
+  using L = StageLayout<TR>;
+  const int T = it.slab_T, gE = it.slab_g, C = it.n_chan;
+  const int e_slot = warp % gE, s = warp / gE;              // which energy of the group, which slab of the tile
+  const int wci = s % wc, wri = s / wc;
+  const int rb0 = wri * NR, cb0 = wci * NCW;
+  const bool diag = it.kind == 0;
+  const int vrb = min(T / 8, (C - it.row0 + 7) / 8);        // row blocks of the tile inside the matrix
+  int nrc[NCW];
+  bool any = false;
+#pragma unroll
+  for (int c = 0; c < NCW; ++c) {
+    const int cb = cb0 + c;
+    const int lim = min(diag ? cb + 1 : T / 8, vrb);         // on a diagonal tile only row blocks rb <= cb
+    nrc[c] = it.col0 + cb * 8 < C ? max(0, min(NR, lim - rb0)) : 0;
+    any = any || nrc[c] > 0;
+  }
+  if (!any) {
+    consume_idle(it.n_kt, ps, lane);
+    return;
+  }
+  const int g = lane >> 2, q = lane & 3;
+  const int jrow = diag ? 0 : T;                             // B fragments: rows of the J panels (behind the I panels)
+  const int aoff = L::W_BASE + L::off(rb0 * 8, 0) + L::off(g, q);
+  const int boff = L::W_BASE + L::off(jrow + cb0 * 8, 0) + L::off(g, q);
+  const int doff = e_slot * KT + q;
+  double acc[NR][NCW][2];
+#pragma unroll
+  for (int bi = 0; bi < NR; ++bi)
+#pragma unroll
+    for (int c = 0; c < NCW; ++c) acc[bi][c][0] = acc[bi][c][1] = 0.0;
+  for (int kt = 0; kt < it.n_kt; ++kt) {
+    mbar_wait(ps.full(), ps.phase);
+    const double *st = ps.stage_ptr();
+    const double *wa = st + aoff;
+    const double *wb = st + boff;
+    const double *dd = st + doff;
+#pragma unroll
+    for (int ks = 0; ks < KT / 4; ++ks) {
+      const double dv = dd[ks * 4];
+      double a[NR];
+#pragma unroll
+      for (int bi = 0; bi < NR; ++bi) a[bi] = wa[L::off(bi * 8, ks * 4)];
+#pragma unroll
+      for (int c = 0; c < NCW; ++c) {
+        const double b = wb[L::off(c * 8, ks * 4)] * dv;     // pole scaling folded into the B fragment
+#pragma unroll
+        for (int bi = 0; bi < NR; ++bi) dmma884(acc[bi][c][0], acc[bi][c][1], a[bi], b);
+      }
+    }
+    release_stage(ps, lane);
+    ps.advance();
+  }
+  // epilogue
+  double *R = it.R + (size_t)e_slot * C * C;
+  const double *da = it.diag_add ? it.diag_add + (size_t)e_slot * C : nullptr;
+  const double sc = it.inv2a;
+#pragma unroll
+  for (int c = 0; c < NCW; ++c) {
+    const int col = it.col0 + (cb0 + c) * 8 + 2 * q;
+#pragma unroll
+    for (int bi = 0; bi < NR; ++bi) {
+      if (bi < nrc[c]) {
+        const int r = it.row0 + (rb0 + bi) * 8 + g;
+        const bool dg = diag && rb0 + bi == cb0 + c;         // a block on the diagonal: keep col >= r only
+        double v0 = acc[bi][c][0] * sc, v1 = acc[bi][c][1] * sc;
+        if (r < C) {
+          if (col < C && (!dg || col >= r)) {
+            if (dg && col == r && da) v0 += __ldg(da + r);
+            __stcs(R + (size_t)r * C + col, v0);
+            if (col != r) __stcs(R + (size_t)col * C + r, v0);
+          }
+          if (col + 1 < C && (!dg || col + 1 >= r)) {
+            if (dg && col + 1 == r && da) v1 += __ldg(da + r);
+            __stcs(R + (size_t)r * C + col + 1, v1);
+            if (col + 1 != r) __stcs(R + (size_t)(col + 1) * C + r, v1);
+          }
         }
       }
     }
@@ -238,43 +384,58 @@ __device__ __forceinline__ void consume_diag(const ItemInfo &it, const unsigned 
 // The tile shapes are compile-time variants (no predicates inside the DMMA loop); ragged edges of
 // a wave pick the variant with fewer 8-wide blocks.
 template <bool TR>
-__device__ __forceinline__ void consume_item_layout(const ItemInfo &it, const unsigned char *smem, PipeState &ps,
-                                                    uint32_t full0, uint32_t empty0, int warp, int lane) {
+__device__ __forceinline__ void consume_item_layout(const ItemInfo &it, Pipe &ps, int warp, int lane) {
+  if (it.slab_T != 0) {
+    const SlabShape sh = slab_shape(it.slab_T, it.slab_g);
+    switch (sh.nr) {
+      case 16: consume_slab<16, 2, TR>(it, ps, warp, lane, sh.wc); break;
+      case 8: consume_slab<8, 2, TR>(it, ps, warp, lane, sh.wc); break;
+      case 4: consume_slab<4, 2, TR>(it, ps, warp, lane, sh.wc); break;
+      default:
+        if (sh.ncw == 2) consume_slab<2, 2, TR>(it, ps, warp, lane, sh.wc);
+        else consume_slab<2, 1, TR>(it, ps, warp, lane, sh.wc);
+        break;
+    }
+    return;
+  }
+  if (warp >= it.n_valid_e) {
+    consume_idle(it.n_kt, ps, lane);
+    return;
+  }
   if (it.kind == 0) {
     switch (it.nblk) {
-      case 8: consume_diag<8, TR>(it, smem, ps, full0, empty0, warp, lane); break;
-      case 7: consume_diag<7, TR>(it, smem, ps, full0, empty0, warp, lane); break;
-      case 6: consume_diag<6, TR>(it, smem, ps, full0, empty0, warp, lane); break;
-      case 5: consume_diag<5, TR>(it, smem, ps, full0, empty0, warp, lane); break;
-      case 4: consume_diag<4, TR>(it, smem, ps, full0, empty0, warp, lane); break;
-      case 3: consume_diag<3, TR>(it, smem, ps, full0, empty0, warp, lane); break;
-      case 2: consume_diag<2, TR>(it, smem, ps, full0, empty0, warp, lane); break;
-      default: consume_diag<1, TR>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 8: consume_diag<8, TR>(it, ps, warp, lane); break;
+      case 7: consume_diag<7, TR>(it, ps, warp, lane); break;
+      case 6: consume_diag<6, TR>(it, ps, warp, lane); break;
+      case 5: consume_diag<5, TR>(it, ps, warp, lane); break;
+      case 4: consume_diag<4, TR>(it, ps, warp, lane); break;
+      case 3: consume_diag<3, TR>(it, ps, warp, lane); break;
+      case 2: consume_diag<2, TR>(it, ps, warp, lane); break;
+      default: consume_diag<1, TR>(it, ps, warp, lane); break;
     }
   } else if (it.nrb == 16) {
-    if (it.nblk == 2) consume_off<2, 16, TR>(it, smem, ps, full0, empty0, warp, lane);
-    else consume_off<1, 16, TR>(it, smem, ps, full0, empty0, warp, lane);
+    if (it.nblk == 2) consume_off<2, 16, TR>(it, ps, warp, lane);
+    else consume_off<1, 16, TR>(it, ps, warp, lane);
   } else if (it.nrb == 8) {
     switch (it.nblk) {
-      case 4: consume_off<4, 8, TR>(it, smem, ps, full0, empty0, warp, lane); break;
-      case 3: consume_off<3, 8, TR>(it, smem, ps, full0, empty0, warp, lane); break;
-      case 2: consume_off<2, 8, TR>(it, smem, ps, full0, empty0, warp, lane); break;
-      default: consume_off<1, 8, TR>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 4: consume_off<4, 8, TR>(it, ps, warp, lane); break;
+      case 3: consume_off<3, 8, TR>(it, ps, warp, lane); break;
+      case 2: consume_off<2, 8, TR>(it, ps, warp, lane); break;
+      default: consume_off<1, 8, TR>(it, ps, warp, lane); break;
     }
   } else {
     switch (it.nblk) {
-      case 4: consume_off<4, 4, TR>(it, smem, ps, full0, empty0, warp, lane); break;
-      case 3: consume_off<3, 4, TR>(it, smem, ps, full0, empty0, warp, lane); break;
-      case 2: consume_off<2, 4, TR>(it, smem, ps, full0, empty0, warp, lane); break;
-      default: consume_off<1, 4, TR>(it, smem, ps, full0, empty0, warp, lane); break;
+      case 4: consume_off<4, 4, TR>(it, ps, warp, lane); break;
+      case 3: consume_off<3, 4, TR>(it, ps, warp, lane); break;
+      case 2: consume_off<2, 4, TR>(it, ps, warp, lane); break;
+      default: consume_off<1, 4, TR>(it, ps, warp, lane); break;
     }
   }
 }
 
-__device__ __forceinline__ void consume_item(const ItemInfo &it, const unsigned char *smem, PipeState &ps,
-                                             uint32_t full0, uint32_t empty0, int warp, int lane) {
-  if (it.tr) consume_item_layout<true>(it, smem, ps, full0, empty0, warp, lane);
-  else consume_item_layout<false>(it, smem, ps, full0, empty0, warp, lane);
+__device__ __forceinline__ void consume_item(const ItemInfo &it, Pipe &ps, int warp, int lane) {
+  if (it.tr) consume_item_layout<true>(it, ps, warp, lane);
+  else consume_item_layout<false>(it, ps, warp, lane);
 }
 
 // ---- producer ----------------------------------------------------------------------------
@@ -341,13 +502,27 @@ __device__ __forceinline__ void decode_tile(const DevWave &w, int tile, int &kin
   }
 }
 
+// Slab tile index -> S(i, j), j >= i, row by row over the upper triangle of slab_nt x slab_nt tiles.
+__device__ __forceinline__ void decode_tile_slab(const DevWave &w, int tile, int &kind, int &row0, int &col0) {
+  int t = tile, i = 0;
+  for (;; ++i) {
+    const int cnt = w.slab_nt - i;
+    if (t < cnt) break;
+    t -= cnt;
+  }
+  row0 = i * w.slab_T;
+  col0 = (i + t) * w.slab_T;
+  kind = t == 0 ? 0 : 1;
+}
+
 // Staging without TMA (W not 16-byte aligned or ldw odd): the producer warp copies the panels
-// with plain loads, zero-filling rows >= n_chan and poles >= n_poles like the TMA path does.
+// with plain loads, zero-filling rows >= n_chan and poles >= n_poles like the TMA path does.  The loads are
+// L2-coherent (ld.global.cg): in the host-buffer call W may still be arriving while earlier slabs are read.
 __device__ __forceinline__ void stage_panel_plain(double *dst, const DevWave &w, int row0, int rows, int k0, int lane) {
   for (int idx = lane; idx < rows * KT; idx += 32) {
     const int r = idx / KT, kk = idx - r * KT;
     const int row = row0 + r, k = k0 + kk;
-    dst[idx] = (row < w.n_chan && k < w.n_poles) ? __ldg(w.W + (size_t)row * w.ldw + k) : 0.0;
+    dst[idx] = (row < w.n_chan && k < w.n_poles) ? __ldcg(w.W + (size_t)row * w.ldw + k) : 0.0;
   }
 }
 
@@ -355,7 +530,7 @@ __device__ __forceinline__ void stage_panel_plain(double *dst, const DevWave &w,
 __device__ __forceinline__ void stage_panel_plain_tr(double *dst, const DevWave &w, int row0, int k0, int lane) {
   for (int kk = 0; kk < KT; ++kk) {
     const int row = row0 + lane, k = k0 + kk;
-    dst[kk * TR_PITCH + lane] = (row < w.n_chan && k < w.n_poles) ? __ldg(w.W + (size_t)k * w.ldw + row) : 0.0;
+    dst[kk * TR_PITCH + lane] = (row < w.n_chan && k < w.n_poles) ? __ldcg(w.W + (size_t)k * w.ldw + row) : 0.0;
   }
 }
 
@@ -363,16 +538,17 @@ template <bool BATCH>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__restrict__ waves,
                        const long long *__restrict__ item_begin, int n_waves, long long n_items,
-                       unsigned long long *counter) {
+                       unsigned long long *counter, const RingGeo geo) {
   extern __shared__ __align__(128) unsigned char smem[];   // used directly: the shared address space is kept (LDS/STS)
   const uint32_t bar0 = smem_u32(smem + SMEM_BARRIER_OFFSET);
-  const uint32_t full0 = bar0, empty0 = bar0 + 8 * STAGES;
-  const uint32_t item_full0 = bar0 + 16 * STAGES, item_empty0 = item_full0 + 16;
-  ItemInfo *ring = reinterpret_cast<ItemInfo *>(smem + SMEM_ITEM_OFFSET);   // 2 slots of 96 B
+  const uint32_t full0 = bar0, empty0 = bar0 + 8 * MAX_STAGES;
+  const uint32_t item_full0 = bar0 + 16 * MAX_STAGES, item_empty0 = item_full0 + 16;
+  ItemInfo *ring = reinterpret_cast<ItemInfo *>(smem + SMEM_ITEM_OFFSET);   // 2 slots of 128 B
+  unsigned char *stages = smem + SMEM_RING_OFFSET;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < STAGES; ++s) {
+    for (int s = 0; s < geo.n_stages; ++s) {
       mbar_init(full0 + 8 * s, PRODUCER_WARPS);   // load warp (TMA expect_tx / plain staging done) + 3 pole-scaling warps
       mbar_init(empty0 + 8 * s, EB);   // one arrival per consumer warp
     }
@@ -384,14 +560,22 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
   }
   __syncthreads();
 
+  Pipe ps;
+  ps.ring = stages;
+  ps.full0 = full0;
+  ps.empty0 = empty0;
+  ps.stage_bytes = geo.stage_bytes;
+  ps.n_stages = geo.n_stages;
+
   if (warp >= EB) {
     // ================= producer warpgroup: give registers away =================
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(PRODUCER_REGS));
     if (warp == EB) {
       // ---- load warp: takes work items, publishes them, stages the W panels (S2, S5) ----
-      PipeState ps;
       uint32_t iq = 0, iphase = 0;
       long long next_static = blockIdx.x;
+      const uint64_t keep_policy = l2_policy_evict_last();
+      int last_wave = -1;
       for (;;) {
         // items are drawn from an atomic counter (batch call: in the workspace; single-wave call: a slot of
         // the library's counter pool), or round-robin when the single-wave call found no free slot
@@ -405,38 +589,51 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
           next_static += gridDim.x;
         }
         const bool stop = item >= n_items;
-        // locate the section: [coarse items of wave 0, 1, ... | fine items of wave 0, 1, ...]
-        int p = 0;
-        bool fine = false;
+        // locate the section: [coarse items of wave 0, 1, ... | slab items of wave 0, 1, ... | fine items of wave 0, 1, ...]
+        int p = 0, sec = 0;
         if (!stop) {
           if (BATCH) {
-            int lo = 0, hi = 2 * n_waves;        // item_begin[lo] <= item < item_begin[hi]
+            int lo = 0, hi = 3 * n_waves;        // item_begin[lo] <= item < item_begin[hi]
             while (hi - lo > 1) {
               const int mid = (lo + hi) >> 1;
               if (__ldg(item_begin + mid) <= item) lo = mid; else hi = mid;
             }
             item -= __ldg(item_begin + lo);
-            fine = lo >= n_waves;
-            p = fine ? lo - n_waves : lo;
+            sec = lo / n_waves;
+            p = lo - sec * n_waves;
           } else {
             const long long n_coarse = (long long)single.n_tiles * single.n_eb_coarse;
-            fine = item >= n_coarse;
-            if (fine) item -= n_coarse;
+            const long long n_slab = (long long)slab_tiles(single.slab_nt) * (single.slab_g2 + single.slab_g1);
+            if (item >= n_coarse + n_slab) { sec = 2; item -= n_coarse + n_slab; }
+            else if (item >= n_coarse) { sec = 1; item -= n_coarse; }
           }
         }
         const DevWave &w = BATCH ? waves[p] : single;
-        int kind = -1, row0 = 0, col0 = 0, nblk = 0, nrb = 0, eb = 0, n_valid = 0, n_kt = 0;
+        int kind = -1, row0 = 0, col0 = 0, nblk = 0, nrb = 0, e_first = 0, n_valid = 0, n_kt = 0, slab_T = 0, slab_g = 0;
         if (!stop) {
-          const int n_eb_sec = fine ? w.n_eb - w.n_eb_coarse : w.n_eb_coarse;
-          const int tile = (int)(item / n_eb_sec);
-          eb = (int)(item - (long long)tile * n_eb_sec) + (fine ? w.n_eb_coarse : 0);
-          if (fine) {
-            decode_tile_fine(w, tile, kind, row0, col0, nblk);
-            nrb = kind == 0 ? nblk : TN / 8;                   // 8-row blocks of the I panel that are read
+          if (sec == 1) {
+            const int n_groups = w.slab_g2 + w.slab_g1;
+            const int tile = (int)(item / n_groups);
+            const int gi = (int)(item - (long long)tile * n_groups);
+            decode_tile_slab(w, tile, kind, row0, col0);
+            slab_T = w.slab_T;
+            slab_g = gi < w.slab_g2 ? 2 : 1;
+            e_first = w.slab_e0 + (gi < w.slab_g2 ? 2 * gi : 2 * w.slab_g2 + (gi - w.slab_g2));
+            n_valid = slab_g;
           } else {
-            decode_tile(w, tile, kind, row0, col0, nblk, nrb);
+            const bool fine = sec == 2;
+            const int n_eb_sec = fine ? w.n_eb - w.n_eb_coarse : w.n_eb_coarse;
+            const int tile = (int)(item / n_eb_sec);
+            const int eb = (int)(item - (long long)tile * n_eb_sec) + (fine ? w.n_eb_coarse : 0);
+            if (fine) {
+              decode_tile_fine(w, tile, kind, row0, col0, nblk);
+              nrb = kind == 0 ? nblk : TN / 8;                   // 8-row blocks of the I panel that are read
+            } else {
+              decode_tile(w, tile, kind, row0, col0, nblk, nrb);
+            }
+            e_first = eb * EB;
+            n_valid = min(EB, w.n_E - e_first);
           }
-          n_valid = min(EB, w.n_E - eb * EB);
           n_kt = w.n_kt;
         }
         mbar_wait(item_empty0 + 8 * iq, iphase ^ 1u);
@@ -444,12 +641,13 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
           ItemInfo &ii = ring[iq];
           ii.kind = (short)kind;
           if (!stop) {
-            ii.R = w.R_out + (size_t)eb * EB * w.n_chan * w.n_chan;
+            ii.R = w.R_out + (size_t)e_first * w.n_chan * w.n_chan;
+            ii.diag_add = w.diag_add ? w.diag_add + (size_t)e_first * w.n_chan : nullptr;
             ii.done = w.done;
             ii.done_flag = w.done_flag;
             ii.done_target = w.done_target;
             ii.E_k = w.E_k;
-            ii.energies = w.energies + (size_t)eb * EB;
+            ii.energies = w.energies + e_first;
             ii.inv2a = w.inv2a;
             ii.n_chan = w.n_chan;
             ii.n_poles = w.n_poles;
@@ -458,6 +656,8 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
             ii.col0 = col0;
             ii.nrb = (unsigned char)nrb;
             ii.tr = (unsigned char)w.tr;
+            ii.slab_T = (unsigned char)slab_T;
+            ii.slab_g = (unsigned char)slab_g;
             ii.nblk = nblk;
             ii.n_kt = n_kt;
           }
@@ -468,51 +668,72 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
         if (stop) break;
 
         const CUtensorMap *map = &w.map;
-        const int i_boxes = (nrb + TN / 8 - 1) / (TN / 8);     // I panel: one to four boxes of 32 rows
-        const uint32_t tx_bytes = (i_boxes + (kind != 0 ? 1 : 0)) * (w.tr ? TR_BOX_BYTES : BOX_BYTES);
+        if (BATCH && w.use_tma && p != last_wave) {
+          if (lane == 0) tensormap_acquire(map);
+          __syncwarp();
+          last_wave = p;
+        }
+        // panels of 32 channels to stage: I rows [row0, ...) into panels [0, i_boxes), J rows [col0, ...) into
+        // panels [j_panel0, j_panel0 + j_boxes); boxes that lie wholly beyond n_chan are not loaded (nothing reads them)
+        int i_boxes, j_boxes, j_panel0;
+        if (slab_T != 0) {
+          i_boxes = (min(slab_T, w.n_chan - row0) + TN - 1) / TN;
+          j_boxes = kind != 0 ? (min(slab_T, w.n_chan - col0) + TN - 1) / TN : 0;
+          j_panel0 = slab_T / TN;
+        } else {
+          i_boxes = (nrb + TN / 8 - 1) / (TN / 8);     // one to four boxes of 32 rows
+          j_boxes = kind != 0 ? 1 : 0;
+          j_panel0 = TW / TN;
+        }
+        const uint32_t box = w.tr ? TR_BOX_BYTES : BOX_BYTES;
+        const uint32_t tx_bytes = (uint32_t)(i_boxes + j_boxes) * box;
         // host-buffer call: W uploaded so far.  Slabs of channels are waited for here, once per item (the rows and
         // columns of its tile); slabs of poles stage by stage below.
         const unsigned int *rows_ready = w.rows_ready;
+        const unsigned long long timeout_ns = (unsigned long long)(w.wait_timeout_ms ? w.wait_timeout_ms : 2000u) * 1000000ULL;
         unsigned int rows_seen = rows_ready ? 0u : 0xffffffffu;
         if (rows_ready && w.ready_counts_channels) {
-          const int last = kind == 0 ? row0 + nrb * 8 : max(row0 + nrb * 8, col0 + nblk * 8);
-          wait_rows_uploaded(rows_ready, (unsigned int)min(last, w.n_chan), rows_seen, lane);
+          const int last = max(row0 + i_boxes * TN, kind != 0 ? col0 + j_boxes * TN : 0);
+          wait_rows_uploaded(rows_ready, (unsigned int)min(last, w.n_chan), rows_seen, w.abort_flag, timeout_ns, lane);
           rows_seen = 0xffffffffu;
         }
         if (w.use_tma) {
           // TMA box coordinates: (pole, channel) for pole-contiguous W, (channel, pole) for the H.DAT order
           const int tr = w.tr;
-          const uint32_t box = tr ? TR_BOX_BYTES : BOX_BYTES;
+          const bool keep = w.l2_keep != 0;
           for (int kt = 0; kt < n_kt; ++kt) {
             const int k0 = kt * KT;
-            wait_rows_uploaded(rows_ready, (unsigned int)min(k0 + KT, w.n_poles), rows_seen, lane);
-            mbar_wait(empty0 + 8 * ps.stage, ps.phase ^ 1u);
+            wait_rows_uploaded(rows_ready, (unsigned int)min(k0 + KT, w.n_poles), rows_seen, w.abort_flag, timeout_ns, lane);
+            mbar_wait(ps.empty(), ps.phase ^ 1u);
             if (lane == 0) {
-              const uint32_t full = full0 + 8 * ps.stage;
-              const uint32_t dst = smem_u32(smem + ps.stage * STAGE_BYTES);
+              const uint32_t full = ps.full();
+              const uint32_t dst = smem_u32(stages + (size_t)ps.stage * ps.stage_bytes) + D_BYTES;
               mbar_arrive_expect_tx(full, tx_bytes);
-              for (int b = 0; b < i_boxes; ++b)
-                tma_load_2d(dst + b * box, map, tr ? row0 + b * TN : k0, tr ? k0 : row0 + b * TN, full);
-              if (kind != 0) tma_load_2d(dst + (TW / TN) * box, map, tr ? col0 : k0, tr ? k0 : col0, full);
+              for (int b = 0; b < i_boxes + j_boxes; ++b) {
+                const int chan = b < i_boxes ? row0 + b * TN : col0 + (b - i_boxes) * TN;
+                const uint32_t d = dst + (uint32_t)(b < i_boxes ? b : j_panel0 + (b - i_boxes)) * box;
+                if (keep) tma_load_2d_hint(d, map, tr ? chan : k0, tr ? k0 : chan, full, keep_policy);
+                else tma_load_2d(d, map, tr ? chan : k0, tr ? k0 : chan, full);
+              }
             }
             ps.advance();
           }
         } else {
           for (int kt = 0; kt < n_kt; ++kt) {
             const int k0 = kt * KT;
-            wait_rows_uploaded(rows_ready, (unsigned int)min(k0 + KT, w.n_poles), rows_seen, lane);
-            mbar_wait(empty0 + 8 * ps.stage, ps.phase ^ 1u);
-            double *sd = reinterpret_cast<double *>(smem + ps.stage * STAGE_BYTES);
+            wait_rows_uploaded(rows_ready, (unsigned int)min(k0 + KT, w.n_poles), rows_seen, w.abort_flag, timeout_ns, lane);
+            mbar_wait(ps.empty(), ps.phase ^ 1u);
+            double *sd = reinterpret_cast<double *>(stages + (size_t)ps.stage * ps.stage_bytes) + D_DOUBLES;
             if (w.tr) {
-              for (int b = 0; b < i_boxes; ++b) stage_panel_plain_tr(sd + b * KT * TR_PITCH, w, row0 + b * TN, k0, lane);
-              if (kind != 0) stage_panel_plain_tr(sd + StageLayout<true>::J_BASE, w, col0, k0, lane);
+              for (int b = 0; b < i_boxes; ++b) stage_panel_plain_tr(sd + b * TR_BOX_DOUBLES, w, row0 + b * TN, k0, lane);
+              for (int b = 0; b < j_boxes; ++b) stage_panel_plain_tr(sd + (j_panel0 + b) * TR_BOX_DOUBLES, w, col0 + b * TN, k0, lane);
             } else {
               stage_panel_plain(sd, w, row0, i_boxes * TN, k0, lane);
-              if (kind != 0) stage_panel_plain(sd + StageLayout<false>::J_BASE, w, col0, TN, k0, lane);
+              if (j_boxes) stage_panel_plain(sd + j_panel0 * TN * KT, w, col0, j_boxes * TN, k0, lane);
             }
             __threadfence_block();   // all lanes' stores performed before lane 0 publishes the stage
             __syncwarp();
-            if (lane == 0) mbar_arrive(full0 + 8 * ps.stage);
+            if (lane == 0) mbar_arrive(ps.full());
             ps.advance();
           }
         }
@@ -532,7 +753,6 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
       constexpr int DW = PRODUCER_WARPS - 1;                 // 3 warps, 96 lanes
       constexpr int DT = (EB * KT + DW * 32 - 1) / (DW * 32);
       const int dl = (warp - EB - 1) * 32 + lane;
-      PipeState ps;
       uint32_t iq = 0, iphase = 0;
       for (;;) {
         mbar_wait(item_full0 + 8 * iq, iphase);
@@ -565,9 +785,8 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
             const int k = k0 + KT + kk[t];
             ek_next[t] = (ev[t] && k < it.n_poles) ? __ldg(it.E_k + k) : 0.0;
           }
-          mbar_wait(empty0 + 8 * ps.stage, ps.phase ^ 1u);
-          double *dsm = reinterpret_cast<double *>(smem + ps.stage * STAGE_BYTES) +
-                        (it.tr ? StageLayout<true>::D_BASE : StageLayout<false>::D_BASE);
+          mbar_wait(ps.empty(), ps.phase ^ 1u);
+          double *dsm = reinterpret_cast<double *>(stages + (size_t)ps.stage * ps.stage_bytes);   // d is first in a stage
 #pragma unroll
           for (int t = 0; t < DT; ++t) {
             // 0 beyond n_poles / n_E so that zero-filled W columns stay zero
@@ -577,22 +796,20 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
           }
           __threadfence_block();     // every lane's d has been written before lane 0 arrives
           __syncwarp();
-          if (lane == 0) mbar_arrive(full0 + 8 * ps.stage);
+          if (lane == 0) mbar_arrive(ps.full());
           ps.advance();
         }
       }
     }
   } else {
-    // ================= consumer warps: one energy of the block each =================
+    // ================= consumer warps =================
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(CONSUMER_REGS));
-    PipeState ps;
     uint32_t iq = 0, iphase = 0;
     for (;;) {
       mbar_wait(item_full0 + 8 * iq, iphase);
       const ItemInfo it = ring[iq];
       if (it.kind < 0) break;
-      if (warp >= it.n_valid_e) consume_idle(it.n_kt, ps, full0, empty0, lane);
-      else consume_item(it, smem, ps, full0, empty0, warp, lane);
+      consume_item(it, ps, warp, lane);
       if (it.done != nullptr) {
         // host-buffer call: the host copies a wave's R back as soon as its last item has been stored.  Every warp
         // makes its stores visible device-wide and counts itself in; the arrival that completes the wave raises
@@ -615,7 +832,8 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
 // ---- verification kernel: eq. 4 term by term, one thread per R element ----------------------
 __global__ void rmat_naive_kernel(const double *__restrict__ W, long long stride_n, long long stride_k,
                                   const double *__restrict__ E_k, const double *__restrict__ energies, int n_chan,
-                                  int n_poles, long long n_elems, double a, double *__restrict__ R_out) {
+                                  int n_poles, long long n_elems, double a, const double *__restrict__ diag_add,
+                                  double *__restrict__ R_out) {
   const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= n_elems) return;
   const long long cc = (long long)n_chan * n_chan;
@@ -631,7 +849,9 @@ __global__ void rmat_naive_kernel(const double *__restrict__ W, long long stride
     c = __dadd_rn(c, fabs(s) >= fabs(t) ? __dadd_rn(__dsub_rn(s, u), t) : __dadd_rn(__dsub_rn(t, u), s));
     s = u;
   }
-  R_out[idx] = __ddiv_rn(__dadd_rn(s, c), __dmul_rn(2.0, a));
+  double r = __ddiv_rn(__dadd_rn(s, c), __dmul_rn(2.0, a));
+  if (diag_add != nullptr && n == m) r = __dadd_rn(r, diag_add[e * n_chan + n]);
+  R_out[idx] = r;
 }
 
 }  // namespace pstgf

@@ -181,6 +181,10 @@ _CONFIGS = {
     # Hamiltonian size of 106 661" (neutral Fe).  W is 6.2 GB, R 422 MB per energy.
     6: dict(seed=5, P=1, C=7261, K=106661, N=16, a=30.0, sigma=0.03, poles=(-30.0, 2000.0), mesh=(0.01, 10.0),
             kind="linear"),
+    # Not in BASELINE.json: many small partial waves in one call (PAPER.md:676 runs 42 partial waves of at most
+    # 1818 channels, the low-L ones with few channels): 256 waves, n_chan uniform in [8, 32], config 4's recipe.
+    7: dict(seed=6, P=256, C=None, C_range=(8, 33), N=512, a=25.0, sigma=0.05, poles=(-20.0, 300.0), mesh=(0.01, 50.0),
+            kind="geometric"),
 }
 POLES_PER_CHANNEL = 20
 PAPER_SCALE_CONFIG = 6
@@ -190,14 +194,19 @@ def _n_poles(c: dict, n_chan: int) -> int:
     return int(c["K"]) if "K" in c else POLES_PER_CHANNEL * n_chan
 
 
+def _draw_channels(c: dict, rng: np.random.Generator) -> list[int]:
+    """n_chan of every wave: fixed, or drawn first (reading R12) from integers(lo, hi)."""
+    if c["C"] is None:
+        lo, hi = c.get("C_range", (16, 401))
+        return [int(x) for x in rng.integers(lo, hi, size=c["P"])]
+    return [c["C"]] * c["P"]
+
+
 def config_shapes(cfg: int, seed: int | None = None) -> list[tuple[int, int, int]]:
     """(n_chan, n_poles, n_E) per wave without drawing W (cheap; for planning)."""
     c = _CONFIGS[cfg]
     rng = np.random.default_rng(c["seed"] if seed is None else seed)
-    if c["C"] is None:
-        chans = [int(x) for x in rng.integers(16, 401, size=c["P"])]
-    else:
-        chans = [c["C"]] * c["P"]
+    chans = _draw_channels(c, rng)
     return [(n, _n_poles(c, n), c["N"]) for n in chans]
 
 
@@ -212,10 +221,7 @@ def make_config(cfg: int, seed: int | None = None, n_E: int | None = None) -> Wo
     s = c["seed"] if seed is None else seed
     rng = np.random.default_rng(s)
     N = c["N"] if n_E is None else int(n_E)
-    if c["C"] is None:
-        chans = [int(x) for x in rng.integers(16, 401, size=c["P"])]
-    else:
-        chans = [c["C"]] * c["P"]
+    chans = _draw_channels(c, rng)
     drawn = [_draw_wave(rng, n, _n_poles(c, n), c["sigma"], *c["poles"]) for n in chans]
     mesh_fn = linear_mesh if c["kind"] == "linear" else geometric_mesh
     mesh = mesh_fn(c["mesh"][0], c["mesh"][1], N)

@@ -1,4 +1,5 @@
-// fp64_probe.cu -- register-resident FP64 throughput probes (include/pstgf_rmat.h, "measurement").
+// fp64_probe.cu -- register-resident FP64 throughput probes: libpstgf_probe.so, a MEASUREMENT utility that
+// bench.py loads beside the product library (it is not part of libpstgf_rmat.so and shares no code with it).
 //
 // MEASURED_PEAKS.json carries no FP64 entry, so the roofline denominator of the DMMA SYRK kernel
 // is measured with these: kind 0 issues DMMA.8x8x4 (mma.sync m8n8k4 f64) in the register-tile
@@ -7,7 +8,6 @@
 // folds away, and the accumulators are written to `sink` at the end.
 #include <cuda_runtime.h>
 
-#include "../../include/pstgf_rmat.h"
 
 namespace {
 
@@ -62,15 +62,20 @@ __global__ void __launch_bounds__(256) probe_kernel(int iters, double *sink) {
 
 }  // namespace
 
-extern "C" pstgf_status_t pstgf_fp64_probe(int kind, int iters, int blocks, int threads, double *sink,
-                                           double *flop_out, void *stream) {
+// kind 0 = DMMA.8x8x4 (the instruction the SYRK kernel issues, in its register-tile pattern), 1 = DFMA, 2 = DMMA on
+// even warps and DFMA on odd warps.  Launches `blocks` CTAs of `threads` threads (multiple of 32, <= 256) that each
+// run `iters` iterations; DEVICE `sink` receives blocks*threads doubles.  HOST `flop_out` (may be NULL) receives
+// the FLOPs the launch performs (2 per FMA).  Asynchronous on `stream` (a cudaStream_t): time it with events.
+// Returns 0, 1 on bad arguments, 5 when the launch fails.
+extern "C" int pstgf_fp64_probe(int kind, int iters, int blocks, int threads, double *sink, double *flop_out,
+                                void *stream) {
   if (kind < 0 || kind > 2 || iters < 0 || blocks <= 0 || threads <= 0 || threads > 256 || threads % 32 != 0 || !sink)
-    return PSTGF_ERR_INVALID_VALUE;
+    return 1;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   if (kind == 0) probe_kernel<0><<<blocks, threads, 0, s>>>(iters, sink);
   else if (kind == 1) probe_kernel<1><<<blocks, threads, 0, s>>>(iters, sink);
   else probe_kernel<2><<<blocks, threads, 0, s>>>(iters, sink);
-  if (cudaGetLastError() != cudaSuccess) return PSTGF_ERR_CUDA;
+  if (cudaGetLastError() != cudaSuccess) return 5;
   if (flop_out) {
     const double warps = (double)blocks * (threads / 32);
     const double per_dmma_warp = (double)iters * 32.0 * 512.0;        // 32 DMMA.8x8x4 (256 FMA each) per iteration
@@ -78,5 +83,5 @@ extern "C" pstgf_status_t pstgf_fp64_probe(int kind, int iters, int blocks, int 
     const double even = (double)blocks * ((threads / 32 + 1) / 2), odd = warps - even;
     *flop_out = kind == 0 ? warps * per_dmma_warp : kind == 1 ? warps * per_dfma_warp : even * per_dmma_warp + odd * per_dfma_warp;
   }
-  return PSTGF_OK;
+  return 0;
 }

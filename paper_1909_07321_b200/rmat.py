@@ -17,12 +17,15 @@ PSTGF_OK = 0
 PSTGF_TAIL_AUTO, PSTGF_TAIL_NONE, PSTGF_TAIL_ALL = 0, 1, 2
 PSTGF_W_POLE_CONTIGUOUS, PSTGF_W_CHANNEL_CONTIGUOUS = 0, 1
 PSTGF_HOST_PIPELINE_AUTO, PSTGF_HOST_PIPELINE_CHUNKED = 0, 1
-_STATUS_NAMES = {0: "PSTGF_OK", 1: "PSTGF_ERR_INVALID_VALUE", 2: "PSTGF_ERR_ALIGNMENT", 3: "PSTGF_ERR_WORKSPACE",
-                 4: "PSTGF_ERR_UNSUPPORTED_DEVICE", 5: "PSTGF_ERR_CUDA"}
+PSTGF_SLAB_AUTO, PSTGF_SLAB_NONE, PSTGF_SLAB_T32, PSTGF_SLAB_T64, PSTGF_SLAB_T128 = 0, 1, 2, 3, 4
+PSTGF_ERR_TIMEOUT, PSTGF_ERR_CAPTURE = 6, 7
+PSTGF_RMAT_VERSION = 200            # must equal include/pstgf_rmat.h; load() checks it against the library
 
-EXPORTS = ["pstgf_rmat_form", "pstgf_rmat_form_hdat", "pstgf_rmat_batch_workspace_bytes", "pstgf_rmat_form_batch", "pstgf_rmat_form_naive",
-           "pstgf_rmat_form_batch_host", "pstgf_rmat_set_tail_policy", "pstgf_rmat_set_host_pipeline", "pstgf_fp64_probe", "pstgf_last_launch_count", "pstgf_status_string", "pstgf_last_cuda_error",
-           "pstgf_version"]
+EXPORTS = ["pstgf_rmat_form", "pstgf_rmat_form_hdat", "pstgf_rmat_batch_workspace_bytes", "pstgf_rmat_form_batch",
+           "pstgf_rmat_form_naive", "pstgf_rmat_form_batch_host", "pstgf_mesh_from_zscaled", "pstgf_rmat_finalize",
+           "pstgf_debug_set_tail_policy", "pstgf_debug_set_slab_policy", "pstgf_debug_set_host_pipeline",
+           "pstgf_debug_set_upload_timeout_ms", "pstgf_debug_stall_upload", "pstgf_last_launch_count",
+           "pstgf_status_string", "pstgf_last_cuda_error", "pstgf_version"]
 
 
 class PstgfError(RuntimeError):
@@ -35,7 +38,7 @@ class pstgf_wave_t(ctypes.Structure):
     _fields_ = [("n_chan", ctypes.c_int), ("n_poles", ctypes.c_int), ("n_E", ctypes.c_int), ("w_layout", ctypes.c_int),
                 ("ldw", ctypes.c_longlong), ("a", ctypes.c_double),
                 ("W", ctypes.c_void_p), ("E_k", ctypes.c_void_p), ("energies", ctypes.c_void_p),
-                ("R_out", ctypes.c_void_p)]
+                ("R_out", ctypes.c_void_p), ("diag_add", ctypes.c_void_p)]
 
 
 _lib = None
@@ -46,24 +49,29 @@ def library_path() -> str:
 
 
 def load(build_if_missing: bool = False):
-    """Load libpstgf_rmat.so (built in-tree).  Raises if it is not there: no fallback exists."""
+    """Load libpstgf_rmat.so (built in-tree).  Raises if it is not there, older than its sources, or of another
+    ABI version than this binding: no fallback exists."""
     global _lib
     if _lib is not None:
         return _lib
     path = library_path()
-    if not os.path.exists(path):
+    if not os.path.exists(path) or _build.is_stale():
         if build_if_missing:
             _build.build()
         else:
-            raise PstgfError(-1, f"{path} is missing: run `python -m paper_1909_07321_b200.build` "
+            what = "is missing" if not os.path.exists(path) else "was built from other sources than csrc/ and include/pstgf_rmat.h now hold"
+            raise PstgfError(-1, f"{path} {what}: run `python -m paper_1909_07321_b200.build` "
                                  "(or __graft_entry__.build()); there is no CPU fallback")
     lib = ctypes.CDLL(path)
+    lib.pstgf_version.restype = ctypes.c_int
+    if int(lib.pstgf_version()) != PSTGF_RMAT_VERSION:
+        raise PstgfError(-1, f"{path} reports ABI version {lib.pstgf_version()}, this binding is for {PSTGF_RMAT_VERSION}: rebuild")
     vp, ll, i, d, sz = ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
     lib.pstgf_rmat_form.argtypes = [vp, ll, vp, vp, i, i, i, d, vp, vp]
     lib.pstgf_rmat_form.restype = i
     lib.pstgf_rmat_form_hdat.argtypes = [vp, ll, vp, vp, i, i, i, d, vp, vp]
     lib.pstgf_rmat_form_hdat.restype = i
-    lib.pstgf_rmat_form_naive.argtypes = [vp, ll, vp, vp, i, i, i, d, vp, i, vp]
+    lib.pstgf_rmat_form_naive.argtypes = [ctypes.POINTER(pstgf_wave_t), vp]
     lib.pstgf_rmat_form_naive.restype = i
     lib.pstgf_rmat_batch_workspace_bytes.argtypes = [ctypes.POINTER(pstgf_wave_t), i]
     lib.pstgf_rmat_batch_workspace_bytes.restype = sz
@@ -71,12 +79,16 @@ def load(build_if_missing: bool = False):
     lib.pstgf_rmat_form_batch.restype = i
     lib.pstgf_rmat_form_batch_host.argtypes = [ctypes.POINTER(pstgf_wave_t), i, sz, vp]
     lib.pstgf_rmat_form_batch_host.restype = i
-    lib.pstgf_rmat_set_tail_policy.argtypes = [i]
-    lib.pstgf_rmat_set_tail_policy.restype = i
-    lib.pstgf_rmat_set_host_pipeline.argtypes = [i]
-    lib.pstgf_rmat_set_host_pipeline.restype = i
-    lib.pstgf_fp64_probe.argtypes = [i, i, i, i, vp, ctypes.POINTER(d), vp]
-    lib.pstgf_fp64_probe.restype = i
+    for name in ("pstgf_debug_set_tail_policy", "pstgf_debug_set_slab_policy", "pstgf_debug_set_host_pipeline",
+                 "pstgf_debug_stall_upload"):
+        getattr(lib, name).argtypes = [i]
+        getattr(lib, name).restype = i
+    lib.pstgf_debug_set_upload_timeout_ms.argtypes = [ctypes.c_uint]
+    lib.pstgf_debug_set_upload_timeout_ms.restype = i
+    lib.pstgf_mesh_from_zscaled.argtypes = [vp, ll, d, vp]
+    lib.pstgf_mesh_from_zscaled.restype = i
+    lib.pstgf_rmat_finalize.argtypes = []
+    lib.pstgf_rmat_finalize.restype = i
     lib.pstgf_last_launch_count.restype = i
     lib.pstgf_status_string.argtypes = [i]
     lib.pstgf_status_string.restype = ctypes.c_char_p
@@ -117,7 +129,7 @@ def _w_dims(W, layout: int):
     return (cols, rows, ldw) if layout == PSTGF_W_CHANNEL_CONTIGUOUS else (rows, cols, ldw)
 
 
-def _wave_struct(W, E_k, energies, a, R_out, layout: int = PSTGF_W_POLE_CONTIGUOUS) -> pstgf_wave_t:
+def _wave_struct(W, E_k, energies, a, R_out, layout: int = PSTGF_W_POLE_CONTIGUOUS, diag_add=None) -> pstgf_wave_t:
     _dev_f64(W, "W"); _dev_f64(E_k, "E_k"); _dev_f64(energies, "energies"); _dev_f64(R_out, "R_out")
     n_chan, n_poles, ldw = _w_dims(W, layout)
     n_E = int(energies.shape[0])
@@ -127,8 +139,12 @@ def _wave_struct(W, E_k, energies, a, R_out, layout: int = PSTGF_W_POLE_CONTIGUO
         raise ValueError("energies must be contiguous [n_E]")
     if tuple(R_out.shape) != (n_E, n_chan, n_chan) or not R_out.is_contiguous():
         raise ValueError("R_out must be contiguous [n_E, n_chan, n_chan]")
+    if diag_add is not None:
+        _dev_f64(diag_add, "diag_add")
+        if tuple(diag_add.shape) != (n_E, n_chan) or not diag_add.is_contiguous():
+            raise ValueError("diag_add must be contiguous [n_E, n_chan]")
     return pstgf_wave_t(n_chan, n_poles, n_E, int(layout), ldw, float(a), W.data_ptr(), E_k.data_ptr(),
-                        energies.data_ptr(), R_out.data_ptr())
+                        energies.data_ptr(), R_out.data_ptr(), diag_add.data_ptr() if diag_add is not None else None)
 
 
 def pstgf_rmat_form(W, E_k, energies, a: float, R_out=None, stream=None) -> torch.Tensor:
@@ -160,21 +176,20 @@ def pstgf_rmat_form_hdat(Wt, E_k, energies, a: float, R_out=None, stream=None) -
 
 
 def pstgf_rmat_form_naive(W, E_k, energies, a: float, R_out=None, stream=None,
-                          layout: int = PSTGF_W_POLE_CONTIGUOUS) -> torch.Tensor:
+                          layout: int = PSTGF_W_POLE_CONTIGUOUS, diag_add=None) -> torch.Tensor:
     """Same result from the library's term-by-term verification kernel (slow)."""
     lib = load()
     n_chan = W.shape[1] if layout == PSTGF_W_CHANNEL_CONTIGUOUS else W.shape[0]
     if R_out is None:
         R_out = torch.empty((energies.shape[0], n_chan, n_chan), dtype=torch.float64, device=W.device)
-    w = _wave_struct(W, E_k, energies, a, R_out, layout)
+    w = _wave_struct(W, E_k, energies, a, R_out, layout, diag_add)
     with torch.cuda.device(W.device):
-        _check(lib.pstgf_rmat_form_naive(w.W, w.ldw, w.E_k, w.energies, w.n_chan, w.n_poles, w.n_E, w.a, w.R_out,
-                                         int(layout), _stream_ptr(stream)))
+        _check(lib.pstgf_rmat_form_naive(ctypes.byref(w), _stream_ptr(stream)))
     return R_out
 
 
 def make_wave_array(waves: Sequence[tuple]) -> "ctypes.Array[pstgf_wave_t]":
-    """waves: sequence of (W, E_k, energies, a, R_out[, w_layout]) tuples of CUDA tensors."""
+    """waves: sequence of (W, E_k, energies, a, R_out[, w_layout[, diag_add]]) tuples of CUDA tensors."""
     arr = (pstgf_wave_t * len(waves))()
     for p, wv in enumerate(waves):
         arr[p] = _wave_struct(*wv)
@@ -198,42 +213,58 @@ def pstgf_rmat_form_batch(wave_array, workspace: torch.Tensor, stream=None, n_wa
 
 
 def pstgf_rmat_form_batch_host(host_waves: Sequence[tuple], max_chunk_bytes: int = 0, stream=None) -> None:
-    """End-to-end call over HOST tensors (pinned recommended): (W, E_k, energies, a, R_out[, w_layout]) per wave,
-    all CPU float64 contiguous tensors; R_out is filled on return (the call synchronises)."""
+    """End-to-end call over HOST tensors (pinned recommended): (W, E_k, energies, a, R_out[, w_layout[, diag_add]])
+    per wave, all CPU float64 contiguous tensors; R_out is filled on return (the call synchronises)."""
     lib = load()
     arr = (pstgf_wave_t * len(host_waves))()
     for p, wv in enumerate(host_waves):
         W, E_k, energies, a, R_out = wv[:5]
         layout = int(wv[5]) if len(wv) > 5 else PSTGF_W_POLE_CONTIGUOUS
-        for t, nm in ((W, "W"), (E_k, "E_k"), (energies, "energies"), (R_out, "R_out")):
-            if t.dtype != torch.float64 or t.is_cuda or not t.is_contiguous():
+        diag_add = wv[6] if len(wv) > 6 else None
+        for t, nm in ((W, "W"), (E_k, "E_k"), (energies, "energies"), (R_out, "R_out"), (diag_add, "diag_add")):
+            if t is not None and (t.dtype != torch.float64 or t.is_cuda or not t.is_contiguous()):
                 raise TypeError(f"{nm} must be a contiguous CPU float64 tensor")
         n_chan, n_poles, ldw = _w_dims(W, layout)
         arr[p] = pstgf_wave_t(n_chan, n_poles, int(energies.shape[0]), layout, ldw, float(a), W.data_ptr(), E_k.data_ptr(),
-                              energies.data_ptr(), R_out.data_ptr())
+                              energies.data_ptr(), R_out.data_ptr(), diag_add.data_ptr() if diag_add is not None else None)
     _check(lib.pstgf_rmat_form_batch_host(arr, len(host_waves), int(max_chunk_bytes), _stream_ptr(stream)))
 
 
-def pstgf_rmat_set_tail_policy(policy: int) -> None:
-    """Scheduling knob: PSTGF_TAIL_AUTO / PSTGF_TAIL_NONE / PSTGF_TAIL_ALL (results are bitwise the same)."""
-    _check(load().pstgf_rmat_set_tail_policy(int(policy)))
+def pstgf_debug_set_tail_policy(policy: int) -> None:
+    """Thread-local scheduling knob: PSTGF_TAIL_AUTO / PSTGF_TAIL_NONE / PSTGF_TAIL_ALL (results are bitwise the same)."""
+    _check(load().pstgf_debug_set_tail_policy(int(policy)))
 
 
-def pstgf_rmat_set_host_pipeline(mode: int) -> None:
-    """PSTGF_HOST_PIPELINE_AUTO (signalled single launch) or PSTGF_HOST_PIPELINE_CHUNKED (one launch per piece)."""
-    _check(load().pstgf_rmat_set_host_pipeline(int(mode)))
+def pstgf_debug_set_slab_policy(policy: int) -> None:
+    """Thread-local: how the n_E mod 8 energies are cut (PSTGF_SLAB_AUTO / _NONE / _T32 / _T64 / _T128); same bits."""
+    _check(load().pstgf_debug_set_slab_policy(int(policy)))
 
 
-def pstgf_fp64_probe(kind: int, iters: int, blocks: int, threads: int, sink: torch.Tensor, stream=None) -> float:
-    """Enqueue the FP64 throughput probe (0 DMMA, 1 DFMA, 2 both); returns the FLOPs of the launch."""
-    lib = load()
-    if sink.dtype != torch.float64 or not sink.is_cuda or sink.numel() < blocks * threads:
-        raise ValueError("sink must be a CUDA float64 tensor of at least blocks*threads elements")
-    flop = d_ = ctypes.c_double(0.0)
-    with torch.cuda.device(sink.device):
-        _check(lib.pstgf_fp64_probe(int(kind), int(iters), int(blocks), int(threads), sink.data_ptr(),
-                                    ctypes.byref(flop), _stream_ptr(stream)))
-    return float(d_.value)
+def pstgf_debug_set_host_pipeline(mode: int) -> None:
+    """Thread-local: PSTGF_HOST_PIPELINE_AUTO (signalled single launch) or PSTGF_HOST_PIPELINE_CHUNKED (one launch per piece)."""
+    _check(load().pstgf_debug_set_host_pipeline(int(mode)))
+
+
+def pstgf_debug_set_upload_timeout_ms(ms: int) -> None:
+    _check(load().pstgf_debug_set_upload_timeout_ms(int(ms)))
+
+
+def pstgf_debug_stall_upload(on: bool) -> None:
+    _check(load().pstgf_debug_stall_upload(1 if on else 0))
+
+
+def pstgf_mesh_from_zscaled(e_scaled, z: float):
+    """E = z^2 * E_scaled for a HOST float64 array (numpy or CPU tensor): PAPER.md:431, :503."""
+    import numpy as np
+    src = np.ascontiguousarray(e_scaled.numpy() if isinstance(e_scaled, torch.Tensor) else e_scaled, dtype=np.float64)
+    out = np.empty_like(src)
+    _check(load().pstgf_mesh_from_zscaled(src.ctypes.data, src.size, float(z), out.ctypes.data))
+    return out
+
+
+def pstgf_rmat_finalize() -> None:
+    """Free everything the library keeps between calls (it may be used again afterwards)."""
+    _check(load().pstgf_rmat_finalize())
 
 
 def pstgf_last_launch_count() -> int:

@@ -53,7 +53,7 @@ def test_header_compiles_as_plain_c(tmp_path):
     """The boundary is C: no C++ or torch types in the signatures."""
     c = tmp_path / "use_header.c"
     c.write_text('#include "pstgf_rmat.h"\n'
-                 "int main(void) { pstgf_wave_t w; (void)w; return sizeof(pstgf_wave_t) == 64 ? 0 : 1; }\n")
+                 "int main(void) { pstgf_wave_t w; (void)w; return sizeof(pstgf_wave_t) == 72 ? 0 : 1; }\n")
     exe = tmp_path / "use_header"
     subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-pedantic", "-I", os.path.join(ROOT, "include"),
                     str(c), "-o", str(exe)], check=True)
@@ -62,10 +62,12 @@ def test_header_compiles_as_plain_c(tmp_path):
 
 def test_wave_struct_layout_matches_binding():
     from paper_1909_07321_b200 import rmat
-    assert ctypes.sizeof(rmat.pstgf_wave_t) == 64
+    assert ctypes.sizeof(rmat.pstgf_wave_t) == 72
     off = {n: getattr(rmat.pstgf_wave_t, n).offset for n, _ in rmat.pstgf_wave_t._fields_}
     assert off == {"n_chan": 0, "n_poles": 4, "n_E": 8, "w_layout": 12, "ldw": 16, "a": 24, "W": 32, "E_k": 40, "energies": 48,
-                   "R_out": 56}
+                   "R_out": 56, "diag_add": 64}
+    m = re.search(r"#define\s+PSTGF_RMAT_VERSION\s+(\d+)", open(HEADER).read())
+    assert rmat.PSTGF_RMAT_VERSION == int(m.group(1))
 
 
 def test_version_and_status_strings(lib):
@@ -75,7 +77,7 @@ def test_version_and_status_strings(lib):
     m = re.search(r"#define\s+PSTGF_RMAT_VERSION\s+(\d+)", open(HEADER).read())
     assert lib.pstgf_version() == int(m.group(1))
     seen = set()
-    for code in range(6):
+    for code in range(8):
         s = lib.pstgf_status_string(code).decode()
         assert s and s not in seen
         seen.add(s)
@@ -100,13 +102,60 @@ def test_argument_errors_need_no_device(lib):
     lib.pstgf_rmat_form_hdat.restype = i
     assert lib.pstgf_rmat_form_hdat(fake, 3, fake, fake, 4, 6, 1, 20.0, fake, None) == 1   # ldw < n_chan
     assert lib.pstgf_rmat_form_hdat(fake, 4, fake, fake, 4, 6, 0, 20.0, fake, None) == 0   # n_E == 0
-    lib.pstgf_rmat_form_naive.argtypes = [vp, ll, vp, vp, i, i, i, d, vp, i, vp]
+    from paper_1909_07321_b200 import rmat
+    lib.pstgf_rmat_form_naive.argtypes = [ctypes.POINTER(rmat.pstgf_wave_t), vp]
     lib.pstgf_rmat_form_naive.restype = i
-    assert lib.pstgf_rmat_form_naive(fake, 6, fake, fake, 4, 6, 1, 20.0, fake, 7, None) == 1   # unknown w_layout
-    lib.pstgf_rmat_set_tail_policy.argtypes = [i]
-    lib.pstgf_rmat_set_tail_policy.restype = i
-    assert lib.pstgf_rmat_set_tail_policy(5) == 1
-    assert lib.pstgf_rmat_set_tail_policy(0) == 0
+    w = rmat.pstgf_wave_t(4, 6, 1, 7, 6, 20.0, fake, fake, fake, fake, None)
+    assert lib.pstgf_rmat_form_naive(ctypes.byref(w), None) == 1                        # unknown w_layout
+    w.w_layout, w.diag_add = 0, fake + 4
+    assert lib.pstgf_rmat_form_naive(ctypes.byref(w), None) == 2                        # misaligned diag_add
+    assert lib.pstgf_rmat_form_naive(None, None) == 1
+    for name, bad in (("pstgf_debug_set_tail_policy", 5), ("pstgf_debug_set_slab_policy", 9),
+                      ("pstgf_debug_set_host_pipeline", 3)):
+        f = getattr(lib, name)
+        f.argtypes, f.restype = [i], i
+        assert f(bad) == 1 and f(0) == 0
+
+
+def test_product_library_holds_no_measurement_code(lib):
+    """The FP64 throughput probe that fixes the roofline denominator is bench-side (libpstgf_probe.so): neither the
+    product header nor the product library knows it."""
+    assert "probe" not in open(HEADER).read()
+    assert not hasattr(lib, "pstgf_fp64_probe")
+    from paper_1909_07321_b200 import build
+    assert hasattr(ctypes.CDLL(build.PROBE_LIB), "pstgf_fp64_probe")
+
+
+def test_mesh_from_zscaled(lib):
+    """input meshes are z-scaled, E/z^2.  Exact dyadic cases, aliasing, argument errors."""
+    import numpy as np
+    from paper_1909_07321_b200 import rmat
+    e = np.array([0.0, 0.5, 1.0, -0.25, 3.0, 2.0 ** -40])
+    for z in (1.0, 2.0, 3.0, 26.0, 0.5):
+        out = rmat.pstgf_mesh_from_zscaled(e, z)
+        assert np.array_equal(out, e * (z * z))              # exact: z*z and every product are representable here
+        assert np.array_equal(out / (z * z), e)              # and E/z^2 gives the input back (PAPER.md:431)
+    rng = np.random.default_rng(3)
+    x = rng.uniform(0.0, 5.0, 1000)
+    out = rmat.pstgf_mesh_from_zscaled(x, 7.0)
+    assert np.array_equal(out, x * 49.0)                     # one rounding per element, as documented
+    vp, ll, d = ctypes.c_void_p, ctypes.c_longlong, ctypes.c_double
+    f = lib.pstgf_mesh_from_zscaled
+    f.argtypes, f.restype = [vp, ll, d, vp], ctypes.c_int
+    buf = np.array([1.0, 2.0])
+    assert f(buf.ctypes.data, 2, 3.0, buf.ctypes.data) == 0  # in place
+    assert np.array_equal(buf, [9.0, 18.0])
+    assert f(buf.ctypes.data, 2, 0.0, buf.ctypes.data) == 1  # z must be > 0
+    assert f(buf.ctypes.data, 2, float("nan"), buf.ctypes.data) == 1
+    assert f(buf.ctypes.data, -1, 1.0, buf.ctypes.data) == 1
+    assert f(None, 2, 1.0, buf.ctypes.data) == 1
+    assert f(None, 0, 1.0, None) == 0
+
+
+def test_finalize_without_a_device_is_harmless(lib):
+    lib.pstgf_rmat_finalize.restype = ctypes.c_int
+    assert lib.pstgf_rmat_finalize() == 0
+    assert lib.pstgf_rmat_finalize() == 0
 
 
 def test_no_device_is_an_error_not_a_fallback(lib):

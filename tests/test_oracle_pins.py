@@ -300,3 +300,66 @@ def test_entries_agree_with_dense_and_exact(oracle):
     with pytest.raises(ValueError):
         oracle.rmat_entries(W, E_k, en, 20.0, [0], [0], [C])
     assert oracle.rmat_entries(W, E_k, en, 20.0, [], [], []).shape == (0,)
+
+
+# ---- the leading dimension: W as a column slice of a wider array (ldw > n_poles) ------------------------------
+def test_leading_dimension_is_honoured(oracle):
+    """W handed over with a row stride larger than n_poles (the C routine's ldw): exact rational brute force on
+    the strided array, and bitwise the compact copy's result.  The padding holds poison (NaN) so that a stride or
+    bound bug (reading column n_poles, or row n with pitch n_poles) cannot go unseen."""
+    rng = np.random.default_rng(77)
+    C, K, N, pad = 4, 6, 3, 5
+    wide = np.full((C, K + pad), np.nan)
+    wide[:, :K] = rng.uniform(-1.0, 1.0, (C, K))
+    Wv = wide[:, :K]
+    assert Wv.strides[0] == (K + pad) * 8 and not Wv.flags.c_contiguous
+    E_k = np.sort(rng.uniform(-2.0, 6.0, K))
+    en = np.array([-3.0, 1.234, 7.5])
+    R = oracle.rmat_form(Wv, E_k, en, 3.0)
+    assert np.all(np.isfinite(R))
+    exact = _exact_eq4(np.ascontiguousarray(Wv), E_k, en, 3.0)
+    Wc = np.ascontiguousarray(Wv)
+    for e, E in enumerate(en):          # same bound as test_exact_rational_brute_force: relative to sum |terms|
+        bound = (np.abs(Wc)[:, None, :] * np.abs(Wc)[None, :, :] / np.abs(E_k - E)).sum(-1) / (2 * 3.0)
+        assert np.all(np.abs(R[e] - exact[e]) <= 4 * np.finfo(float).eps * bound)
+    assert np.array_equal(R, oracle.rmat_form(np.ascontiguousarray(Wv), E_k, en, 3.0))
+    # the entry-by-entry routine needs a compact W and says so
+    with pytest.raises(ValueError):
+        oracle.rmat_entries(Wv, E_k, en, 3.0, [0], [0], [0])
+
+
+# ---- the diagonal addend (where a caller's Buttle correction goes; PAPER.md:524-528, :544) -------------------
+def test_diag_add_exact_and_local(oracle):
+    """R[e][n][n] = eq. 4 + diag_add[e][n]: exact rational brute force including the addend; a zero addend is
+    bitwise the plain result; off-diagonal entries are bitwise untouched; the addend enters once, after the 1/(2a)
+    (a -> 2a halves eq. 4's part only), on the right energy and channel (an addend that is non-zero in one slot)."""
+    rng = np.random.default_rng(91)
+    C, K, N, a = 3, 5, 4, 2.0
+    W = rng.uniform(-1.0, 1.0, (C, K))
+    E_k = np.sort(rng.uniform(-2.0, 6.0, K))
+    en = np.array([-3.0, 0.77, 2.5, 9.0])
+    da = rng.uniform(-0.5, 0.5, (N, C))
+    plain = oracle.rmat_form(W, E_k, en, a)
+    R = oracle.rmat_form(W, E_k, en, a, diag_add=da)
+    assert np.array_equal(plain, oracle.rmat_form(W, E_k, en, a, diag_add=np.zeros((N, C))))
+    off = ~np.eye(C, dtype=bool)
+    assert np.array_equal(R[:, off], plain[:, off])
+    # exact: (sum / 2a) + addend in rationals, rounded once; the oracle rounds twice (eq. 4, then the add): <= 1 ulp more
+    for e in range(N):
+        for n in range(C):
+            s = sum(Fraction(float(W[n, k])) ** 2 / (Fraction(float(E_k[k])) - Fraction(float(en[e]))) for k in range(K))
+            exact = float(s / (2 * Fraction(a)) + Fraction(float(da[e, n])))
+            assert abs(R[e, n, n] - exact) <= 3 * np.spacing(max(abs(exact), abs(plain[e, n, n]), abs(da[e, n])))
+            assert R[e, n, n] == plain[e, n, n] + da[e, n]            # one rounded add, after the division by 2a
+    # where a and the addend enter: doubling a halves eq. 4's part and leaves the addend alone
+    R2 = oracle.rmat_form(W, E_k, en, 2 * a, diag_add=da)
+    idx = np.arange(C)
+    assert np.array_equal(R2[:, idx, idx], plain[:, idx, idx] / 2 + da)
+    # locality: one non-zero slot moves exactly one entry
+    one = np.zeros((N, C))
+    one[2, 1] = 0.125
+    R1 = oracle.rmat_form(W, E_k, en, a, diag_add=one)
+    diff = R1 != plain
+    assert diff.sum() == 1 and diff[2, 1, 1]
+    with pytest.raises(ValueError):
+        oracle.rmat_form(W, E_k, en, a, diag_add=np.zeros((C, N)))   # transposed shape is rejected

@@ -96,9 +96,9 @@ EDGE_SHAPES = [
 def tail_policy(rmat):
     """Sets the scheduling knob for one test and restores the default afterwards."""
     def set_policy(policy):
-        rmat.pstgf_rmat_set_tail_policy(policy)
+        rmat.pstgf_debug_set_tail_policy(policy)
     yield set_policy
-    rmat.pstgf_rmat_set_tail_policy(rmat.PSTGF_TAIL_AUTO)
+    rmat.pstgf_debug_set_tail_policy(rmat.PSTGF_TAIL_AUTO)
 
 
 @pytest.mark.parametrize("C,K,N", EDGE_SHAPES)
@@ -136,6 +136,266 @@ def test_tail_split_inside_a_wave(rmat, oracle, tail_policy):
     Rs = _form_batch(rmat, [w, w2])
     assert np.array_equal(R, Rs[0].cpu().numpy())
     _check(Rs[1].cpu().numpy(), oracle.rmat_form(w2.W, w2.E_k, w2.energies, w2.a, threads=_threads()))
+
+
+# ---- few energies: slab items (the eight warps share one or two energies and split the tile) ---------------
+@pytest.fixture
+def slab_policy(rmat):
+    def set_policy(policy):
+        rmat.pstgf_debug_set_slab_policy(policy)
+    yield set_policy
+    rmat.pstgf_debug_set_slab_policy(rmat.PSTGF_SLAB_AUTO)
+
+
+FEW_ENERGY_SHAPES = [(1, 3, 1), (7, 40, 2), (8, 21, 3), (9, 19, 1), (15, 60, 5), (16, 33, 7), (31, 45, 1), (33, 45, 3),
+                     (63, 100, 2), (64, 80, 6), (65, 61, 5), (96, 40, 4), (127, 33, 1), (129, 41, 3), (200, 104, 7),
+                     (257, 50, 2), (300, 64, 1)]
+
+
+@pytest.mark.parametrize("C,K,N", FEW_ENERGY_SHAPES)
+def test_few_energies_match_full_blocks(rmat, oracle, slab_policy, C, K, N):
+    """PSTGF forms R once per (wave, energy): calls with n_E < 8.  Every slab tile edge
+    (32, 64, 128: all per-warp register tiles, diagonal and ragged edge tiles), both memory orders of W, the
+    single-wave and the batch call: <= 1e-13 against the oracle, and bitwise equal to the same energies computed
+    as part of a full block of 8 (one energy per warp) -- the operands and the k order are the same."""
+    from paper_1909_07321_b200 import inputs
+    w8 = inputs.make_wave(7000 + 13 * C + N, C, K, 8)
+    w = inputs.Wave(w8.W, w8.E_k, w8.energies[:N].copy(), w8.a)
+    R_ref = oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads())
+    R8 = _form(rmat, w8)[:N]                                   # n_E = 8: one classic block, no slab items
+    Wt = _dev(w.W.T)
+    for policy in (rmat.PSTGF_SLAB_T32, rmat.PSTGF_SLAB_T64, rmat.PSTGF_SLAB_T128, rmat.PSTGF_SLAB_AUTO, rmat.PSTGF_SLAB_NONE):
+        slab_policy(policy)
+        R = _form(rmat, w)
+        _check(R, R_ref)
+        assert np.array_equal(R, R8), f"policy {policy}: differs from the full-block result"
+        Rb = _form_batch(rmat, [w])[0].cpu().numpy()
+        assert np.array_equal(R, Rb)
+        Rh = rmat.pstgf_rmat_form_hdat(Wt, _dev(w.E_k), _dev(w.energies), w.a)
+        torch.cuda.synchronize()
+        assert np.array_equal(R, Rh.cpu().numpy())
+
+
+def test_energy_remainders_in_a_ragged_batch(rmat, oracle, slab_policy):
+    """n_E = 8 q + r for every r: classic blocks and slab groups of one wave in one launch, several waves with
+    different tile edges (and so the larger ring stage) in one batch, with a fine tail as well."""
+    from paper_1909_07321_b200 import inputs
+    waves = [inputs.make_wave(8100 + r, C, K, 8 * q + r) for r, (C, K, q) in
+             enumerate([(70, 90, 2), (150, 120, 1), (33, 200, 3), (260, 60, 0), (8, 160, 5), (100, 41, 1), (64, 64, 0), (190, 77, 2)])]
+    refs = [oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads()) for w in waves]
+    slab_policy(rmat.PSTGF_SLAB_NONE)
+    base = [r.cpu().numpy() for r in _form_batch(rmat, waves)]
+    for ref, b in zip(refs, base):
+        _check(b, ref)
+    for policy in (rmat.PSTGF_SLAB_AUTO, rmat.PSTGF_SLAB_T32, rmat.PSTGF_SLAB_T64, rmat.PSTGF_SLAB_T128):
+        slab_policy(policy)
+        for got, b in zip(_form_batch(rmat, waves), base):
+            assert np.array_equal(got.cpu().numpy(), b)
+    # the non-TMA staging path (odd leading dimension) under every edge
+    w = waves[1]
+    buf = torch.zeros((w.n_chan, w.n_poles + 1), dtype=torch.float64, device="cuda")
+    buf[:, :w.n_poles] = _dev(w.W)
+    for policy in (rmat.PSTGF_SLAB_T32, rmat.PSTGF_SLAB_T64, rmat.PSTGF_SLAB_T128):
+        slab_policy(policy)
+        R = rmat.pstgf_rmat_form(buf[:, :w.n_poles], _dev(w.E_k), _dev(w.energies), w.a)
+        torch.cuda.synchronize()
+        assert np.array_equal(R.cpu().numpy(), base[1])
+
+
+def test_single_energy_of_a_large_wave(rmat, oracle):
+    """n_E = 1 at config 5's shape, in the configuration the bench times (automatic tile edge)."""
+    from paper_1909_07321_b200 import inputs
+    w = inputs.make_config(5, n_E=3).waves[0]
+    R_ref = oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads())
+    _check(_form(rmat, w), R_ref)
+    one = inputs.Wave(w.W, w.E_k, w.energies[1:2].copy(), w.a)
+    R1 = _form(rmat, one)
+    _check(R1, R_ref[1:2])
+
+
+# ---- the diagonal addend (Buttle-type correction supplied by the caller; PAPER.md:524-528, :544) -------------
+@pytest.mark.parametrize("C,K,N", [(1, 3, 1), (9, 19, 3), (64, 80, 8), (65, 61, 13), (130, 41, 10), (200, 104, 7), (40, 0, 5)])
+def test_diag_add(rmat, oracle, slab_policy, C, K, N):
+    """R[e][n][n] = eq. 4 + diag_add[e][n], applied in the epilogue; the off-diagonal elements are bitwise those of
+    a call without the addend, the diagonal is the oracle's eq. 4 + addend (one rounding), and a zero addend changes
+    nothing.  Batch call, host call, term-by-term kernel; classic, fine and slab tiles."""
+    from paper_1909_07321_b200 import inputs
+    w = inputs.make_wave(9100 + C + N, C, K, N)
+    rng = np.random.default_rng(C * 100 + N)
+    da = rng.normal(0.0, 0.05, (N, C))
+    R_ref = oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads(), diag_add=da)
+    R_plain_ref = oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads())
+    idx = np.arange(C)
+    expect = R_plain_ref.copy()
+    expect[:, idx, idx] += da
+    assert np.array_equal(R_ref, expect)                       # the oracle's addend is one rounded add on the diagonal
+    Wd, Ek, en, dad = _dev(w.W), _dev(w.E_k), _dev(w.energies), _dev(da)
+
+    def run(diag, policy_tail, policy_slab):
+        rmat.pstgf_debug_set_tail_policy(policy_tail)
+        slab_policy(policy_slab)
+        R = torch.full((N, C, C), float("nan"), dtype=torch.float64, device="cuda")
+        arr = rmat.make_wave_array([(Wd, Ek, en, w.a, R, rmat.PSTGF_W_POLE_CONTIGUOUS, diag)])
+        ws = torch.empty(rmat.pstgf_rmat_batch_workspace_bytes(arr), dtype=torch.uint8, device="cuda")
+        rmat.pstgf_rmat_form_batch(arr, ws)
+        torch.cuda.synchronize()
+        return R.cpu().numpy()
+
+    try:
+        plain = run(None, rmat.PSTGF_TAIL_AUTO, rmat.PSTGF_SLAB_AUTO)
+        zero = run(torch.zeros_like(dad), rmat.PSTGF_TAIL_AUTO, rmat.PSTGF_SLAB_AUTO)
+        assert np.array_equal(plain, zero)
+        for pt, psl in ((rmat.PSTGF_TAIL_AUTO, rmat.PSTGF_SLAB_AUTO), (rmat.PSTGF_TAIL_NONE, rmat.PSTGF_SLAB_NONE),
+                        (rmat.PSTGF_TAIL_ALL, rmat.PSTGF_SLAB_T32), (rmat.PSTGF_TAIL_AUTO, rmat.PSTGF_SLAB_T128)):
+            R = run(dad, pt, psl)
+            off = ~np.eye(C, dtype=bool)
+            assert np.array_equal(R[:, off], plain[:, off])                    # off-diagonals untouched, bitwise
+            assert np.array_equal(R[:, idx, idx], plain[:, idx, idx] + da)     # one rounded add after the 1/(2a) scale
+            if K > 0:
+                _check(R, R_ref)
+            else:
+                assert np.array_equal(R, R_ref)
+    finally:
+        rmat.pstgf_debug_set_tail_policy(rmat.PSTGF_TAIL_AUTO)
+    Rn = rmat.pstgf_rmat_form_naive(Wd, Ek, en, w.a, diag_add=dad).cpu().numpy()
+    if K > 0:
+        _check(Rn, R_ref, tol=1e-15)
+    Rh = torch.full((N, C, C), float("nan"), dtype=torch.float64).pin_memory()
+    rmat.pstgf_rmat_form_batch_host([(torch.from_numpy(w.W).pin_memory(), torch.from_numpy(w.E_k).pin_memory(),
+                                      torch.from_numpy(w.energies).pin_memory(), w.a, Rh, rmat.PSTGF_W_POLE_CONTIGUOUS,
+                                      torch.from_numpy(da).pin_memory())])
+    assert np.array_equal(Rh.numpy(), R)
+
+
+# ---- boundary hygiene ------------------------------------------------------------------------------------------
+def test_workspace_reused_with_other_waves(rmat, oracle):
+    """The batch call keeps its TMA descriptors in the caller's workspace, which the next call rewrites: a second
+    call on the SAME workspace with other W pointers, shapes and memory orders must see the new descriptors
+    (fence.proxy.tensormap acquire in the load warp), back to back on one stream and without a sync in between."""
+    from paper_1909_07321_b200 import inputs
+    sets = [[inputs.make_wave(601, 150, 300, 19), inputs.make_wave(602, 72, 144, 33)],
+            [inputs.make_wave(603, 90, 500, 11), inputs.make_wave(604, 200, 100, 9)],
+            [inputs.make_wave(605, 33, 1000, 40), inputs.make_wave(606, 130, 260, 3)]]
+    layouts = [[0, 1], [1, 0], [1, 1]]
+    ws = torch.empty(rmat.pstgf_rmat_batch_workspace_bytes(None, 2), dtype=torch.uint8, device="cuda")
+    keep, outs = [], []
+    for rep in range(3):
+        for waves, lays in zip(sets, layouts):
+            dev = []
+            for w, lay in zip(waves, lays):
+                Wh = np.ascontiguousarray(w.W.T) if lay else w.W
+                R = torch.full((w.n_E, w.n_chan, w.n_chan), float("nan"), dtype=torch.float64, device="cuda")
+                dev.append((_dev(Wh), _dev(w.E_k), _dev(w.energies), w.a, R, lay))
+            arr = rmat.make_wave_array(dev)
+            rmat.pstgf_rmat_form_batch(arr, ws)                # no synchronisation between the calls
+            keep.append(dev)
+            outs.append((waves, [d[4] for d in dev]))
+    torch.cuda.synchronize()
+    refs = {}
+    for waves, Rs in outs:
+        for w, R in zip(waves, Rs):
+            if id(w) not in refs:
+                refs[id(w)] = oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads())
+            _check(R.cpu().numpy(), refs[id(w)])
+
+
+def test_batch_call_refuses_stream_capture(rmat):
+    from paper_1909_07321_b200 import inputs
+    w = inputs.make_wave(611, 40, 60, 9)
+    R = torch.empty((w.n_E, w.n_chan, w.n_chan), dtype=torch.float64, device="cuda")
+    arr = rmat.make_wave_array([(_dev(w.W), _dev(w.E_k), _dev(w.energies), w.a, R)])
+    ws = torch.empty(rmat.pstgf_rmat_batch_workspace_bytes(arr), dtype=torch.uint8, device="cuda")
+    lib = rmat.load()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(g, stream=side):
+            st = lib.pstgf_rmat_form_batch(arr, 1, ws.data_ptr(), ws.numel(), side.cuda_stream)
+    assert st == rmat.PSTGF_ERR_CAPTURE
+    torch.cuda.synchronize()
+    rmat.pstgf_rmat_form_batch(arr, ws)                        # and it still works outside the capture
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(R).all())
+
+
+def test_upload_wait_times_out(rmat, oracle):
+    """The kernel's wait for a slab of W is bounded.  With the "slab uploaded" signals withheld (debug knob) the load
+    warps give up after the time-out, the launch drains and the host call reports PSTGF_ERR_TIMEOUT instead of
+    hanging; the next call works."""
+    from paper_1909_07321_b200 import inputs
+    w = inputs.make_wave(621, 160, 30000, 96)                 # 7.4e10 counted FLOP: the signalled pipeline (>= 2 ms)
+    host = [(torch.from_numpy(w.W).pin_memory(), torch.from_numpy(w.E_k).pin_memory(),
+             torch.from_numpy(w.energies).pin_memory(), w.a,
+             torch.full((w.n_E, w.n_chan, w.n_chan), np.nan, dtype=torch.float64).pin_memory())]
+    rmat.pstgf_debug_set_upload_timeout_ms(50)
+    rmat.pstgf_debug_stall_upload(True)
+    try:
+        with pytest.raises(rmat.PstgfError) as info:
+            rmat.pstgf_rmat_form_batch_host(host)
+        assert info.value.status == rmat.PSTGF_ERR_TIMEOUT
+    finally:
+        rmat.pstgf_debug_stall_upload(False)
+        rmat.pstgf_debug_set_upload_timeout_ms(0)
+    rmat.pstgf_rmat_form_batch_host(host)
+    pick = [0, 31, 95]
+    _check(host[0][4].numpy()[pick], oracle.rmat_form(w.W, w.E_k, w.energies[pick], w.a, threads=_threads()))
+
+
+def test_finalize_and_reuse(rmat, oracle):
+    """pstgf_rmat_finalize frees the counter pool, the host call's memory pool and completion words; the library
+    works again afterwards (everything is re-created on demand)."""
+    from paper_1909_07321_b200 import inputs
+    w = inputs.make_wave(631, 160, 30000, 40)
+    R_ref = oracle.rmat_form(w.W, w.E_k, w.energies[[0, 39]], w.a, threads=_threads())
+    host = [(torch.from_numpy(w.W).pin_memory(), torch.from_numpy(w.E_k).pin_memory(),
+             torch.from_numpy(w.energies).pin_memory(), w.a,
+             torch.full((w.n_E, w.n_chan, w.n_chan), np.nan, dtype=torch.float64).pin_memory())]
+    for _ in range(2):
+        R = _form(rmat, w)
+        rmat.pstgf_rmat_form_batch_host(host)
+        assert np.array_equal(host[0][4].numpy(), R)
+        _check(R[[0, 39]], R_ref)
+        free_before, _ = torch.cuda.mem_get_info()
+        rmat.pstgf_rmat_finalize()
+        free_after, _ = torch.cuda.mem_get_info()
+        assert free_after >= free_before                       # the pools went back to the driver
+
+
+def test_duplicate_and_unsorted_poles(rmat, oracle):
+    """The header says E_k may come in any order: shuffled poles, and poles that occur twice."""
+    from paper_1909_07321_b200 import inputs
+    w = inputs.make_wave(641, 70, 120, 11)
+    rng = np.random.default_rng(5)
+    perm = rng.permutation(w.n_poles)
+    W2 = np.ascontiguousarray(np.concatenate([w.W[:, perm], w.W[:, :30]], axis=1))
+    Ek2 = np.concatenate([w.E_k[perm], w.E_k[:30]])
+    w2 = inputs.Wave(W2, Ek2, w.energies, w.a)
+    _check(_form(rmat, w2), oracle.rmat_form(W2, Ek2, w.energies, w.a, threads=_threads()))
+
+
+def test_batch_with_empty_waves(rmat, oracle):
+    """Waves with n_E == 0, n_chan == 0 or n_poles == 0 inside a batch: skipped or zero-filled, the others formed."""
+    from paper_1909_07321_b200 import inputs
+    real = [inputs.make_wave(651, 50, 70, 9), inputs.make_wave(652, 20, 33, 4)]
+    z = torch.zeros(0, dtype=torch.float64, device="cuda")
+    dev = []
+    for w in real:
+        dev.append((_dev(w.W), _dev(w.E_k), _dev(w.energies), w.a,
+                    torch.full((w.n_E, w.n_chan, w.n_chan), float("nan"), dtype=torch.float64, device="cuda")))
+    no_E = (_dev(real[0].W), _dev(real[0].E_k), z, 20.0, torch.zeros((0, 50, 50), dtype=torch.float64, device="cuda"))
+    no_chan = (torch.zeros((0, 7), dtype=torch.float64, device="cuda"), torch.arange(7, dtype=torch.float64, device="cuda"),
+               torch.ones(3, dtype=torch.float64, device="cuda"), 20.0, torch.zeros((3, 0, 0), dtype=torch.float64, device="cuda"))
+    no_poles = (torch.zeros((5, 0), dtype=torch.float64, device="cuda"), z, torch.ones(2, dtype=torch.float64, device="cuda"), 20.0,
+                torch.full((2, 5, 5), 7.0, dtype=torch.float64, device="cuda"))
+    order = [no_E, dev[0], no_chan, no_poles, dev[1]]
+    arr = rmat.make_wave_array(order)
+    ws = torch.empty(rmat.pstgf_rmat_batch_workspace_bytes(arr), dtype=torch.uint8, device="cuda")
+    rmat.pstgf_rmat_form_batch(arr, ws)
+    torch.cuda.synchronize()
+    assert torch.all(no_poles[4] == 0)
+    for w, d in zip(real, dev):
+        _check(d[4].cpu().numpy(), oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads()))
 
 
 # ---- W in the H.DAT record order (PAPER.md:535: channels fastest, one pole after the other) ----------------
@@ -507,7 +767,7 @@ def test_host_end_to_end_call(rmat, oracle, pipeline):
     from paper_1909_07321_b200 import inputs
     waves = [inputs.make_wave(21, 90, 140, 40), inputs.make_wave(22, 33, 61, 19), inputs.make_wave(23, 8, 0, 3),
              inputs.make_wave(24, 150, 200, 77)]
-    rmat.pstgf_rmat_set_host_pipeline(rmat.PSTGF_HOST_PIPELINE_CHUNKED if pipeline == "chunked"
+    rmat.pstgf_debug_set_host_pipeline(rmat.PSTGF_HOST_PIPELINE_CHUNKED if pipeline == "chunked"
                                       else rmat.PSTGF_HOST_PIPELINE_AUTO)
     try:
         for cap in (90 * 90 * 8 * 16, 1 << 10, 0):       # several pieces per wave; smaller than one energy block; default
@@ -524,7 +784,7 @@ def test_host_end_to_end_call(rmat, oracle, pipeline):
                 assert launches >= 3
             # (jobs this small take one launch per piece under either setting; the signalled pipeline has its own test)
     finally:
-        rmat.pstgf_rmat_set_host_pipeline(rmat.PSTGF_HOST_PIPELINE_AUTO)
+        rmat.pstgf_debug_set_host_pipeline(rmat.PSTGF_HOST_PIPELINE_AUTO)
 
 
 # ---- the paper's own problem size (7261 channels x 106 661 poles) -----------------
