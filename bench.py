@@ -479,6 +479,17 @@ def run_cuda(args):
                 torch.cuda.synchronize()
                 best = max(best, fl / (e0.elapsed_time(e1) * 1e-3) / 1e12)
             probe[name] = best
+        # dependent-issue latency of DMMA.8x8x4 in SM clocks: one chain per warp, one warp per sub-partition
+        it_chain = 2000
+        best_ms = 1e30
+        for _ in range(3):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            probe_lib.fp64_probe(3, it_chain, sms, 128, sink)
+            e1.record()
+            torch.cuda.synchronize()
+            best_ms = min(best_ms, e0.elapsed_time(e1))
+        probe["dmma_dependent_latency_clk"] = best_ms * 1e-3 * peaks["sm_max_mhz"] * 1e6 / (it_chain * 32)
     # Peak: the FP64 tensor (DMMA) rate measured live by the probe above (burst, this kernel is timed alone);
     # MEASURED_PEAKS.json has no FP64 entry.  The guide's rule (another dtype's measured peak x nominal ratio)
     # gives a LOWER figure because the bf16 measurement is power-limited (1335 MHz) while FP64 runs at 1965 MHz;

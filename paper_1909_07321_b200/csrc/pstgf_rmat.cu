@@ -188,7 +188,7 @@ double simulate_makespan(const std::vector<std::pair<double, int>> &runs, int gr
 double slab_item_cost(int T, int g, int n_kt) {
   const pstgf::SlabShape sh = pstgf::slab_shape(T, g);
   const int blocks = sh.nr * sh.ncw;
-  const double quality = blocks >= 32 ? 1.0 : blocks >= 16 ? 1.03 : blocks >= 8 ? 1.08 : blocks >= 4 ? 1.25 : 1.5;
+  const double quality = blocks >= 32 ? 1.0 : blocks >= 16 ? 1.04 : blocks >= 8 ? 1.10 : blocks >= 4 ? 1.15 : 1.25;
   return blocks * quality * ((double)n_kt + 3.0);
 }
 
@@ -256,13 +256,16 @@ void plan_slabs(std::vector<DevWave> &ds, int grid) {
   }
 }
 
-// Ring geometry of a launch: the classic stage (5 panels of 32 channels) unless a wave has slab tiles of edge 128
-// (8 panels); as many stages as fit, at most MAX_STAGES.
+// Ring geometry of a launch: a stage holds the most panels any of its items needs (5 for classic items, 8 / 4 / 2
+// for slab tiles of edge 128 / 64 / 32); as many stages as fit, at most MAX_STAGES.  Small stages make a deep ring:
+// items that spend a few hundred cycles on a stage need many stages in flight to cover the load latency.
 pstgf::RingGeo ring_geometry(const std::vector<DevWave> &ds) {
   int bytes = 0;
   for (const DevWave &d : ds) {
-    const bool big = slab_items(d) > 0 && d.slab_T == 128;
-    bytes = std::max(bytes, pstgf::stage_bytes_for(d.tr != 0, big ? pstgf::BIG_PANELS : pstgf::CLASSIC_PANELS));
+    int panels = 0;
+    if (coarse_items(d) + fine_items(d) > 0) panels = pstgf::CLASSIC_PANELS;
+    if (slab_items(d) > 0) panels = std::max(panels, pstgf::slab_panels(d.slab_T));
+    bytes = std::max(bytes, pstgf::stage_bytes_for(d.tr != 0, panels));
   }
   pstgf::RingGeo g;
   g.stage_bytes = bytes;

@@ -40,7 +40,7 @@ constexpr int TW = 128;     // WIDE tile rows (the I panel region of a classic s
 constexpr int TWN = 16;     // WIDE tile columns
 constexpr int KT = 20;      // poles per pipeline stage; row pitch 20 doubles == 4 (mod 16) -> conflict-free LDS.64
 constexpr int EB = 8;       // energies per item == consumer warps per CTA
-constexpr int MAX_STAGES = 7;   // smem ring depth (fewer when a launch needs the larger stage of 128-row slab tiles)
+constexpr int MAX_STAGES = 16;  // smem ring depth: as many stages as fit (7 classic, 5 with 128-row slab tiles, 16 with 32-row ones)
 constexpr int PRODUCER_WARPS = 4;                    // one warpgroup: 1 load warp + 3 pole-scaling warps
 constexpr int NUM_THREADS = (EB + PRODUCER_WARPS) * 32;   // 8 consumer warps + the producer warpgroup
 constexpr int PRODUCER_REGS = 56;                    // setmaxnreg targets: 8*224 + 4*56 = 12*168, the launch allocation
@@ -71,13 +71,13 @@ struct StageLayout {
 };
 constexpr int stage_bytes_for(bool tr, int panels) { return D_BYTES + panels * (tr ? TR_BOX_BYTES : BOX_BYTES); }
 constexpr int CLASSIC_PANELS = TW / TN + 1;          // 5
-constexpr int BIG_PANELS = 2 * (TW / TN);            // 8: slab tiles of edge 128
+constexpr int slab_panels(int T) { return 2 * (T / TN); }   // 8, 4, 2 for slab tiles of edge 128, 64, 32
 
 // Shared memory of a CTA: [mbarriers | two ItemInfo slots | ring of n_stages stages]; the ring geometry is a launch
 // parameter (RingGeo) because slab tiles of edge 128 need 8 panels per stage instead of 5.
-constexpr int SMEM_BARRIER_OFFSET = 0;               // (2 MAX_STAGES + 4) x 8 B
-constexpr int SMEM_ITEM_OFFSET = 256;                // 2 x 128 B
-constexpr int SMEM_RING_OFFSET = 512;
+constexpr int SMEM_BARRIER_OFFSET = 0;               // (2 MAX_STAGES + 4) x 8 B = 288
+constexpr int SMEM_ITEM_OFFSET = 384;                // 2 x 128 B
+constexpr int SMEM_RING_OFFSET = 640;
 constexpr int SMEM_ALIGN_SLACK = 128;
 constexpr int SMEM_MAX_OPTIN = 232448;               // 227 KB
 struct RingGeo {

@@ -84,6 +84,11 @@ __device__ __forceinline__ uint64_t l2_policy_evict_last() {
   asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
   return p;
 }
+__device__ __forceinline__ uint64_t l2_policy_evict_normal() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
 // A tensor map that lives in global memory (the batch call's workspace, rewritten by every call) must be
 // acquired by the CTA before its first use by the TMA unit, or a stale cached copy may be used.
 __device__ __forceinline__ void tensormap_acquire(const CUtensorMap *map) {
@@ -295,11 +300,15 @@ __device__ __forceinline__ void consume_diag(const ItemInfo &it, Pipe &ps, int w
 // blocks [cb0, cb0 + NCW) of 8 x 8.  The DMMA loop has no predicates: a warp whose slab is cut by the diagonal or by
 // the edge of the matrix computes all of its register tile and stores only what is wanted (nrc[c] row blocks of
 // column c: a prefix, because rows ascend); a warp with nothing wanted only keeps the ring moving.  A = rows of
-// the I panels, B = scaled rows of the J panels (the I panels on a diagonal tile): the same operands and k order
-// as a classic item gives the element, hence the same bits.
-template <int NR, int NCW, bool TR>
+// the I panels, B = scaled rows of the J panels (the I panels on a diagonal tile): the same operands and (NCH == 1,
+// what the library uses) the same k order as a classic item gives the element, hence the same bits.  NCH == 5 sums
+// the five k-steps of a stage into five chains that are added at the end: a different association of the same
+// terms; measured to buy nothing (a dependent DMMA issues after 26.5 clk, so two accumulators per warp already fill
+// the pipe's 16-clk slots), kept as a compile-time option only.
+template <int NR, int NCW, int NCH, bool TR>
 __device__ __forceinline__ void consume_slab(const ItemInfo &it, Pipe &ps, int warp, int lane, int wc) {
   using L = StageLayout<TR>;
+  static_assert(NCH == 1 || NCH == KT / 4, "one summation chain, or one per k-step of a stage");
   const int T = it.slab_T, gE = it.slab_g, C = it.n_chan;
   const int e_slot = warp % gE, s = warp / gE;              // which energy of the group, which slab of the tile
   const int wci = s % wc, wri = s / wc;
@@ -324,11 +333,13 @@ __device__ __forceinline__ void consume_slab(const ItemInfo &it, Pipe &ps, int w
   const int aoff = L::W_BASE + L::off(rb0 * 8, 0) + L::off(g, q);
   const int boff = L::W_BASE + L::off(jrow + cb0 * 8, 0) + L::off(g, q);
   const int doff = e_slot * KT + q;
-  double acc[NR][NCW][2];
+  double acc[NCH][NR][NCW][2];
 #pragma unroll
-  for (int bi = 0; bi < NR; ++bi)
+  for (int h = 0; h < NCH; ++h)
 #pragma unroll
-    for (int c = 0; c < NCW; ++c) acc[bi][c][0] = acc[bi][c][1] = 0.0;
+    for (int bi = 0; bi < NR; ++bi)
+#pragma unroll
+      for (int c = 0; c < NCW; ++c) acc[h][bi][c][0] = acc[h][bi][c][1] = 0.0;
   for (int kt = 0; kt < it.n_kt; ++kt) {
     mbar_wait(ps.full(), ps.phase);
     const double *st = ps.stage_ptr();
@@ -337,6 +348,7 @@ __device__ __forceinline__ void consume_slab(const ItemInfo &it, Pipe &ps, int w
     const double *dd = st + doff;
 #pragma unroll
     for (int ks = 0; ks < KT / 4; ++ks) {
+      const int h = NCH == 1 ? 0 : ks;                       // the chain this k-step adds to
       const double dv = dd[ks * 4];
       double a[NR];
 #pragma unroll
@@ -345,7 +357,7 @@ __device__ __forceinline__ void consume_slab(const ItemInfo &it, Pipe &ps, int w
       for (int c = 0; c < NCW; ++c) {
         const double b = wb[L::off(c * 8, ks * 4)] * dv;     // pole scaling folded into the B fragment
 #pragma unroll
-        for (int bi = 0; bi < NR; ++bi) dmma884(acc[bi][c][0], acc[bi][c][1], a[bi], b);
+        for (int bi = 0; bi < NR; ++bi) dmma884(acc[h][bi][c][0], acc[h][bi][c][1], a[bi], b);
       }
     }
     release_stage(ps, lane);
@@ -363,7 +375,15 @@ __device__ __forceinline__ void consume_slab(const ItemInfo &it, Pipe &ps, int w
       if (bi < nrc[c]) {
         const int r = it.row0 + (rb0 + bi) * 8 + g;
         const bool dg = diag && rb0 + bi == cb0 + c;         // a block on the diagonal: keep col >= r only
-        double v0 = acc[bi][c][0] * sc, v1 = acc[bi][c][1] * sc;
+        double v0 = acc[0][bi][c][0], v1 = acc[0][bi][c][1];
+        if (NCH > 1) {                                       // fixed order: ((c0 + c1) + (c2 + c3)) + c4
+          v0 = __dadd_rn(__dadd_rn(__dadd_rn(v0, acc[1 % NCH][bi][c][0]), __dadd_rn(acc[2 % NCH][bi][c][0], acc[3 % NCH][bi][c][0])),
+                         acc[4 % NCH][bi][c][0]);
+          v1 = __dadd_rn(__dadd_rn(__dadd_rn(v1, acc[1 % NCH][bi][c][1]), __dadd_rn(acc[2 % NCH][bi][c][1], acc[3 % NCH][bi][c][1])),
+                         acc[4 % NCH][bi][c][1]);
+        }
+        v0 *= sc;
+        v1 *= sc;
         if (r < C) {
           if (col < C && (!dg || col >= r)) {
             if (dg && col == r && da) v0 += __ldg(da + r);
@@ -388,12 +408,12 @@ __device__ __forceinline__ void consume_item_layout(const ItemInfo &it, Pipe &ps
   if (it.slab_T != 0) {
     const SlabShape sh = slab_shape(it.slab_T, it.slab_g);
     switch (sh.nr) {
-      case 16: consume_slab<16, 2, TR>(it, ps, warp, lane, sh.wc); break;
-      case 8: consume_slab<8, 2, TR>(it, ps, warp, lane, sh.wc); break;
-      case 4: consume_slab<4, 2, TR>(it, ps, warp, lane, sh.wc); break;
+      case 16: consume_slab<16, 2, 1, TR>(it, ps, warp, lane, sh.wc); break;
+      case 8: consume_slab<8, 2, 1, TR>(it, ps, warp, lane, sh.wc); break;
+      case 4: consume_slab<4, 2, 1, TR>(it, ps, warp, lane, sh.wc); break;
       default:
-        if (sh.ncw == 2) consume_slab<2, 2, TR>(it, ps, warp, lane, sh.wc);
-        else consume_slab<2, 1, TR>(it, ps, warp, lane, sh.wc);
+        if (sh.ncw == 2) consume_slab<2, 2, 1, TR>(it, ps, warp, lane, sh.wc);
+        else consume_slab<2, 1, 1, TR>(it, ps, warp, lane, sh.wc);
         break;
     }
     return;
@@ -549,7 +569,7 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < geo.n_stages; ++s) {
-      mbar_init(full0 + 8 * s, PRODUCER_WARPS);   // load warp (TMA expect_tx / plain staging done) + 3 pole-scaling warps
+      mbar_init(full0 + 8 * s, 2);     // load warp (TMA expect_tx / plain staging done) + the pole-scaling warp whose turn it is
       mbar_init(empty0 + 8 * s, EB);   // one arrival per consumer warp
     }
     for (int s = 0; s < 2; ++s) {
@@ -574,7 +594,7 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
       // ---- load warp: takes work items, publishes them, stages the W panels (S2, S5) ----
       uint32_t iq = 0, iphase = 0;
       long long next_static = blockIdx.x;
-      const uint64_t keep_policy = l2_policy_evict_last();
+      const uint64_t keep_policy = l2_policy_evict_last(), normal_policy = l2_policy_evict_normal();
       int last_wave = -1;
       for (;;) {
         // items are drawn from an atomic counter (batch call: in the workspace; single-wave call: a slot of
@@ -698,24 +718,29 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
           rows_seen = 0xffffffffu;
         }
         if (w.use_tma) {
-          // TMA box coordinates: (pole, channel) for pole-contiguous W, (channel, pole) for the H.DAT order
-          const int tr = w.tr;
-          const bool keep = w.l2_keep != 0;
+          // One box per lane: lane b < i_boxes + j_boxes issues box b of every stage.  Everything that does not
+          // change from stage to stage is worked out here, so that a stage costs this warp a few dozen
+          // instructions: items that spend only a few hundred cycles on a stage (slab tiles of edge 32) would
+          // otherwise be bound by this loop.  TMA box coordinates: (pole, channel) for pole-contiguous W,
+          // (channel, pole) for the H.DAT order.
+          const int nb = i_boxes + j_boxes;
+          const bool my_box = lane < nb;
+          const int my_chan = lane < i_boxes ? row0 + lane * TN : col0 + (lane - i_boxes) * TN;
+          const uint32_t my_dst = smem_u32(stages) + D_BYTES + (uint32_t)(lane < i_boxes ? lane : j_panel0 + (lane - i_boxes)) * box;
+          int c0 = w.tr ? my_chan : 0, c1 = w.tr ? 0 : my_chan;
+          const int s0 = w.tr ? 0 : KT, s1 = w.tr ? KT : 0;
+          const uint64_t policy = w.l2_keep ? keep_policy : normal_policy;
+          const int n_poles = w.n_poles;
+          unsigned int *const abort_flag = w.abort_flag;
           for (int kt = 0; kt < n_kt; ++kt) {
-            const int k0 = kt * KT;
-            wait_rows_uploaded(rows_ready, (unsigned int)min(k0 + KT, w.n_poles), rows_seen, w.abort_flag, timeout_ns, lane);
+            if (rows_ready != nullptr)
+              wait_rows_uploaded(rows_ready, (unsigned int)min(kt * KT + KT, n_poles), rows_seen, abort_flag, timeout_ns, lane);
             mbar_wait(ps.empty(), ps.phase ^ 1u);
-            if (lane == 0) {
-              const uint32_t full = ps.full();
-              const uint32_t dst = smem_u32(stages + (size_t)ps.stage * ps.stage_bytes) + D_BYTES;
-              mbar_arrive_expect_tx(full, tx_bytes);
-              for (int b = 0; b < i_boxes + j_boxes; ++b) {
-                const int chan = b < i_boxes ? row0 + b * TN : col0 + (b - i_boxes) * TN;
-                const uint32_t d = dst + (uint32_t)(b < i_boxes ? b : j_panel0 + (b - i_boxes)) * box;
-                if (keep) tma_load_2d_hint(d, map, tr ? chan : k0, tr ? k0 : chan, full, keep_policy);
-                else tma_load_2d(d, map, tr ? chan : k0, tr ? k0 : chan, full);
-              }
-            }
+            const uint32_t full = ps.full();
+            if (lane == 0) mbar_arrive_expect_tx(full, tx_bytes);
+            if (my_box) tma_load_2d_hint(my_dst + ps.stage * (uint32_t)ps.stage_bytes, map, c0, c1, full, policy);
+            c0 += s0;
+            c1 += s1;
             ps.advance();
           }
         } else {
@@ -747,12 +772,14 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
       }
     } else {
       // ---- pole-scaling warps (S1): d_e[k] = 1/(E_k - E_e) of every stage, built in shared memory.
-      // Three warps on three different SM sub-partitions share the EB x KT entries of a stage: the FP64
-      // pipe they need is saturated by the consumers' DMMAs, and one warp alone cannot get enough issue
-      // slots to keep up with the ring.
-      constexpr int DW = PRODUCER_WARPS - 1;                 // 3 warps, 96 lanes
-      constexpr int DT = (EB * KT + DW * 32 - 1) / (DW * 32);
-      const int dl = (warp - EB - 1) * 32 + lane;
+      // The three warps take the stages of an item in turn (warp j the k-tiles j, j + 3, ...), lane = pole of the
+      // tile, a loop over the item's energies.  An FP64 division is a dependent chain of some 300 cycles; a warp
+      // computes the divisions of its NEXT stage right after it has handed the current one over, so that chain runs
+      // while the warp waits for its next empty slot, and with three warps in turn a stage can be handed over
+      // every ~100 cycles -- slab items of edge 32 consume one every ~300 (classic items every 5000).
+      constexpr int DW = PRODUCER_WARPS - 1;                 // 3 warps
+      const int sw = warp - EB - 1;
+      const bool pole_lane = lane < KT;
       uint32_t iq = 0, iphase = 0;
       for (;;) {
         mbar_wait(item_full0 + 8 * iq, iphase);
@@ -763,40 +790,42 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
         iq ^= 1u;
         if (iq == 0) iphase ^= 1u;
         if (it.kind < 0) break;
-        double en[DT], ek[DT];
-        int kk[DT], slot[DT];
-        bool ev[DT];
+        const int nv = it.n_valid_e;
+        double en[EB], dv[EB];
 #pragma unroll
-        for (int t = 0; t < DT; ++t) {
-          const int idx = dl + DW * 32 * t;
-          const int e = idx / KT;
-          slot[t] = idx < EB * KT ? idx : -1;
-          kk[t] = idx - e * KT;
-          ev[t] = slot[t] >= 0 && e < it.n_valid_e;
-          en[t] = ev[t] ? __ldg(it.energies + e) : 0.0;
-          ek[t] = (ev[t] && kk[t] < it.n_poles) ? __ldg(it.E_k + kk[t]) : 0.0;
-        }
+        for (int e = 0; e < EB; ++e) en[e] = (pole_lane && e < nv) ? __ldg(it.energies + e) : 0.0;
+        auto load_pole = [&](int kt) -> double {
+          const int k = kt * KT + lane;
+          return (pole_lane && kt < it.n_kt && k < it.n_poles) ? __ldg(it.E_k + k) : 0.0;
+        };
+        auto scale = [&](int kt, double ek) {
+          // 0 beyond n_poles so that zero-filled W columns stay zero; energy slots beyond the item's are never read
+          const bool ok = pole_lane && kt * KT + lane < it.n_poles;
+#pragma unroll
+          for (int e = 0; e < EB; ++e)
+            if (e < nv) dv[e] = ok ? 1.0 / (ek - en[e]) : 0.0;
+        };
+        scale(sw, load_pole(sw));
+        double ek_next = load_pole(sw + DW);                 // poles are fetched two turns ahead (an L2 round trip)
+        int turn = sw;                                       // k-tiles until this warp's next stage
         for (int kt = 0; kt < it.n_kt; ++kt) {
-          const int k0 = kt * KT;
-          // prefetch the next stage's poles before blocking on the ring
-          double ek_next[DT];
+          if (turn == 0) {
+            const double ek_after = load_pole(kt + 2 * DW);
+            mbar_wait(ps.empty(), ps.phase ^ 1u);
+            double *dsm = reinterpret_cast<double *>(stages + (size_t)ps.stage * ps.stage_bytes);   // d is first in a stage
+            if (pole_lane) {
 #pragma unroll
-          for (int t = 0; t < DT; ++t) {
-            const int k = k0 + KT + kk[t];
-            ek_next[t] = (ev[t] && k < it.n_poles) ? __ldg(it.E_k + k) : 0.0;
+              for (int e = 0; e < EB; ++e)
+                if (e < nv) dsm[e * KT + lane] = dv[e];
+            }
+            __threadfence_block();     // every lane's d has been written before lane 0 arrives
+            __syncwarp();
+            if (lane == 0) mbar_arrive(ps.full());
+            scale(kt + DW, ek_next);
+            ek_next = ek_after;
+            turn = DW;
           }
-          mbar_wait(ps.empty(), ps.phase ^ 1u);
-          double *dsm = reinterpret_cast<double *>(stages + (size_t)ps.stage * ps.stage_bytes);   // d is first in a stage
-#pragma unroll
-          for (int t = 0; t < DT; ++t) {
-            // 0 beyond n_poles / n_E so that zero-filled W columns stay zero
-            const bool ok = ev[t] && (k0 + kk[t] < it.n_poles);
-            if (slot[t] >= 0) dsm[slot[t]] = ok ? 1.0 / (ek[t] - en[t]) : 0.0;
-            ek[t] = ek_next[t];
-          }
-          __threadfence_block();     // every lane's d has been written before lane 0 arrives
-          __syncwarp();
-          if (lane == 0) mbar_arrive(ps.full());
+          --turn;
           ps.advance();
         }
       }

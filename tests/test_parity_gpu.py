@@ -198,7 +198,9 @@ def test_energy_remainders_in_a_ragged_batch(rmat, oracle, slab_policy):
     for policy in (rmat.PSTGF_SLAB_T32, rmat.PSTGF_SLAB_T64, rmat.PSTGF_SLAB_T128):
         slab_policy(policy)
         R = rmat.pstgf_rmat_form(buf[:, :w.n_poles], _dev(w.E_k), _dev(w.energies), w.a)
+        Rt = rmat.pstgf_rmat_form(_dev(w.W), _dev(w.E_k), _dev(w.energies), w.a)        # the TMA path, same policy
         torch.cuda.synchronize()
+        assert torch.equal(R, Rt)
         assert np.array_equal(R.cpu().numpy(), base[1])
 
 
@@ -242,11 +244,11 @@ def test_diag_add(rmat, oracle, slab_policy, C, K, N):
         return R.cpu().numpy()
 
     try:
-        plain = run(None, rmat.PSTGF_TAIL_AUTO, rmat.PSTGF_SLAB_AUTO)
         zero = run(torch.zeros_like(dad), rmat.PSTGF_TAIL_AUTO, rmat.PSTGF_SLAB_AUTO)
-        assert np.array_equal(plain, zero)
+        assert np.array_equal(run(None, rmat.PSTGF_TAIL_AUTO, rmat.PSTGF_SLAB_AUTO), zero)
         for pt, psl in ((rmat.PSTGF_TAIL_AUTO, rmat.PSTGF_SLAB_AUTO), (rmat.PSTGF_TAIL_NONE, rmat.PSTGF_SLAB_NONE),
                         (rmat.PSTGF_TAIL_ALL, rmat.PSTGF_SLAB_T32), (rmat.PSTGF_TAIL_AUTO, rmat.PSTGF_SLAB_T128)):
+            plain = run(None, pt, psl)                                         # the same schedule without the addend
             R = run(dad, pt, psl)
             off = ~np.eye(C, dtype=bool)
             assert np.array_equal(R[:, off], plain[:, off])                    # off-diagonals untouched, bitwise
