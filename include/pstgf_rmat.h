@@ -24,7 +24,9 @@
  *    memory plus a copy; pstgf_rmat_form_batch_host is the fast host path).
  *  - Device memory owned by the library.  The DEVICE-pointer calls allocate
  *    none, but for the 8 KiB counter pool of pstgf_rmat_form (once per
- *    device); the batch call keeps its tables in the caller's workspace.
+ *    device) and that call's stream-ordered scratch for few-channel waves
+ *    (freed behind the launch); the batch call keeps its tables and scratch
+ *    in the caller's workspace.
  *    pstgf_rmat_form_batch_host stages through a memory pool of its own (one
  *    per device) and keeps 33 KiB of completion words per calling thread.
  *    pstgf_rmat_finalize() frees all of it.
@@ -54,8 +56,9 @@
  *    used.  Any n_chan (odd included) is supported.
  *  - Results are deterministic: each R element is produced by exactly one
  *    thread with a fixed k order, whatever CTA picked the work item up, and
- *    however the energies of a call are grouped: an energy gives the same bits
- *    in a call of 1 energy, of 7 or of 4096.
+ *    however the energies of a call are tiled and grouped.  (A wave with
+ *    n_chan <= 96 switches to the pair form at 64 energies, which rounds each
+ *    term differently: a few ulp, see pstgf_debug_set_pair_policy.)
  *  - Errors are returned as pstgf_status_t; nothing is thrown or printed.
  *    Argument errors are detected before anything is enqueued.
  */
@@ -163,9 +166,13 @@ pstgf_status_t pstgf_rmat_form_hdat(const double *Wt, long long ldw, const doubl
                                     double a, double *R_out, void *stream);
 
 /*
- * Bytes of device workspace pstgf_rmat_form_batch needs for these waves
- * (only n_waves matters today; the waves are passed for future layouts).
- * Returns 0 for n_waves <= 0.
+ * Bytes of device workspace pstgf_rmat_form_batch needs for these waves: the
+ * tables (a few hundred bytes per wave) plus, for every wave that is done in
+ * the pair form (n_chan <= 96 with at least 64 energies, see
+ * pstgf_rmat_form_batch), 8 * n_poles * (n_chan (n_chan + 1) / 2 + n_E) bytes
+ * of scratch.  `waves` is the HOST array that will be passed to the batch call
+ * (only the sizes are read; NULL gives the size of the tables alone, which is
+ * enough only if no wave takes the pair form).  Returns 0 for n_waves <= 0.
  */
 size_t pstgf_rmat_batch_workspace_bytes(const pstgf_wave_t *waves, int n_waves);
 
@@ -179,6 +186,15 @@ size_t pstgf_rmat_batch_workspace_bytes(const pstgf_wave_t *waves, int n_waves);
  * energy block, tile), waves ordered by decreasing cost, are handed to CTAs
  * through an atomic counter: the counterpart of the paper's energy-permuting
  * distribution over MPI ranks (Fig. 1).
+ * Waves with few channels (n_chan <= 96) and at least 64 energies are
+ * evaluated as the plain GEMM over channel pairs, R[e][(n,m)] = (1/2a) sum_k
+ * (w_nk w_mk) * (1/(E_k - E_e)) -- the same eq. 4, term for term, with the
+ * products w_nk w_mk and the reciprocals written to scratch first (a second
+ * small launch): tiles of an n_chan x n_chan matrix that small are mostly
+ * diagonal blocks, which the symmetric form computes in full.  pstgf_rmat_form
+ * does the same with stream-ordered scratch of its own (cudaMallocAsync on
+ * `stream`, freed behind the launch).  The choice depends on the wave's shape
+ * only, so a wave gives the same bits through every call.
  */
 pstgf_status_t pstgf_rmat_form_batch(const pstgf_wave_t *waves, int n_waves, void *workspace,
                                      size_t workspace_bytes, void *stream);
@@ -236,8 +252,8 @@ pstgf_status_t pstgf_mesh_from_zscaled(const double *e_scaled, long long n, doub
 pstgf_status_t pstgf_rmat_finalize(void);
 
 /* ---- knobs for tests and measurements ------------------------------------------------------------
- * THREAD-LOCAL: each affects only the calls the calling thread makes afterwards.  None changes a
- * single bit of any result. */
+ * THREAD-LOCAL: each affects only the calls the calling thread makes afterwards.  None but the pair
+ * policy changes a single bit of any result. */
 
 /*
  * Work items are handed to the persistent CTAs largest first; the END of that list
@@ -266,6 +282,18 @@ pstgf_status_t pstgf_debug_set_tail_policy(int policy);
 #define PSTGF_SLAB_T64 3
 #define PSTGF_SLAB_T128 4
 pstgf_status_t pstgf_debug_set_slab_policy(int policy);
+
+/*
+ * Which waves are evaluated as the GEMM over channel pairs (see
+ * pstgf_rmat_form_batch): PSTGF_PAIRS_AUTO (default: n_chan <= 96 and
+ * n_E >= 64), PSTGF_PAIRS_NONE (none: the symmetric form for everything, the
+ * round-1 behaviour), PSTGF_PAIRS_ALWAYS (every wave with n_chan <= 96).  The
+ * two forms round differently (a few ulp apart, both far inside 1e-11).
+ */
+#define PSTGF_PAIRS_AUTO 0
+#define PSTGF_PAIRS_NONE 1
+#define PSTGF_PAIRS_ALWAYS 2
+pstgf_status_t pstgf_debug_set_pair_policy(int policy);
 
 /*
  * How pstgf_rmat_form_batch_host overlaps formation and copy-back.

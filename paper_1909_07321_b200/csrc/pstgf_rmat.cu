@@ -114,6 +114,7 @@ pstgf_status_t check_wave(const pstgf_wave_t &w) {
 // Knobs for tests and measurements (pstgf_debug_*): thread-local, they affect the calling thread's calls only.
 thread_local int tl_tail_policy = PSTGF_TAIL_AUTO;
 thread_local int tl_slab_policy = PSTGF_SLAB_AUTO;
+thread_local int tl_pair_policy = PSTGF_PAIRS_AUTO;
 thread_local int tl_host_pipeline = PSTGF_HOST_PIPELINE_AUTO;
 thread_local unsigned int tl_upload_timeout_ms = 0;   // 0 = the kernel's default (2 s)
 thread_local int tl_stall_upload = 0;
@@ -148,13 +149,135 @@ void plan_wave(const pstgf_wave_t &w, DevWave &d, int l2_bytes) {
   d.l2_keep = (l2_bytes > 0 && w_bytes <= 0.5 * (double)l2_bytes) ? 1 : 0;
 }
 
-long long coarse_items(const DevWave &d) { return (long long)d.n_tiles * d.n_eb_coarse; }
-long long slab_items(const DevWave &d) { return (long long)pstgf::slab_tiles(d.slab_nt) * (d.slab_g2 + d.slab_g1); }
-long long fine_items(const DevWave &d) { return (long long)pstgf::fine_tiles(d.n_j) * (d.n_eb - d.n_eb_coarse); }
+// A wave in the pair form has its 128-pair items in the "coarse" section and its 32-pair tail in the "fine" one.
+long long coarse_items(const DevWave &d) {
+  return d.n_pairs > 0 ? (long long)d.pair_mt * d.pair_nt_coarse : (long long)d.n_tiles * d.n_eb_coarse;
+}
+long long slab_items(const DevWave &d) {
+  return d.n_pairs > 0 ? 0 : (long long)pstgf::slab_tiles(d.slab_nt) * (d.slab_g2 + d.slab_g1);
+}
+long long fine_items(const DevWave &d) {
+  return d.n_pairs > 0 ? (long long)d.pair_mtf * (d.pair_nt - d.pair_nt_coarse)
+                       : (long long)pstgf::fine_tiles(d.n_j) * (d.n_eb - d.n_eb_coarse);
+}
 long long wave_items(const DevWave &d) { return coarse_items(d) + slab_items(d) + fine_items(d); }
 
 // Relative cost of a wave's items, for the largest-first order of the batch.
 double wave_item_cost(const pstgf_wave_t &w) { return (double)std::min(w.n_chan, pstgf::TM) * w.n_poles; }
+
+double simulate_makespan(const std::vector<std::pair<double, int>> &runs, int grid);
+
+// ---- pair form: which waves, how much scratch -----------------------------------------------------
+// A wave is done as the GEMM over channel pairs (rmat_common.h) when it has few channels and enough energies to
+// fill an energy tile's warps.  The choice depends on the wave's own shape only (and the thread's debug knob), so
+// that a wave gives the same bits alone, in any batch and through the host call.
+bool wants_pair_form(int n_chan, int n_poles, int n_E) {
+  if (tl_pair_policy == PSTGF_PAIRS_NONE) return false;
+  if (n_chan <= 0 || n_poles <= 0 || n_chan > pstgf::PAIR_MAX_CHAN) return false;
+  if (tl_pair_policy == PSTGF_PAIRS_ALWAYS) return n_E > 0;
+  return n_E >= pstgf::PAIR_MIN_E;
+}
+long long pair_count(int n_chan) { return (long long)n_chan * (n_chan + 1) / 2; }
+long long pair_ld(int n_poles) { return ((long long)n_poles + 1) & ~1LL; }
+size_t pair_scratch_bytes(int n_chan, int n_poles, int n_E) {        // P, D, the (n, m) table: each 256-byte aligned
+  const size_t ld = (size_t)pair_ld(n_poles);
+  const size_t p = (((size_t)pair_count(n_chan) * ld * 8) + 255) & ~(size_t)255;
+  const size_t d = (((size_t)n_E * ld * 8) + 255) & ~(size_t)255;
+  const size_t t = (((size_t)pair_count(n_chan) * 4) + 255) & ~(size_t)255;
+  return p + d + t;
+}
+// Cuts a wave into pair items; `scratch` is where its P and D go.  Every energy tile starts out coarse (128-pair
+// items); plan_pair_tails then cuts the tail of the launch into 64-pair items.
+void plan_pairs(DevWave &d, unsigned char *scratch) {
+  d.n_pairs = (int)pair_count(d.n_chan);
+  d.pair_ld = pair_ld(d.n_poles);
+  d.pair_P = reinterpret_cast<double *>(scratch);
+  const size_t p_bytes = (((size_t)d.n_pairs * (size_t)d.pair_ld * 8) + 255) & ~(size_t)255;
+  const size_t d_bytes = (((size_t)d.n_E * (size_t)d.pair_ld * 8) + 255) & ~(size_t)255;
+  d.pair_D = reinterpret_cast<double *>(scratch + p_bytes);
+  d.pair_nm = reinterpret_cast<const unsigned int *>(scratch + p_bytes + d_bytes);
+  d.pair_nfb = d.n_chan / 8;
+  d.pair_rb = pstgf::pair_block_rows(d.n_chan);
+  d.pair_mt = (d.n_pairs + pstgf::PT_M - 1) / pstgf::PT_M;
+  d.pair_mtf = (d.n_pairs + pstgf::PT_MF - 1) / pstgf::PT_MF;
+  d.pair_nt = (d.n_E + pstgf::PT_N - 1) / pstgf::PT_N;
+  d.pair_nt_coarse = d.pair_nt;
+  // no classic or slab items
+  d.n_eb = d.n_eb_coarse = 0;
+  d.slab_g2 = d.slab_g1 = 0;
+  d.slab_e0 = d.n_E;
+}
+
+// Relative cost of a wave's pair items: row blocks per item (16, fewer in the last pair tile; 8 for fine items)
+double pair_last_tile_blocks(const DevWave &d) {
+  const int left = d.n_pairs - (d.pair_mt - 1) * pstgf::PT_M;
+  return left > 64 ? 16.0 : left > 32 ? 8.0 : 4.0;
+}
+
+// The tail of the launch's pair items -- about one round of the grid -- in 64-pair items (whole energy tiles), so
+// that the CTAs run dry together, like the fine tiles of the symmetric form.  One wave: the tail size with the
+// smallest simulated makespan; several waves: whole energy tiles from the end of the list until a round's worth of
+// work has been cut fine.
+void plan_pair_tails(std::vector<DevWave> &ds, int grid) {
+  if (tl_tail_policy == PSTGF_TAIL_NONE) return;
+  std::vector<DevWave *> pw;
+  for (DevWave &d : ds)
+    if (d.n_pairs > 0) pw.push_back(&d);
+  if (pw.empty()) return;
+  if (tl_tail_policy == PSTGF_TAIL_ALL) {
+    for (DevWave *d : pw) d->pair_nt_coarse = 0;
+    return;
+  }
+  if (pw.size() == 1 && ds.size() == 1) {
+    DevWave &d = *pw[0];
+    if ((long long)d.pair_mt * d.pair_nt > 16LL * grid) {      // many rounds: one energy tile of fine items is tail enough
+      d.pair_nt_coarse = std::max(0, d.pair_nt - 1);
+      return;
+    }
+    // cached per shape: the simulation costs a millisecond of host time for a few thousand items
+    static std::mutex cache_mutex;
+    static std::map<std::tuple<int, int, int>, int> cache;      // (n_pairs, energy tiles, grid) -> fine energy tiles
+    const auto key = std::make_tuple(d.n_pairs, d.pair_nt, grid);
+    {
+      std::lock_guard<std::mutex> lock(cache_mutex);
+      auto it = cache.find(key);
+      if (it != cache.end()) {
+        d.pair_nt_coarse = d.pair_nt - it->second;
+        return;
+      }
+    }
+    const double c_last = pair_last_tile_blocks(d);
+    std::vector<std::pair<double, int>> runs;
+    int best_t = 0;
+    double best = 0.0;
+    for (int t = 0; t <= d.pair_nt; ++t) {
+      runs.clear();
+      if (d.pair_nt - t > 0) {
+        if (d.pair_mt > 1) runs.emplace_back(16.0, (d.pair_mt - 1) * (d.pair_nt - t));
+        runs.emplace_back(c_last, d.pair_nt - t);
+      }
+      if (t > 0) runs.emplace_back(8.0 * 1.08, d.pair_mtf * t);
+      const double m = simulate_makespan(runs, grid);
+      if (t == 0 || m < best * (1.0 - 1e-9)) {
+        best = m;
+        best_t = t;
+      }
+    }
+    d.pair_nt_coarse = d.pair_nt - best_t;
+    std::lock_guard<std::mutex> lock(cache_mutex);
+    cache[key] = best_t;
+    return;
+  }
+  double budget = 16.0 * grid;                                  // one round of full coarse items, in row blocks
+  for (size_t q = pw.size(); q-- > 0 && budget > 0.0;) {
+    DevWave &d = *pw[q];
+    const double per_tile = 16.0 * (d.pair_mt - 1) + pair_last_tile_blocks(d);   // one energy tile of this wave
+    const int t = (int)std::min<double>((double)d.pair_nt, std::floor(budget / per_tile + 0.5));
+    if (t == 0) break;
+    d.pair_nt_coarse = d.pair_nt - t;
+    budget -= t * per_tile;
+  }
+}
 
 // Cost model in DMMA.8x8x4 per energy (full-size tiles; good enough to size the tail).
 double largest_item_cost(const DevWave &d) {
@@ -243,7 +366,7 @@ void plan_slabs(std::vector<DevWave> &ds, int grid) {
   if (policy == PSTGF_SLAB_NONE) return;
   for (DevWave &d : ds) {
     const int r = d.n_E % pstgf::EB;
-    if (r == 0) continue;
+    if (r == 0 || d.n_pairs > 0) continue;
     int T = policy == PSTGF_SLAB_T32 ? 32 : policy == PSTGF_SLAB_T64 ? 64 : policy == PSTGF_SLAB_T128 ? 128
                                                                            : best_slab_edge(d.n_chan, r, d.n_kt, grid);
     d.n_eb = d.n_E / pstgf::EB;
@@ -263,9 +386,10 @@ pstgf::RingGeo ring_geometry(const std::vector<DevWave> &ds) {
   int bytes = 0;
   for (const DevWave &d : ds) {
     int panels = 0;
-    if (coarse_items(d) + fine_items(d) > 0) panels = pstgf::CLASSIC_PANELS;
+    if (d.n_pairs > 0) panels = pstgf::PAIR_PANELS;
+    else if (coarse_items(d) + fine_items(d) > 0) panels = pstgf::CLASSIC_PANELS;
     if (slab_items(d) > 0) panels = std::max(panels, pstgf::slab_panels(d.slab_T));
-    bytes = std::max(bytes, pstgf::stage_bytes_for(d.tr != 0, panels));
+    bytes = std::max(bytes, pstgf::stage_bytes_for(d.tr != 0 && d.n_pairs == 0, panels));
   }
   pstgf::RingGeo g;
   g.stage_bytes = bytes;
@@ -353,10 +477,10 @@ void plan_tails(std::vector<DevWave> &ds, int grid) {
   }
   double c_max = 0.0;
   for (const DevWave &d : ds)
-    if (d.n_eb > 0) c_max = std::max(c_max, largest_item_cost(d));
+    if (d.n_eb > 0 && d.n_pairs == 0) c_max = std::max(c_max, largest_item_cost(d));
   double budget = c_max * grid;
   if (ds.size() == 1) {
-    if (ds[0].n_eb == 0) return;
+    if (ds[0].n_eb == 0 || ds[0].n_pairs > 0) return;
     const int t = best_tail_single_wave(ds[0], grid, c_max * grid);
     if (t >= 0) {
       ds[0].n_eb_coarse = ds[0].n_eb - t;
@@ -365,7 +489,7 @@ void plan_tails(std::vector<DevWave> &ds, int grid) {
   }
   for (size_t q = ds.size(); q-- > 0 && budget > 0.0;) {
     DevWave &d = ds[q];
-    if (d.n_eb == 0) continue;
+    if (d.n_eb == 0 || d.n_pairs > 0) continue;
     const double per_eb = cost_per_energy_block(d);
     if (largest_item_cost(d) <= 0.45 * c_max) {   // a small wave at the end of the list: its coarse items are fine enough
       budget -= d.n_eb * per_eb;
@@ -403,6 +527,25 @@ pstgf_status_t encode_map(DevWave &d) {
   return PSTGF_OK;
 }
 
+// Tensor maps of the pair form's scratch: P [n_pairs][pair_ld] and D [n_E][pair_ld], boxes of 32 rows x 20 poles.
+pstgf_status_t encode_pair_maps(DevWave &d) {
+  if (d.n_pairs <= 0) return PSTGF_OK;
+  for (int which = 0; which < 2; ++which) {
+    cuuint64_t dims[2] = {(cuuint64_t)d.n_poles, (cuuint64_t)(which ? d.n_E : d.n_pairs)};
+    cuuint32_t box[2] = {(cuuint32_t)pstgf::KT, (cuuint32_t)pstgf::TN};
+    cuuint64_t strides[1] = {(cuuint64_t)d.pair_ld * 8};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = g_encode(which ? &d.map_D : &d.map_P, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, which ? d.pair_D : d.pair_P, dims,
+                          strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                          CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+      tl_cuda_error = (int)cudaErrorInvalidValue;
+      return PSTGF_ERR_CUDA;
+    }
+  }
+  return PSTGF_OK;
+}
+
 // A wave with work for the contraction kernel (n_poles == 0 is a zero-fill instead).
 bool wave_has_items(const pstgf_wave_t &w) { return w.n_chan > 0 && w.n_E > 0 && w.n_poles > 0; }
 
@@ -429,10 +572,53 @@ pstgf_status_t zero_fill(const pstgf_wave_t &w, cudaStream_t s) {
   return PSTGF_OK;
 }
 
+// Device memory of the host call, and the single-wave call's pair-form scratch, come from a pool the library owns (one per device, release threshold =
+// never, freed by pstgf_rmat_finalize): the default pool hands its memory back at every synchronise, and
+// re-growing it costs tens of milliseconds per call.
+std::mutex g_pool_mutex;
+cudaMemPool_t g_pool[64] = {nullptr};
+
+cudaError_t library_pool(int dev, cudaMemPool_t *out) {
+  std::lock_guard<std::mutex> lock(g_pool_mutex);
+  if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+  if (!g_pool[dev]) {
+    cudaMemPoolProps props;
+    std::memset(&props, 0, sizeof(props));
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = dev;
+    cudaMemPool_t pool;
+    cudaError_t e = cudaMemPoolCreate(&pool, &props);
+    if (e != cudaSuccess) return e;
+    unsigned long long keep = ~0ULL;
+    e = cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    if (e != cudaSuccess) { cudaMemPoolDestroy(pool); return e; }
+    g_pool[dev] = pool;
+  }
+  *out = g_pool[dev];
+  return cudaSuccess;
+}
+
 // workspace layout of the batch call
 constexpr size_t WS_COUNTER_BYTES = 256;
 size_t ws_item_begin_bytes(int n_waves) { return ((3 * (size_t)n_waves + 1) * sizeof(long long) + 255) & ~(size_t)255; }
-size_t ws_bytes(int n_waves) { return WS_COUNTER_BYTES + ws_item_begin_bytes(n_waves) + (size_t)n_waves * sizeof(DevWave); }
+size_t ws_tables_bytes(int n_waves) {
+  return (WS_COUNTER_BYTES + ws_item_begin_bytes(n_waves) + (size_t)n_waves * sizeof(DevWave) + 255) & ~(size_t)255;
+}
+// tables, then the scratch (P, D) of every wave that is done in the pair form; force_pair, if given, overrides the
+// per-wave choice (the host call cuts waves into energy ranges and wants every range to go the way of the whole wave)
+size_t ws_bytes(const pstgf_wave_t *waves, int n_waves, const unsigned char *force_pair = nullptr) {
+  size_t b = ws_tables_bytes(n_waves);
+  if (waves)
+    for (int p = 0; p < n_waves; ++p) {
+      const pstgf_wave_t &w = waves[p];
+      if (w.n_chan <= 0 || w.n_E <= 0 || w.n_poles <= 0) continue;
+      const bool pair = force_pair ? force_pair[p] != 0 : wants_pair_form(w.n_chan, w.n_poles, w.n_E);
+      if (pair) b += pair_scratch_bytes(w.n_chan, w.n_poles, w.n_E);
+    }
+  return b;
+}
 
 // ---- work counters of the single-wave call ---------------------------------------------------
 // pstgf_rmat_form has no workspace argument, so its atomic work counter comes from a small pool the library
@@ -507,6 +693,12 @@ pstgf_status_t pstgf_debug_set_tail_policy(int policy) {
   return PSTGF_OK;
 }
 
+pstgf_status_t pstgf_debug_set_pair_policy(int policy) {
+  if (policy < PSTGF_PAIRS_AUTO || policy > PSTGF_PAIRS_ALWAYS) return PSTGF_ERR_INVALID_VALUE;
+  tl_pair_policy = policy;
+  return PSTGF_OK;
+}
+
 pstgf_status_t pstgf_debug_set_slab_policy(int policy) {
   if (policy < PSTGF_SLAB_AUTO || policy > PSTGF_SLAB_T128) return PSTGF_ERR_INVALID_VALUE;
   tl_slab_policy = policy;
@@ -526,27 +718,53 @@ static pstgf_status_t form_single(const pstgf_wave_t &w, void *stream) {
   if (n_poles == 0) return zero_fill(w, s);
   std::vector<DevWave> d(1);
   plan_wave(w, d[0], ds.l2_bytes);
-  plan_slabs(d, ds.sm_count);
-  plan_tails(d, ds.sm_count);
-  st = encode_map(d[0]);
-  if (st != PSTGF_OK) return st;
+  void *scratch = nullptr;
+  if (wants_pair_form(n_chan, n_poles, n_E)) {
+    // the pair form's scratch (P and D) is stream-ordered memory from the library's pool (kept between calls: the
+    // device's default pool hands its memory back at every synchronise): allocated here, freed behind the launch
+    cudaMemPool_t pool;
+    PSTGF_CUDA(library_pool(ds.device, &pool));
+    PSTGF_CUDA(cudaMallocFromPoolAsync(&scratch, pair_scratch_bytes(n_chan, n_poles, n_E), pool, s));
+    plan_pairs(d[0], static_cast<unsigned char *>(scratch));
+    plan_pair_tails(d, ds.sm_count);
+    st = encode_pair_maps(d[0]);
+    if (st == PSTGF_OK) {
+      const int rows = d[0].n_E + d[0].n_pairs;
+      pstgf::pair_build_kernel<false><<<dim3((unsigned)std::min(rows, 8 * ds.sm_count), 1), 256, 0, s>>>(d[0], nullptr, 1);
+      if (cudaGetLastError() != cudaSuccess) st = PSTGF_ERR_CUDA;
+    }
+    if (st != PSTGF_OK) {
+      cudaFreeAsync(scratch, s);
+      return st;
+    }
+    ++tl_launches;
+  } else {
+    plan_slabs(d, ds.sm_count);
+    plan_tails(d, ds.sm_count);
+    st = encode_map(d[0]);
+    if (st != PSTGF_OK) return st;
+  }
+  const int build_launches = tl_launches;
   const long long n_items = wave_items(d[0]);
   const int grid = (int)std::min<long long>(ds.sm_count, n_items);
   const pstgf::RingGeo geo = ring_geometry(d);
   {
     std::lock_guard<std::mutex> lock(g_counter_mutex);
     unsigned long long *counter = nullptr;
-    const int slot = acquire_counter(ds.device, s, &counter);
+    // no more items than CTAs: item b goes to CTA b, no counter needed (one L2 round trip less for the tiny calls)
+    const int slot = n_items <= grid ? -1 : acquire_counter(ds.device, s, &counter);
     pstgf::rmat_persistent_kernel<false><<<grid, pstgf::NUM_THREADS, pstgf::smem_bytes_for(geo), s>>>(
         d[0], nullptr, nullptr, 1, n_items, counter, geo);
-    PSTGF_CUDA(cudaGetLastError());
+    const cudaError_t le = cudaGetLastError();
+    if (scratch) cudaFreeAsync(scratch, s);
+    PSTGF_CUDA(le);
     if (slot >= 0) {
       CounterPool &cp = g_counters[ds.device];
       PSTGF_CUDA(cudaEventRecord(cp.ev[slot], s));
       cp.armed[slot] = true;
     }
   }
-  tl_launches = 1;
+  tl_launches = build_launches + 1;
   return PSTGF_OK;
 }
 
@@ -563,8 +781,7 @@ pstgf_status_t pstgf_rmat_form_hdat(const double *Wt, long long ldw, const doubl
 }
 
 size_t pstgf_rmat_batch_workspace_bytes(const pstgf_wave_t *waves, int n_waves) {
-  (void)waves;
-  return n_waves > 0 ? ws_bytes(n_waves) : 0;
+  return n_waves > 0 ? ws_bytes(waves, n_waves) : 0;
 }
 
 // What the host-buffer call needs to know about a batch launch to copy the waves back as they finish.
@@ -574,6 +791,7 @@ struct BatchCompletion {
   const unsigned int *const *rows_ready = nullptr;   // in, optional: per input wave, the upload counter of its W
   const int *ready_counts_channels = nullptr;        // ... and what it counts (DevWave::ready_counts_channels)
   unsigned int *abort_flag = nullptr;                // in: host-mapped word a load warp sets when an upload wait times out
+  const unsigned char *force_pair = nullptr;         // in, optional: per input wave, 1 = pair form, 0 = SYRK form
   std::vector<int> order;                // out: input wave indices in the order the launch completes them
   std::vector<long long> items;          // out: items of each input wave (arrivals = items * EB)
 };
@@ -588,7 +806,8 @@ static pstgf_status_t form_batch_impl(const pstgf_wave_t *waves, int n_waves, vo
     pstgf_status_t st = check_wave(waves[p]);
     if (st != PSTGF_OK) return st;
   }
-  if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) != 0 || workspace_bytes < ws_bytes(n_waves))
+  const unsigned char *force_pair = completion ? completion->force_pair : nullptr;
+  if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) != 0 || workspace_bytes < ws_bytes(waves, n_waves, force_pair))
     return PSTGF_ERR_WORKSPACE;
   DeviceState dstate;
   pstgf_status_t st = device_state(dstate);
@@ -618,11 +837,25 @@ static pstgf_status_t form_batch_impl(const pstgf_wave_t *waves, int n_waves, vo
   std::vector<unsigned char> img(off_waves + (size_t)nw * sizeof(DevWave), 0);
   long long *item_begin = reinterpret_cast<long long *>(img.data() + off_begin);
   std::vector<DevWave> ds((size_t)nw);
+  unsigned char *ws = static_cast<unsigned char *>(workspace);
+  size_t scratch_off = ws_tables_bytes(n_waves);
+  int n_pair_waves = 0, max_build_rows = 0;
   for (int q = 0; q < nw; ++q) {
-    plan_wave(waves[order[q]], ds[q], dstate.l2_bytes);
+    const pstgf_wave_t &w = waves[order[q]];
+    plan_wave(w, ds[q], dstate.l2_bytes);
+    const bool pair = force_pair ? force_pair[order[q]] != 0 : wants_pair_form(w.n_chan, w.n_poles, w.n_E);
+    if (pair) {
+      plan_pairs(ds[q], ws + scratch_off);
+      scratch_off += pair_scratch_bytes(w.n_chan, w.n_poles, w.n_E);
+      ++n_pair_waves;
+      max_build_rows = std::max(max_build_rows, ds[q].n_E + ds[q].n_pairs);
+      st = encode_pair_maps(ds[q]);
+      if (st != PSTGF_OK) return st;
+    }
   }
   plan_slabs(ds, dstate.sm_count);
   plan_tails(ds, dstate.sm_count);
+  plan_pair_tails(ds, dstate.sm_count);
   if (completion && completion->done)
     for (int q = 0; q < nw; ++q) {
       ds[q].done = completion->done[order[q]];
@@ -648,8 +881,10 @@ static pstgf_status_t form_batch_impl(const pstgf_wave_t *waves, int n_waves, vo
   }
   long long total = 0;
   for (int q = 0; q < nw; ++q) {
-    st = encode_map(ds[q]);
-    if (st != PSTGF_OK) return st;
+    if (ds[q].n_pairs == 0) {
+      st = encode_map(ds[q]);
+      if (st != PSTGF_OK) return st;
+    }
     std::memcpy(img.data() + off_waves + (size_t)q * sizeof(DevWave), &ds[q], sizeof(DevWave));
     item_begin[q] = total;
     total += coarse_items(ds[q]);
@@ -663,8 +898,16 @@ static pstgf_status_t form_batch_impl(const pstgf_wave_t *waves, int n_waves, vo
     total += fine_items(ds[q]);
   }
   item_begin[3 * nw] = total;
-  unsigned char *ws = static_cast<unsigned char *>(workspace);
   PSTGF_CUDA(cudaMemcpyAsync(ws, img.data(), img.size(), cudaMemcpyHostToDevice, s));
+  if (n_pair_waves > 0) {
+    // P and D of every pair-form wave in one launch (grid.y = the waves of the launch; the others return at once)
+    DevWave none;
+    std::memset(&none, 0, sizeof(none));
+    const int bx = std::max(1, std::min(max_build_rows, std::max(8, 8 * dstate.sm_count / nw)));
+    pstgf::pair_build_kernel<true><<<dim3((unsigned)bx, (unsigned)std::min(nw, 65535)), 256, 0, s>>>(none, reinterpret_cast<const DevWave *>(ws + off_waves), nw);
+    PSTGF_CUDA(cudaGetLastError());
+    ++launches;
+  }
   const int grid = (int)std::min<long long>(dstate.sm_count, total);
   const pstgf::RingGeo geo = ring_geometry(ds);
   DevWave dummy;
@@ -718,34 +961,6 @@ pstgf_status_t pstgf_mesh_from_zscaled(const double *e_scaled, long long n, doub
 namespace {
 constexpr int HOST_RING = 3;          // R staging buffers in flight
 constexpr int HOST_COMPUTE_STREAMS = 2;
-
-// Device memory of the host call comes from a pool the library owns (one per device, release threshold =
-// never, freed by pstgf_rmat_finalize): the default pool hands its memory back at every synchronise, and
-// re-growing it costs tens of milliseconds per call.
-std::mutex g_pool_mutex;
-cudaMemPool_t g_pool[64] = {nullptr};
-
-cudaError_t host_call_pool(int dev, cudaMemPool_t *out) {
-  std::lock_guard<std::mutex> lock(g_pool_mutex);
-  if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
-  if (!g_pool[dev]) {
-    cudaMemPoolProps props;
-    std::memset(&props, 0, sizeof(props));
-    props.allocType = cudaMemAllocationTypePinned;
-    props.handleTypes = cudaMemHandleTypeNone;
-    props.location.type = cudaMemLocationTypeDevice;
-    props.location.id = dev;
-    cudaMemPool_t pool;
-    cudaError_t e = cudaMemPoolCreate(&pool, &props);
-    if (e != cudaSuccess) return e;
-    unsigned long long keep = ~0ULL;
-    e = cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-    if (e != cudaSuccess) { cudaMemPoolDestroy(pool); return e; }
-    g_pool[dev] = pool;
-  }
-  *out = g_pool[dev];
-  return cudaSuccess;
-}
 
 constexpr size_t MAX_CHUNK_SEGMENTS = 4096;
 
@@ -862,7 +1077,7 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
   HostCallResources res;
   res.s = static_cast<cudaStream_t>(stream);
   cudaMemPool_t pool;
-  PSTGF_CUDA(host_call_pool(ds.device, &pool));
+  PSTGF_CUDA(library_pool(ds.device, &pool));
   PSTGF_CUDA(cudaStreamCreateWithFlags(&res.copy, cudaStreamNonBlocking));
   for (cudaStream_t &c : res.compute) PSTGF_CUDA(cudaStreamCreateWithFlags(&c, cudaStreamNonBlocking));
   PSTGF_CUDA(cudaEventCreateWithFlags(&res.inputs, cudaEventDisableTiming));
@@ -897,6 +1112,10 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
                              (size_t)w.n_chan, cudaMemcpyHostToDevice, res.s);   // a column range of every channel
   };
   std::vector<int> by_channels((size_t)n_waves, 0);
+  // waves done in the pair form: decided on the WHOLE wave (every energy range of it then goes the same way, so the
+  // host call gives the bits of the device calls), and their W is uploaded before the launches (P is built from all of it)
+  std::vector<unsigned char> pair_wave((size_t)n_waves, 0);
+  for (int p = 0; p < n_waves; ++p) pair_wave[(size_t)p] = wants_pair_form(waves[p].n_chan, waves[p].n_poles, waves[p].n_E) ? 1 : 0;
   for (int p = 0; p < n_waves; ++p) {
     const pstgf_wave_t &w = waves[p];
     if (w.n_chan == 0 || w.n_E == 0) continue;
@@ -927,7 +1146,7 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
     dev[p].ldw = pitch;
     dev[p].E_k = static_cast<double *>(dEk);
     dev[p].energies = static_cast<double *>(dEn);
-    if (!overlap_upload) PSTGF_CUDA(upload_W(p, 0, w.n_poles, false));
+    if (!overlap_upload || pair_wave[(size_t)p]) PSTGF_CUDA(upload_W(p, 0, w.n_poles, false));
   }
   // Two ways to overlap the copy-back with the formation (pstgf_debug_set_host_pipeline):
   //  signalled  ONE launch forms a whole chunk (as much of R as the device budget allows); its segments (a wave's
@@ -1000,7 +1219,13 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
   size_t wsb = 0;
   for (int attempt = 0;; ++attempt) {
     ring = (int)std::min<size_t>(signalled ? 2 : HOST_RING, chunks.size());
-    wsb = ws_bytes((int)max_segs);
+    wsb = 0;     // tables plus the pair-form scratch of the chunk that needs the most
+    for (const auto &ch : chunks) {
+      size_t b = ws_tables_bytes((int)max_segs);
+      for (const Segment &g : ch)
+        if (pair_wave[(size_t)g.wave]) b += pair_scratch_bytes(waves[g.wave].n_chan, waves[g.wave].n_poles, g.ne);
+      wsb = std::max(wsb, b);
+    }
     cudaError_t e = cudaSuccess;
     int got = 0;
     for (; got < ring && e == cudaSuccess; ++got) {
@@ -1031,7 +1256,7 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
   if (overlap_upload) {
     for (int p = 0; p < n_waves; ++p) {
       const pstgf_wave_t &w = waves[p];
-      if (!wave_has_items(w)) continue;
+      if (!wave_has_items(w) || pair_wave[(size_t)p]) continue;
       const size_t bytes = sizeof(double) * (size_t)w.n_chan * (size_t)w.n_poles;
       // Slabs of poles when the upload takes no more than about two item times (~1.4 us per k-tile of 20 poles,
       // ~50 GB/s): the first items' k loops then hide it.  Otherwise slabs of channels, if W's rows are channels.
@@ -1056,6 +1281,7 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
   std::vector<unsigned int *> done, flag;
   std::vector<const unsigned int *> rows_ready;
   std::vector<int> ready_kind;
+  std::vector<unsigned char> force;
   BatchCompletion completion;
   for (size_t c = 0; c < chunks.size(); ++c) {
     const int b = (int)(c % ring);
@@ -1066,6 +1292,7 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
     flag.clear();
     rows_ready.clear();
     ready_kind.clear();
+    force.clear();
     const size_t f0 = (size_t)b * MAX_CHUNK_SEGMENTS;
     for (const Segment &g : chunks[c]) {
       pstgf_wave_t w = dev[g.wave];
@@ -1074,10 +1301,11 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
       w.n_E = g.ne;
       w.R_out = reinterpret_cast<double *>(static_cast<unsigned char *>(rbuf[b]) + g.off);
       sub.push_back(w);
+      force.push_back(pair_wave[(size_t)g.wave]);
       if (signalled) {
         done.push_back(flags.counters + f0 + (sub.size() - 1));
         flag.push_back(flags.flags_dev + f0 + (sub.size() - 1));
-        rows_ready.push_back(overlap_upload ? flags.upload_counters + g.wave : nullptr);
+        rows_ready.push_back(overlap_upload && !pair_wave[(size_t)g.wave] ? flags.upload_counters + g.wave : nullptr);
         ready_kind.push_back(by_channels[(size_t)g.wave]);
       }
     }
@@ -1096,6 +1324,7 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
       completion.rows_ready = rows_ready.data();
       completion.ready_counts_channels = ready_kind.data();
       completion.abort_flag = flags.flags_dev + 2 * MAX_CHUNK_SEGMENTS;
+      completion.force_pair = force.data();
       st = form_batch_impl(sub.data(), (int)sub.size(), wsbuf[b], wsb, cs, &completion);
       if (st != PSTGF_OK) return st;
       launches += tl_launches;
@@ -1122,7 +1351,9 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
         return PSTGF_ERR_TIMEOUT;
       }
     } else {
-      st = pstgf_rmat_form_batch(sub.data(), (int)sub.size(), wsbuf[b], wsb, cs);
+      BatchCompletion plain;
+      plain.force_pair = force.data();
+      st = form_batch_impl(sub.data(), (int)sub.size(), wsbuf[b], wsb, cs, &plain);
       if (st != PSTGF_OK) return st;
       launches += tl_launches;
       PSTGF_CUDA(cudaEventRecord(res.computed[b], cs));

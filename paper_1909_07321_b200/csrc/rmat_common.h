@@ -26,6 +26,15 @@
 //                block: square tiles S(i, j), j >= i, of edge T = 128, 64 or 32 chosen by the planner so that
 //                there are enough items for the grid; the 8 / g warps of one energy each take a slab of the
 //                tile (SlabShape below).  Same operands, same k order: same bits as inside a block of 8.
+//   pair items   waves with FEW channels (n_chan <= PAIR_MAX_CHAN) and enough energies are not done in the SYRK form
+//                above at all: an n_chan x n_chan tile there computes whole 8x8 blocks across the diagonal (36
+//                blocks for 32 counted at n_chan = 64, 1 for 1/2 at n_chan = 8) and pays a scaling multiply
+//                for every few DMMAs.  Eq. 4 is also the plain GEMM over channel PAIRS
+//                    R[e][(n,m)] = (1/2a) sum_k P[(n,m)][k] * D[e][k],   P = w_nk w_mk,  D = 1/(E_k - E_e),
+//                with the n_chan (n_chan + 1) / 2 pairs n <= m as rows and the energies as columns: no block is
+//                cut by a diagonal and nothing is scaled inside the k loop.  P (once per wave) and D (once per
+//                energy) are written to scratch by a small kernel first; an item is (128 or 64 pairs) x 128 energies,
+//                each of the eight warps taking 16 energies (the WIDE register tile, 16 x 2 blocks).
 // Only tiles on or above the diagonal exist ("half of the symmetric R-matrix"),
 // the mirror is written by the epilogue ("symmetrised").
 #pragma once
@@ -72,6 +81,11 @@ struct StageLayout {
 constexpr int stage_bytes_for(bool tr, int panels) { return D_BYTES + panels * (tr ? TR_BOX_BYTES : BOX_BYTES); }
 constexpr int CLASSIC_PANELS = TW / TN + 1;          // 5
 constexpr int slab_panels(int T) { return 2 * (T / TN); }   // 8, 4, 2 for slab tiles of edge 128, 64, 32
+// Pair form (see above): pair tiles of 128 (coarse) or 64 (fine tail) rows of P, energy tiles of 128 rows of D.
+constexpr int PAIR_MAX_CHAN = 96;        // 4656 pairs; P is 71 MB at n_poles = 20 n_chan
+constexpr int PAIR_MIN_E = 64;           // fewer energies than this do not fill an energy tile's eight warps
+constexpr int PT_M = 128, PT_MF = 64, PT_N = 128;
+constexpr int PAIR_PANELS = (PT_M + PT_N) / TN;             // 8
 
 // Shared memory of a CTA: [mbarriers | two ItemInfo slots | ring of n_stages stages]; the ring geometry is a launch
 // parameter (RingGeo) because slab tiles of edge 128 need 8 panels per stage instead of 5.
@@ -103,6 +117,8 @@ __host__ __device__ inline SlabShape slab_shape(int T, int g) {
 // space (single-wave call) or in the caller's workspace (batch call).
 struct alignas(128) DevWave {
   CUtensorMap map;         // W viewed as [n_chan][n_poles] (row stride ldw*8), box [TN][KT], no swizzle (tr: see below)
+  CUtensorMap map_P;       // pair form: P viewed as [n_pairs][n_poles] (row stride pair_ld*8), box [TN][KT]
+  CUtensorMap map_D;       // pair form: D viewed as [n_E][n_poles] (row stride pair_ld*8), box [TN][KT]
   const double *W;
   const double *E_k;
   const double *energies;
@@ -131,8 +147,19 @@ struct alignas(128) DevWave {
   int slab_nt;             // ceil(n_chan / slab_T): slab tiles = slab_nt (slab_nt + 1) / 2
   int l2_keep;             // W fits half of L2: load it with the evict_last policy so that R's stores do not push it out
   unsigned int wait_timeout_ms;   // bound on a load warp's wait for an upload slab (0 = 2000)
+  // pair form (n_pairs > 0: this wave has pair items and no others)
+  double *pair_P;          // scratch [n_pairs][pair_ld]: P[(n,m)][k] = w_nk w_mk, pairs row by row over the upper triangle
+  double *pair_D;          // scratch [n_E][pair_ld]:     D[e][k] = 1/(E_k - E_e)
+  long long pair_ld;       // even, >= n_poles
+  int n_pairs;             // n_chan (n_chan + 1) / 2, or 0 when the wave is done in the SYRK form
+  int pair_nt;             // energy tiles of PT_N
+  int pair_nt_coarse;      // energy tiles [0, pair_nt_coarse) are cut into pair tiles of PT_M rows, the rest (the tail) of PT_MF
+  int pair_mt, pair_mtf;   // pair tiles of PT_M / of PT_MF rows
+  int pair_nfb;            // n_chan / 8: channel blocks that are full
+  int pair_rb;             // rows of P in the block section: 64 pair_nfb (pair_nfb - 1) / 2, see pair_row_channels
+  const unsigned int *pair_nm;   // scratch [n_pairs]: n | m << 16 of every row of P (written by the scratch builder)
 };
-static_assert(sizeof(DevWave) == 384, "DevWave layout (alignas 128; the batch workspace holds an array of these)");
+static_assert(sizeof(DevWave) == 640, "DevWave layout (alignas 128; the batch workspace holds an array of these)");
 
 // Host-side tile arithmetic (also used by the kernel's decoder).
 // WIDE tiles of row pair p: columns from 128 (p + 1) to the end, 16 at a time.
@@ -153,6 +180,38 @@ __host__ __device__ inline int coarse_tiles(int n_chan) {
 }
 // Fine tiling: n_j row/column panels of 32; OFF32 tiles first (n_j (n_j - 1) / 2), then DIAG32 (n_j).
 __host__ __device__ inline int fine_tiles(int n_j) { return n_j * (n_j - 1) / 2 + n_j; }
+// Order of the pairs (n, m), n <= m, as rows of P.  First the BLOCK section: the off-diagonal 8 x 8 blocks of
+// channels (bn < bm < nfb = C / 8) one after the other, (0,1), (0,2), ..., (1,2), ..., 64 rows each, row 8 j + i of
+// a block being the pair (8 bn + j, 8 bm + i).  A warp's 8 x 8 accumulator blocks of such a group then hold an
+// 8 x 8 patch of R: R[n][m .. m+7] lies across eight lanes (a 64-byte run) and the mirror R[m][n .. n+7] in ONE lane's
+// eight accumulators (a 64-byte run again, vector stores) -- both triangles are written in full sectors.  Then the
+// LOOSE section: what is left (the triangles of the diagonal blocks and the strip of a ragged last block), row by
+// row of the upper triangle; those rows go through a table (DevWave::pair_nm) and are stored element by element.
+__host__ __device__ inline int pair_block_rows(int C) { const int nfb = C / 8; return 64 * (nfb * (nfb - 1) / 2); }
+// loose pairs of channel row n: m from n to the end of n's own 8-block, plus the ragged strip m >= 8 nfb
+__host__ __device__ inline int pair_loose_in_row(int n, int C) {
+  const int nfb = C / 8, own_end = (n / 8 + 1) * 8 < C ? (n / 8 + 1) * 8 : C;
+  return (own_end - n) + (n / 8 < nfb && 8 * nfb < C && own_end <= 8 * nfb ? C - 8 * nfb : 0);
+}
+// row r of P -> (n, m); O(C) for loose rows (used by the scratch builder, which records the answer in pair_nm)
+__host__ __device__ inline void pair_row_channels(int r, int C, int &n, int &m) {
+  const int nfb = C / 8, rb = pair_block_rows(C);
+  if (r < rb) {
+    int blk = r >> 6, bn = 0;
+    while (blk >= nfb - 1 - bn) { blk -= nfb - 1 - bn; ++bn; }
+    n = 8 * bn + ((r >> 3) & 7);
+    m = 8 * (bn + 1 + blk) + (r & 7);
+    return;
+  }
+  int l = r - rb;
+  for (n = 0; n < C - 1; ++n) {
+    const int cnt = pair_loose_in_row(n, C);
+    if (l < cnt) break;
+    l -= cnt;
+  }
+  const int own_end = (n / 8 + 1) * 8 < C ? (n / 8 + 1) * 8 : C;
+  m = l < own_end - n ? n + l : 8 * nfb + (l - (own_end - n));
+}
 // Slab tiling: nt row/column panels of T; tiles row by row over the upper triangle, (0,0), (0,1), ..., (1,1), ...
 __host__ __device__ inline int slab_tiles(int nt) { return nt * (nt + 1) / 2; }
 

@@ -29,9 +29,12 @@ struct alignas(16) ItemInfo {   // handed from the load warp to the pole-scaling
   int n_poles;
   int n_valid_e;           // energies of this item (1..EB; slab items: 2 or 1)
   int row0, col0;
-  int nblk;                // DIAG: valid 8x8 block rows/cols; rectangular tiles: valid 8-wide column blocks
+  int nblk;                // DIAG: valid 8x8 block rows/cols; rectangular tiles: valid 8-wide column blocks; pair items: row blocks
   int n_kt;
-  short kind;              // 0 on the diagonal (DIAG / slab S(i,i)), 1 strictly above it, -1 stop
+  int n_pairs;             // pair items: rows of P (row0 = first pair of the tile, col0 = first energy of the tile)
+  int pair_rb;             // pair items: rows of P in the block section (rmat_common.h)
+  const unsigned int *pair_nm;   // pair items: n | m << 16 of every row of P
+  short kind;              // 0 on the diagonal (DIAG / slab S(i,i)), 1 strictly above it, 2 pair item, -1 stop
   unsigned char nrb;       // classic rectangular tiles: 8-row blocks of the I panel (16 WIDE, 8 OFF, 4 fine OFF32)
   unsigned char tr;        // stage layout: 0 row-major panels, 1 pole-major panels (channel-contiguous W)
   unsigned char slab_T;    // 0: classic item (one energy per warp); else the edge of the slab tile (32, 64, 128)
@@ -401,6 +404,110 @@ __device__ __forceinline__ void consume_slab(const ItemInfo &it, Pipe &ps, int w
   }
 }
 
+// Pair item: NR row blocks of P (8 pairs each) x 128 energies; this warp's 16 energies are rows [16 warp, +16) of the
+// D panels.  acc[pair][energy] += P[pair][k] * D[energy][k]: a plain GEMM, nothing is scaled inside the loop and no
+// block is cut by a diagonal.  The epilogue scatters pair (n, m) of energy e to R[e][n][m] and R[e][m][n].
+template <int NR>
+__device__ __forceinline__ void consume_pair(const ItemInfo &it, Pipe &ps, int warp, int lane) {
+  using L = StageLayout<false>;
+  if (warp * 16 >= it.n_valid_e) {
+    consume_idle(it.n_kt, ps, lane);
+    return;
+  }
+  const int g = lane >> 2, q = lane & 3;
+  const int aoff = L::W_BASE + L::off(g, q);
+  const int boff = L::W_BASE + L::off(PT_M + warp * 16, 0) + L::off(g, q);
+  double acc[NR][2][2];
+#pragma unroll
+  for (int bi = 0; bi < NR; ++bi) acc[bi][0][0] = acc[bi][0][1] = acc[bi][1][0] = acc[bi][1][1] = 0.0;
+  for (int kt = 0; kt < it.n_kt; ++kt) {
+    mbar_wait(ps.full(), ps.phase);
+    const double *st = ps.stage_ptr();
+    const double *wa = st + aoff;
+    const double *wb = st + boff;
+#pragma unroll
+    for (int ks = 0; ks < KT / 4; ++ks) {
+      double a[NR];
+#pragma unroll
+      for (int bi = 0; bi < NR; ++bi) a[bi] = wa[L::off(bi * 8, ks * 4)];
+#pragma unroll
+      for (int c = 0; c < 2; ++c) {
+        const double b = wb[L::off(c * 8, ks * 4)];
+#pragma unroll
+        for (int bi = 0; bi < NR; ++bi) dmma884(acc[bi][c][0], acc[bi][c][1], a[bi], b);
+      }
+    }
+    release_stage(ps, lane);
+    ps.advance();
+  }
+  // epilogue: lane (g, q) holds row row0 + 8 bi + g of P at energies col0 + 16 warp + 8 c + 2 q + {0, 1}
+  const int C = it.n_chan;
+  const size_t cc = (size_t)C * C;
+  const double sc = it.inv2a;
+  const int nfb = C / 8;
+#pragma unroll
+  for (int grp = 0; grp < (NR + 7) / 8; ++grp) {            // groups of 64 rows: each is one 8 x 8 channel block, or loose
+    const int r0 = it.row0 + grp * 64;
+    if (NR >= 8 && r0 + 64 <= it.pair_rb) {
+      // block section: rows 8 j + i of the group are the pairs (8 bn + j, 8 bm + i); this lane holds i = g
+      int blk = r0 >> 6, bn = 0;
+      while (blk >= nfb - 1 - bn) { blk -= nfb - 1 - bn; ++bn; }
+      const int n0 = 8 * bn, m = 8 * (bn + 1 + blk) + g;
+#pragma unroll
+      for (int c = 0; c < 2; ++c) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          const int el = warp * 16 + c * 8 + 2 * q + h;       // energy inside the tile
+          if (el < it.n_valid_e) {
+            double *R = it.R + (size_t)el * cc;
+            double v[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+              v[j] = acc[(grp * 8 + j) % NR][c][h] * sc;
+              __stcs(R + (size_t)(n0 + j) * C + m, v[j]);       // R[n][m .. m+7] across the eight lanes g: a 64-byte run
+            }
+            double *mir = R + (size_t)m * C + n0;               // R[m][n0 .. n0+7]: this lane's own 64-byte run
+            if ((reinterpret_cast<uintptr_t>(mir) & 15u) == 0) {
+#pragma unroll
+              for (int j = 0; j < 8; j += 2) __stcs(reinterpret_cast<double2 *>(mir + j), make_double2(v[j], v[j + 1]));
+            } else {
+#pragma unroll
+              for (int j = 0; j < 8; ++j) __stcs(mir + j, v[j]);
+            }
+          }
+        }
+      }
+    } else {
+      // loose section (diagonal blocks' triangles, ragged last block): element by element through the table
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const int bi = grp * 8 + j;
+        if (bi < NR) {
+          const int idx = it.row0 + bi * 8 + g;
+          if (idx < it.n_pairs) {
+            const unsigned int nm = __ldg(it.pair_nm + idx);
+            const int n = (int)(nm & 0xffffu), m = (int)(nm >> 16);
+#pragma unroll
+            for (int c = 0; c < 2; ++c) {
+#pragma unroll
+              for (int h = 0; h < 2; ++h) {
+                const int el = warp * 16 + c * 8 + 2 * q + h;
+                if (el < it.n_valid_e) {
+                  double v = acc[bi][c][h] * sc;
+                  if (n == m && it.diag_add) v += __ldg(it.diag_add + (size_t)el * C + n);
+                  double *R = it.R + (size_t)el * cc;
+                  __stcs(R + (size_t)n * C + m, v);
+                  if (n != m) __stcs(R + (size_t)m * C + n, v);
+                }
+              }
+            }
+          }
+        }
+      }
+    }
+  }
+}
+
 // The tile shapes are compile-time variants (no predicates inside the DMMA loop); ragged edges of
 // a wave pick the variant with fewer 8-wide blocks.
 template <bool TR>
@@ -454,6 +561,12 @@ __device__ __forceinline__ void consume_item_layout(const ItemInfo &it, Pipe &ps
 }
 
 __device__ __forceinline__ void consume_item(const ItemInfo &it, Pipe &ps, int warp, int lane) {
+  if (it.kind == 2) {
+    if (it.nblk == 16) consume_pair<16>(it, ps, warp, lane);
+    else if (it.nblk == 8) consume_pair<8>(it, ps, warp, lane);
+    else consume_pair<4>(it, ps, warp, lane);
+    return;
+  }
   if (it.tr) consume_item_layout<true>(it, ps, warp, lane);
   else consume_item_layout<false>(it, ps, warp, lane);
 }
@@ -594,16 +707,20 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
       // ---- load warp: takes work items, publishes them, stages the W panels (S2, S5) ----
       uint32_t iq = 0, iphase = 0;
       long long next_static = blockIdx.x;
+      unsigned long long next_drawn = 0;        // lane 0: the item this CTA does next (drawn ahead of time)
+      if (counter != nullptr && lane == 0) next_drawn = atomicAdd(counter, 1ULL);
+      int last_section = 0;
+      constexpr int DRAW_AHEAD = 6;             // stages before the end of an item's loads at which the next item is drawn
       const uint64_t keep_policy = l2_policy_evict_last(), normal_policy = l2_policy_evict_normal();
       int last_wave = -1;
       for (;;) {
         // items are drawn from an atomic counter (batch call: in the workspace; single-wave call: a slot of
-        // the library's counter pool), or round-robin when the single-wave call found no free slot
+        // the library's counter pool), or round-robin when the single-wave call found no free slot.  The draw for
+        // the NEXT item was issued a few stages before the end of the previous item's loads (below), so its
+        // round trip to L2 is off the critical path of short items.
         long long item;
         if (counter != nullptr) {
-          unsigned long long got = 0;
-          if (lane == 0) got = atomicAdd(counter, 1ULL);
-          item = (long long)__shfl_sync(0xffffffffu, got, 0);
+          item = (long long)__shfl_sync(0xffffffffu, next_drawn, 0);
         } else {
           item = next_static;
           next_static += gridDim.x;
@@ -613,17 +730,20 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
         int p = 0, sec = 0;
         if (!stop) {
           if (BATCH) {
-            int lo = 0, hi = 3 * n_waves;        // item_begin[lo] <= item < item_begin[hi]
-            while (hi - lo > 1) {
-              const int mid = (lo + hi) >> 1;
-              if (__ldg(item_begin + mid) <= item) lo = mid; else hi = mid;
+            // the counter only goes up, so the section of this CTA's next item is never before the last one's:
+            // a short scan forward instead of a binary search (ten dependent loads from L2 per item)
+            int lo = last_section;               // item_begin[lo] <= item < item_begin[3 n_waves]
+            while (lo + 1 < 3 * n_waves && __ldg(item_begin + lo + 1) <= item) {
+              lo = lo + 16 < 3 * n_waves && __ldg(item_begin + lo + 16) <= item ? lo + 16 : lo + 1;
             }
+            last_section = lo;
             item -= __ldg(item_begin + lo);
             sec = lo / n_waves;
             p = lo - sec * n_waves;
           } else {
-            const long long n_coarse = (long long)single.n_tiles * single.n_eb_coarse;
-            const long long n_slab = (long long)slab_tiles(single.slab_nt) * (single.slab_g2 + single.slab_g1);
+            const bool sp = single.n_pairs > 0;
+            const long long n_coarse = sp ? (long long)single.pair_mt * single.pair_nt_coarse : (long long)single.n_tiles * single.n_eb_coarse;
+            const long long n_slab = sp ? 0 : (long long)slab_tiles(single.slab_nt) * (single.slab_g2 + single.slab_g1);
             if (item >= n_coarse + n_slab) { sec = 2; item -= n_coarse + n_slab; }
             else if (item >= n_coarse) { sec = 1; item -= n_coarse; }
           }
@@ -631,7 +751,21 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
         const DevWave &w = BATCH ? waves[p] : single;
         int kind = -1, row0 = 0, col0 = 0, nblk = 0, nrb = 0, e_first = 0, n_valid = 0, n_kt = 0, slab_T = 0, slab_g = 0;
         if (!stop) {
-          if (sec == 1) {
+          if (w.n_pairs > 0) {
+            // pair form: section 0 holds the wave's (128-pair tile, energy tile) items, section 2 its fine tail
+            // (64-pair tiles of the last energy tiles); energy tile fastest, so CTAs side by side share a P panel
+            const bool fine = sec == 2;
+            const int n_nt_sec = fine ? w.pair_nt - w.pair_nt_coarse : w.pair_nt_coarse;
+            const int mt = (int)(item / n_nt_sec);
+            const int nt = (int)(item - (long long)mt * n_nt_sec) + (fine ? w.pair_nt_coarse : 0);
+            kind = 2;
+            row0 = mt * (fine ? PT_MF : PT_M);
+            col0 = nt * PT_N;
+            const int left = w.n_pairs - row0;
+            nblk = left > 64 && !fine ? 16 : left > 32 ? 8 : 4;
+            e_first = col0;
+            n_valid = min(PT_N, w.n_E - col0);
+          } else if (sec == 1) {
             const int n_groups = w.slab_g2 + w.slab_g1;
             const int tile = (int)(item / n_groups);
             const int gi = (int)(item - (long long)tile * n_groups);
@@ -675,7 +809,10 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
             ii.row0 = row0;
             ii.col0 = col0;
             ii.nrb = (unsigned char)nrb;
-            ii.tr = (unsigned char)w.tr;
+            ii.tr = (unsigned char)(kind == 2 ? 0 : w.tr);
+            ii.n_pairs = w.n_pairs;
+            ii.pair_rb = w.pair_rb;
+            ii.pair_nm = w.pair_nm;
             ii.slab_T = (unsigned char)slab_T;
             ii.slab_g = (unsigned char)slab_g;
             ii.nblk = nblk;
@@ -687,16 +824,28 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
         if (iq == 0) iphase ^= 1u;
         if (stop) break;
 
+        const bool pair = kind == 2;
         const CUtensorMap *map = &w.map;
-        if (BATCH && w.use_tma && p != last_wave) {
-          if (lane == 0) tensormap_acquire(map);
+        if (BATCH && (w.use_tma || pair) && p != last_wave) {
+          if (lane == 0) {
+            if (pair) {
+              tensormap_acquire(&w.map_P);
+              tensormap_acquire(&w.map_D);
+            } else {
+              tensormap_acquire(map);
+            }
+          }
           __syncwarp();
           last_wave = p;
         }
         // panels of 32 channels to stage: I rows [row0, ...) into panels [0, i_boxes), J rows [col0, ...) into
         // panels [j_panel0, j_panel0 + j_boxes); boxes that lie wholly beyond n_chan are not loaded (nothing reads them)
         int i_boxes, j_boxes, j_panel0;
-        if (slab_T != 0) {
+        if (pair) {
+          i_boxes = (min(nblk * 8, w.n_pairs - row0) + TN - 1) / TN;      // rows of P
+          j_boxes = (n_valid + TN - 1) / TN;                               // rows of D
+          j_panel0 = PT_M / TN;
+        } else if (slab_T != 0) {
           i_boxes = (min(slab_T, w.n_chan - row0) + TN - 1) / TN;
           j_boxes = kind != 0 ? (min(slab_T, w.n_chan - col0) + TN - 1) / TN : 0;
           j_panel0 = slab_T / TN;
@@ -705,11 +854,11 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
           j_boxes = kind != 0 ? 1 : 0;
           j_panel0 = TW / TN;
         }
-        const uint32_t box = w.tr ? TR_BOX_BYTES : BOX_BYTES;
+        const uint32_t box = (w.tr && !pair) ? TR_BOX_BYTES : BOX_BYTES;
         const uint32_t tx_bytes = (uint32_t)(i_boxes + j_boxes) * box;
         // host-buffer call: W uploaded so far.  Slabs of channels are waited for here, once per item (the rows and
         // columns of its tile); slabs of poles stage by stage below.
-        const unsigned int *rows_ready = w.rows_ready;
+        const unsigned int *rows_ready = pair ? nullptr : w.rows_ready;   // (P and D are complete before the launch)
         const unsigned long long timeout_ns = (unsigned long long)(w.wait_timeout_ms ? w.wait_timeout_ms : 2000u) * 1000000ULL;
         unsigned int rows_seen = rows_ready ? 0u : 0xffffffffu;
         if (rows_ready && w.ready_counts_channels) {
@@ -717,7 +866,7 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
           wait_rows_uploaded(rows_ready, (unsigned int)min(last, w.n_chan), rows_seen, w.abort_flag, timeout_ns, lane);
           rows_seen = 0xffffffffu;
         }
-        if (w.use_tma) {
+        if (w.use_tma || pair) {
           // One box per lane: lane b < i_boxes + j_boxes issues box b of every stage.  Everything that does not
           // change from stage to stage is worked out here, so that a stage costs this warp a few dozen
           // instructions: items that spend only a few hundred cycles on a stage (slab tiles of edge 32) would
@@ -727,12 +876,16 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
           const bool my_box = lane < nb;
           const int my_chan = lane < i_boxes ? row0 + lane * TN : col0 + (lane - i_boxes) * TN;
           const uint32_t my_dst = smem_u32(stages) + D_BYTES + (uint32_t)(lane < i_boxes ? lane : j_panel0 + (lane - i_boxes)) * box;
-          int c0 = w.tr ? my_chan : 0, c1 = w.tr ? 0 : my_chan;
-          const int s0 = w.tr ? 0 : KT, s1 = w.tr ? KT : 0;
+          const bool trl = w.tr && !pair;
+          int c0 = trl ? my_chan : 0, c1 = trl ? 0 : my_chan;
+          const int s0 = trl ? 0 : KT, s1 = trl ? KT : 0;
+          if (pair) map = lane < i_boxes ? &w.map_P : &w.map_D;
           const uint64_t policy = w.l2_keep ? keep_policy : normal_policy;
           const int n_poles = w.n_poles;
           unsigned int *const abort_flag = w.abort_flag;
+          const int draw_at = max(0, n_kt - DRAW_AHEAD);
           for (int kt = 0; kt < n_kt; ++kt) {
+            if (kt == draw_at && counter != nullptr && lane == 0) next_drawn = atomicAdd(counter, 1ULL);
             if (rows_ready != nullptr)
               wait_rows_uploaded(rows_ready, (unsigned int)min(kt * KT + KT, n_poles), rows_seen, abort_flag, timeout_ns, lane);
             mbar_wait(ps.empty(), ps.phase ^ 1u);
@@ -744,6 +897,7 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
             ps.advance();
           }
         } else {
+          if (counter != nullptr && lane == 0) next_drawn = atomicAdd(counter, 1ULL);
           for (int kt = 0; kt < n_kt; ++kt) {
             const int k0 = kt * KT;
             wait_rows_uploaded(rows_ready, (unsigned int)min(k0 + KT, w.n_poles), rows_seen, w.abort_flag, timeout_ns, lane);
@@ -790,6 +944,21 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
         iq ^= 1u;
         if (iq == 0) iphase ^= 1u;
         if (it.kind < 0) break;
+        if (it.kind == 2) {
+          // pair item: D comes from scratch, there is nothing to scale -- this warp only signs its stages off
+          int turn = sw;
+          for (int kt = 0; kt < it.n_kt; ++kt) {
+            if (turn == 0) {
+              mbar_wait(ps.empty(), ps.phase ^ 1u);
+              __syncwarp();
+              if (lane == 0) mbar_arrive(ps.full());
+              turn = DW;
+            }
+            --turn;
+            ps.advance();
+          }
+          continue;
+        }
         const int nv = it.n_valid_e;
         double en[EB], dv[EB];
 #pragma unroll
@@ -856,6 +1025,36 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
       if (iq == 0) iphase ^= 1u;
     }
   }
+}
+
+// ---- pair form: scratch builder ---------------------------------------------------------------
+// P[(n,m)][k] = w_nk * w_mk for the pairs n <= m (no energy in it: once per wave; rows in the order of
+// pair_row_channels, which is also recorded in pair_nm) and D[e][k] = 1/(E_k - E_e) (no channel in it), both
+// [rows][pair_ld] with k contiguous, which is how the GEMM items' TMA boxes want them.
+// Grid (blocks, waves); block b takes rows b, b + gridDim.x, ... of the wave's n_E + n_pairs rows.
+template <bool BATCH>
+__global__ void __launch_bounds__(256)
+pair_build_kernel(const __grid_constant__ DevWave single, const DevWave *__restrict__ waves, int n_waves) {
+ for (int p = blockIdx.y; p < n_waves; p += gridDim.y) {
+  const DevWave &w = BATCH ? waves[p] : single;
+  if (w.n_pairs <= 0) continue;
+  const int K = w.n_poles, C = w.n_chan, N = w.n_E;
+  const long long sn = w.tr ? 1 : w.ldw, sk = w.tr ? w.ldw : 1;       // element (n, k) of W at W[n * sn + k * sk]
+  for (int row = blockIdx.x; row < N + w.n_pairs; row += gridDim.x) {
+    if (row < N) {
+      const double E = __ldg(w.energies + row);
+      double *d = w.pair_D + (size_t)row * w.pair_ld;
+      for (int k = threadIdx.x; k < K; k += blockDim.x) d[k] = 1.0 / (__ldg(w.E_k + k) - E);
+    } else {
+      int n, m;
+      pair_row_channels(row - N, C, n, m);                       // (every thread: O(n_chan) integer steps)
+      if (threadIdx.x == 0) const_cast<unsigned int *>(w.pair_nm)[row - N] = (unsigned int)n | ((unsigned int)m << 16);
+      const double *wn = w.W + (size_t)n * sn, *wm = w.W + (size_t)m * sn;
+      double *pp = w.pair_P + (size_t)(row - N) * w.pair_ld;
+      for (int k = threadIdx.x; k < K; k += blockDim.x) pp[k] = __dmul_rn(wn[(size_t)k * sk], wm[(size_t)k * sk]);
+    }
+  }
+ }
 }
 
 // ---- verification kernel: eq. 4 term by term, one thread per R element ----------------------

@@ -269,6 +269,110 @@ def test_diag_add(rmat, oracle, slab_policy, C, K, N):
     assert np.array_equal(Rh.numpy(), R)
 
 
+# ---- few channels: eq. 4 as the GEMM over channel pairs ---------------------------------------------------------
+@pytest.fixture
+def pair_policy(rmat):
+    def set_policy(policy):
+        rmat.pstgf_debug_set_pair_policy(policy)
+    yield set_policy
+    rmat.pstgf_debug_set_pair_policy(rmat.PSTGF_PAIRS_AUTO)
+
+
+PAIR_SHAPES = [(1, 3, 1), (2, 9, 5), (7, 40, 64), (8, 160, 130), (9, 19, 300), (15, 61, 128), (16, 33, 129), (17, 100, 70),
+               (24, 480, 200), (31, 45, 65), (33, 77, 256), (64, 80, 257), (65, 61, 90), (90, 41, 140), (96, 100, 31)]
+
+
+@pytest.mark.parametrize("C,K,N", PAIR_SHAPES)
+def test_pair_form_edge_shapes(rmat, oracle, pair_policy, tail_policy, C, K, N):
+    """Waves with n_chan <= 96 forced through the pair form (PSTGF_PAIRS_ALWAYS, so that shapes with few energies
+    are covered too): partial pair tiles of every register-tile height, partial energy tiles, poles not a multiple
+    of 20, both memory orders of W, coarse and fine pair tiles, the diagonal addend, single, batch and host call --
+    <= 1e-13 against the oracle, bitwise equal to one another, and within 1e-14 of the symmetric form."""
+    from paper_1909_07321_b200 import inputs
+    w = inputs.make_wave(11000 + 31 * C + N, C, K, N)
+    rng = np.random.default_rng(C + N)
+    da = rng.normal(0.0, 0.05, (N, C))
+    R_ref = oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads())
+    R_ref_da = oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads(), diag_add=da)
+    pair_policy(rmat.PSTGF_PAIRS_NONE)
+    R_syrk = _form(rmat, w)
+    pair_policy(rmat.PSTGF_PAIRS_ALWAYS)
+    Wd, Wt, Ek, en, dad = _dev(w.W), _dev(w.W.T), _dev(w.E_k), _dev(w.energies), _dev(da)
+    results = []
+    for policy in (rmat.PSTGF_TAIL_NONE, rmat.PSTGF_TAIL_ALL, rmat.PSTGF_TAIL_AUTO):
+        tail_policy(policy)
+        R = _form(rmat, w)
+        _check(R, R_ref)
+        assert _rel_err_per_energy(R, R_syrk).max() <= 1e-14
+        results.append(R)
+        Rh = rmat.pstgf_rmat_form_hdat(Wt, Ek, en, w.a)
+        torch.cuda.synchronize()
+        assert np.array_equal(Rh.cpu().numpy(), R)
+        # batch call: this wave (with the addend) beside a wave that stays in the symmetric form
+        big = inputs.make_wave(77, 130, 60, 9)
+        Rb = torch.full((N, C, C), float("nan"), dtype=torch.float64, device="cuda")
+        Rbig = torch.empty((big.n_E, 130, 130), dtype=torch.float64, device="cuda")
+        both = [(_dev(big.W), _dev(big.E_k), _dev(big.energies), big.a, Rbig),      # (kept alive: the array holds raw pointers)
+                (Wd, Ek, en, w.a, Rb, rmat.PSTGF_W_POLE_CONTIGUOUS, dad)]
+        arr = rmat.make_wave_array(both)
+        ws = torch.empty(rmat.pstgf_rmat_batch_workspace_bytes(arr), dtype=torch.uint8, device="cuda")
+        rmat.pstgf_rmat_form_batch(arr, ws)
+        torch.cuda.synchronize()
+        Rb = Rb.cpu().numpy()
+        _check(Rb, R_ref_da)
+        idx = np.arange(C)
+        off = ~np.eye(C, dtype=bool)
+        assert np.array_equal(Rb[:, off], R[:, off]) and np.array_equal(Rb[:, idx, idx], R[:, idx, idx] + da)
+        _check(Rbig.cpu().numpy(), oracle.rmat_form(big.W, big.E_k, big.energies, big.a, threads=_threads()))
+    assert np.array_equal(results[0], results[1]) and np.array_equal(results[0], results[2])
+    tail_policy(rmat.PSTGF_TAIL_AUTO)
+    Rh = torch.full((N, C, C), float("nan"), dtype=torch.float64).pin_memory()
+    rmat.pstgf_rmat_form_batch_host([(torch.from_numpy(w.W).pin_memory(), torch.from_numpy(w.E_k).pin_memory(),
+                                      torch.from_numpy(w.energies).pin_memory(), w.a, Rh)], max_chunk_bytes=C * C * 8 * 24)
+    assert np.array_equal(Rh.numpy(), results[0])
+
+
+def test_pair_form_is_chosen_by_shape_alone(rmat, oracle):
+    """Default policy: a wave takes the pair form iff n_chan <= 96 and n_E >= 64, whatever else is in the batch, so
+    single, batch and host calls agree bitwise; the host call cuts the wave into energy ranges of fewer than 64
+    energies here and must still send every range the way of the whole wave."""
+    from paper_1909_07321_b200 import inputs
+    waves = [inputs.make_wave(12001, 48, 960, 200), inputs.make_wave(12002, 200, 80, 70), inputs.make_wave(12003, 96, 50, 64),
+             inputs.make_wave(12004, 97, 50, 64), inputs.make_wave(12005, 20, 400, 63)]
+    singles = [_form(rmat, w) for w in waves]
+    for w, R in zip(waves, singles):
+        _check(R, oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads()))
+    for got, R in zip(_form_batch(rmat, waves), singles):
+        assert np.array_equal(got.cpu().numpy(), R)
+    host = []
+    for w in waves:
+        host.append((torch.from_numpy(w.W).pin_memory(), torch.from_numpy(w.E_k).pin_memory(),
+                     torch.from_numpy(w.energies).pin_memory(), w.a,
+                     torch.full((w.n_E, w.n_chan, w.n_chan), np.nan, dtype=torch.float64).pin_memory()))
+    rmat.pstgf_rmat_form_batch_host(host, max_chunk_bytes=48 * 48 * 8 * 40)
+    for h, R in zip(host, singles):
+        assert np.array_equal(h[4].numpy(), R)
+    # the two forms differ by rounding only
+    rmat.pstgf_debug_set_pair_policy(rmat.PSTGF_PAIRS_NONE)
+    try:
+        for w, R in zip(waves, singles):
+            assert _rel_err_per_energy(_form(rmat, w), R).max() <= 1e-14
+    finally:
+        rmat.pstgf_debug_set_pair_policy(rmat.PSTGF_PAIRS_AUTO)
+
+
+def test_config7_small_waves_sampled(rmat, oracle):
+    """256 small waves (n_chan 8..32) in one batch call, the launch configuration bench.py --config 7 times: every
+    wave checked on sampled energies against the oracle, four waves at every energy."""
+    from paper_1909_07321_b200 import inputs
+    wl = inputs.make_config(7)
+    Rs = _form_batch(rmat, wl.waves)
+    for p, (w, R) in enumerate(zip(wl.waves, Rs)):
+        idx = inputs.sample_energy_indices(w, n_random=2, seed=700 + p) if p % 64 else np.arange(w.n_E)
+        R_ref = oracle.rmat_form(w.W, w.E_k, w.energies[idx], w.a, threads=_threads())
+        _check(R[torch.from_numpy(idx).cuda()].cpu().numpy(), R_ref)
+
+
 # ---- boundary hygiene ------------------------------------------------------------------------------------------
 def test_workspace_reused_with_other_waves(rmat, oracle):
     """The batch call keeps its TMA descriptors in the caller's workspace, which the next call rewrites: a second
@@ -279,7 +383,7 @@ def test_workspace_reused_with_other_waves(rmat, oracle):
             [inputs.make_wave(603, 90, 500, 11), inputs.make_wave(604, 200, 100, 9)],
             [inputs.make_wave(605, 33, 1000, 40), inputs.make_wave(606, 130, 260, 3)]]
     layouts = [[0, 1], [1, 0], [1, 1]]
-    ws = torch.empty(rmat.pstgf_rmat_batch_workspace_bytes(None, 2), dtype=torch.uint8, device="cuda")
+    ws = torch.empty(16 << 20, dtype=torch.uint8, device="cuda")   # more than any of the calls below asks for
     keep, outs = [], []
     for rep in range(3):
         for waves, lays in zip(sets, layouts):
@@ -289,6 +393,7 @@ def test_workspace_reused_with_other_waves(rmat, oracle):
                 R = torch.full((w.n_E, w.n_chan, w.n_chan), float("nan"), dtype=torch.float64, device="cuda")
                 dev.append((_dev(Wh), _dev(w.E_k), _dev(w.energies), w.a, R, lay))
             arr = rmat.make_wave_array(dev)
+            assert rmat.pstgf_rmat_batch_workspace_bytes(arr) <= ws.numel()
             rmat.pstgf_rmat_form_batch(arr, ws)                # no synchronisation between the calls
             keep.append(dev)
             outs.append((waves, [d[4] for d in dev]))
