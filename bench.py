@@ -63,6 +63,9 @@ def parse_args():
                          "(default), left to a partly idle block of 8 (round-1 behaviour), or a forced edge; same bits")
     ap.add_argument("--e2e-chunk-mib", type=int, default=0,
                     help="max_chunk_bytes of pstgf_rmat_form_batch_host in MiB (0 = the library's default)")
+    ap.add_argument("--scaling", choices=["weak", "strong"], default="weak",
+                    help="N > 1 ranks: weak = the configuration with an N times finer mesh (per-rank work fixed, default); "
+                         "strong = the configuration as it is, its energy blocks split over the ranks (total work fixed)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
@@ -140,6 +143,16 @@ class ClockSampler:
 
 
 # ---- workload --------------------------------------------------------------------------------
+def job_workload(args, world: int):
+    """The workload of the whole job (all ranks): the configuration as it is at N = 1 and under --scaling strong,
+    the configuration with an N times finer mesh under --scaling weak (per-rank work fixed)."""
+    from paper_1909_07321_b200 import inputs
+    if world == 1 or args.scaling == "strong":
+        return inputs.make_config(args.config, n_E=args.n_E or None)
+    base = inputs.config_shapes(args.config)
+    return inputs.make_config(args.config, n_E=world * (args.n_E or base[0][2]))
+
+
 def workload_description(cfg: int, wl) -> dict:
     names = {1: "configs[0] single wave 8x160, n_E 1000", 2: "configs[1] single wave 64x1280, n_E 4096",
              3: "configs[2] 8 waves 256x5120, n_E 2048 shared", 4: "configs[3] ragged 32 waves n_chan U[16,400], n_E 512",
@@ -195,20 +208,32 @@ def cpu_baseline_entries(wl, target_seconds: float, cores: int) -> dict:
             "counted_gflops": S * w.n_poles / dt / 1e9}
 
 
+def sample_energies_per_wave(wl, seconds: float, cores: int) -> int:
+    """Energies per wave for about `seconds` of wall time with `cores` threads over the energies of a wave: a whole
+    multiple of the core count (rounded UP, so that no core idles and the oracle is timed at full occupancy), capped
+    by the shortest mesh."""
+    per_e = est_oracle_seconds_per_energy(wl)                   # one thread, one energy of an average wave
+    k = max(1, round(seconds * cores / (per_e * len(wl.waves))))
+    k = -(-k // cores) * cores
+    return int(min(k, min(w.n_E for w in wl.waves)))
+
+
 def cpu_baseline(wl, target_seconds: float) -> dict:
     cores = oracle_cores()
-    per_e = est_oracle_seconds_per_energy(wl)                   # one thread, one energy of an average wave
+    per_e = est_oracle_seconds_per_energy(wl)
     if len(wl.waves) == 1 and per_e > 4 * target_seconds * cores:
         return cpu_baseline_entries(wl, target_seconds, cores)
-    # energies per wave so that the wall time is ~target_seconds with `cores` threads over energies
-    k = int(max(1, min(min(w.n_E for w in wl.waves), round(target_seconds * cores / (per_e * len(wl.waves))))))
-    if k >= cores:
-        k -= k % cores
+    k = sample_energies_per_wave(wl, target_seconds, cores)
     n, dt = oracle_sample_run(wl, k, cores)
+    # the same loop on ONE thread (BASELINE.md section 4), on a sample of about a fifth of the CPU time
+    k1 = int(max(1, min(min(w.n_E for w in wl.waves), round(0.2 * target_seconds / (per_e * len(wl.waves))))))
+    n1, dt1 = oracle_sample_run(wl, k1, 1)
     return {"value": n / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"first {k} energies of each of {len(wl.waves)} wave(s), {n} energies, {dt:.2f} s wall, "
                       f"OpenMP over energies; every energy of a wave costs the same, so energies/s extrapolates",
-            "counted_gflops": n and sum(min(k, w.n_E) * w.n_chan ** 2 * w.n_poles for w in wl.waves) / dt / 1e9}
+            "counted_gflops": n and sum(min(k, w.n_E) * w.n_chan ** 2 * w.n_poles for w in wl.waves) / dt / 1e9,
+            "one_thread": {"value": n1 / dt1, "unit": UNIT, "cores": 1,
+                           "sample": f"first {k1} energies of each wave, {n1} energies, {dt1:.2f} s wall"}}
 
 
 def run_reference(args):
@@ -216,8 +241,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    from paper_1909_07321_b200 import inputs
-    wl = inputs.make_config(args.config, n_E=args.n_E or None)
+    wl = job_workload(args, int(os.environ.get("WORLD_SIZE", "1")))
     cores = oracle_cores()
     per_e = est_oracle_seconds_per_energy(wl)
     budget = 120.0 / max(1, args.steps + args.warmup)            # whole run within a few minutes
@@ -227,16 +251,14 @@ def run_reference(args):
         runs = [cpu_baseline_entries(wl, min(budget, 20.0), cores) for _ in range(args.steps)]
         value = len(runs) / sum(1.0 / r["value"] for r in runs)
         line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 0, "steps": args.steps,
-                "warmup": args.warmup, "ms_per_step": None, "higher_is_better": True, "scaling": "weak",
+                "warmup": args.warmup, "ms_per_step": None, "higher_is_better": True, "scaling": args.scaling,
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_description(args.config, wl),
                 "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
                                  "sample": "each step: " + runs[0]["sample"]},
                 "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
         print(json.dumps(line), flush=True)
         return 0
-    k = int(max(1, min(min(w.n_E for w in wl.waves), round(min(budget, 20.0) * cores / (per_e * len(wl.waves))))))
-    if k >= cores:
-        k -= k % cores
+    k = sample_energies_per_wave(wl, min(budget, 20.0), cores)
     for _ in range(args.warmup):
         oracle_sample_run(wl, k, cores)
     total_n, total_t = 0, 0.0
@@ -248,7 +270,7 @@ def run_reference(args):
     sample = f"each step: first {k} energies of each of {len(wl.waves)} wave(s) ({total_n // max(1, args.steps)} energies)"
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 0, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * total_t / max(1, args.steps), "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "scaling": args.scaling, "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": workload_description(args.config, wl),
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -374,14 +396,14 @@ def run_cuda(args):
     # Weak scaling over ranks: at N ranks the job is the configuration with an N times
     # finer energy mesh; shard.plan gives each rank its wave-rotated share of the energy blocks (PAPER.md:116,
     # :135-137, Fig. 1), i.e. the configuration's own n_E per wave and rank.  No data-path collective.
+    # --scaling strong splits the configuration's own energy blocks over the ranks instead (total work fixed).
+    wl_job = job_workload(args, world)
+    n_e_job = wl_job.n_energies()
+    job_description = workload_description(args.config, wl_job)
     if world == 1:
-        wl = inputs.make_config(args.config, n_E=args.n_E or None)
-        n_e_job = wl.n_energies()
+        wl = wl_job
     else:
         from paper_1909_07321_b200 import shard
-        base = inputs.config_shapes(args.config)
-        wl_job = inputs.make_config(args.config, n_E=world * (args.n_E or base[0][2]))
-        n_e_job = wl_job.n_energies()
         wl = inputs.Workload(name=wl_job.name, seed=wl_job.seed)
         for p, idx in shard.plan([w.n_E for w in wl_job.waves], rank, world):
             w = wl_job.waves[p]
@@ -510,7 +532,9 @@ def run_cuda(args):
                 "hbm_peak_gbs": peaks["hbm_gbs"]}
     if probe:
         roofline["fp64_probe_tflops"] = probe
-    roofline["traffic"] = ncu_traffic(args.config)
+    roofline["traffic"] = ncu_traffic(args.config) if not args.n_E else None
+    roofline["traffic_source"] = ("committed ncu --set full capture (profiles/traffic.csv): DRAM bytes read + written "
+                                  "per launch; not measured in this run") if roofline["traffic"] is not None else None
 
     # ---- end to end: HOST buffers through the C ABI, copies inside the timed region ----
     e2e = None
@@ -561,12 +585,13 @@ def run_cuda(args):
     vs_baseline = value / PAPER_ENERGIES_PER_S if (args.config == 6 and world == 1) else None
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+                "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": args.scaling,
                 "vs_baseline": vs_baseline, "dtype": "f64", "data": "synthetic",
-                "config": dict(workload_description(args.config, wl), n_energies_per_step=n_e_job, n_energies_per_rank=n_e,
-                               l2="flushed between timed steps (512 MiB write)", w_layout=args.w_layout, tail_policy=args.tail_policy,
-                               sha256=wl.sha256()[:16]),
-                "tflops_counted": world * flop * args.steps / (total_ms_max * 1e-3) / 1e12,   # ranks carry equal shares
+                "config": job_description,           # the same dict as --impl reference prints
+                "run": {"n_energies_per_rank": n_e, "l2": "flushed between timed steps (512 MiB write)",
+                        "w_layout": args.w_layout, "tail_policy": args.tail_policy, "slab_policy": args.slab_policy,
+                        "sha256": wl_job.sha256()[:16]},
+                "tflops_counted": wl_job.counted_flop() * args.steps / (total_ms_max * 1e-3) / 1e12,
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,
                 **({"prior_art": prior} if prior else {}),
                 "clocks": clocks, "wall_s_timed_region": wall, "step_ms_min_max": [min(step_ms), max(step_ms)]}

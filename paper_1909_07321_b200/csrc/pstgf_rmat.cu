@@ -18,7 +18,8 @@
 #include <chrono>
 
 #include "../../include/pstgf_rmat.h"
-#include "rmat_kernel.cuh"
+#include "rmat_aux.cuh"
+#include "rmat_launch.h"
 
 namespace {
 
@@ -81,10 +82,7 @@ pstgf_status_t device_state(DeviceState &ds) {
   {
     std::lock_guard<std::mutex> lock(g_attr_mutex);
     if (dev < 64 && !g_attr_set[dev]) {
-      PSTGF_CUDA(cudaFuncSetAttribute(pstgf::rmat_persistent_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      pstgf::SMEM_MAX_OPTIN));
-      PSTGF_CUDA(cudaFuncSetAttribute(pstgf::rmat_persistent_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      pstgf::SMEM_MAX_OPTIN));
+      PSTGF_CUDA(pstgf::persistent_prepare_all());
       g_attr_set[dev] = true;
     }
   }
@@ -377,6 +375,16 @@ void plan_slabs(std::vector<DevWave> &ds, int grid) {
     d.slab_g2 = T == 128 ? 0 : r / 2;       // tiles of edge 128 take one energy at a time (8 warps x 16 x 2 blocks)
     d.slab_g1 = T == 128 ? r : r % 2;
   }
+}
+
+// Item families of a launch (rmat_common.h): the kernel instantiation that holds no more code than the items need.
+int launch_family(const std::vector<DevWave> &ds) {
+  int fam = pstgf::FAM_CLASSIC;
+  for (const DevWave &d : ds) {
+    if (d.n_pairs > 0) return pstgf::FAM_PAIR;
+    if (slab_items(d) > 0) fam = pstgf::FAM_SLAB;
+  }
+  return fam;
 }
 
 // Ring geometry of a launch: a stage holds the most panels any of its items needs (5 for classic items, 8 / 4 / 2
@@ -753,9 +761,8 @@ static pstgf_status_t form_single(const pstgf_wave_t &w, void *stream) {
     unsigned long long *counter = nullptr;
     // no more items than CTAs: item b goes to CTA b, no counter needed (one L2 round trip less for the tiny calls)
     const int slot = n_items <= grid ? -1 : acquire_counter(ds.device, s, &counter);
-    pstgf::rmat_persistent_kernel<false><<<grid, pstgf::NUM_THREADS, pstgf::smem_bytes_for(geo), s>>>(
-        d[0], nullptr, nullptr, 1, n_items, counter, geo);
-    const cudaError_t le = cudaGetLastError();
+    pstgf::PersistentArgs pa{&d[0], nullptr, nullptr, 1, n_items, counter, geo, grid};
+    const cudaError_t le = pstgf::persistent_launch_family(launch_family(d), false, pa, s);
     if (scratch) cudaFreeAsync(scratch, s);
     PSTGF_CUDA(le);
     if (slot >= 0) {
@@ -790,7 +797,8 @@ struct BatchCompletion {
   unsigned int *const *flag = nullptr;   // in: per input wave, a zeroed host-mapped word (device-visible address)
   const unsigned int *const *rows_ready = nullptr;   // in, optional: per input wave, the upload counter of its W
   const int *ready_counts_channels = nullptr;        // ... and what it counts (DevWave::ready_counts_channels)
-  unsigned int *abort_flag = nullptr;                // in: host-mapped word a load warp sets when an upload wait times out
+  unsigned int *abort_flag = nullptr;                // in: zeroed DEVICE word the load warps poll and set when an upload wait times out
+  unsigned int *abort_flag_host = nullptr;           // in: host-mapped word the warp that timed out sets as well
   const unsigned char *force_pair = nullptr;         // in, optional: per input wave, 1 = pair form, 0 = SYRK form
   std::vector<int> order;                // out: input wave indices in the order the launch completes them
   std::vector<long long> items;          // out: items of each input wave (arrivals = items * EB)
@@ -865,6 +873,7 @@ static pstgf_status_t form_batch_impl(const pstgf_wave_t *waves, int n_waves, vo
         ds[q].rows_ready = completion->rows_ready[order[q]];
         ds[q].ready_counts_channels = completion->ready_counts_channels[order[q]];
         ds[q].abort_flag = completion->abort_flag;
+        ds[q].abort_flag_host = completion->abort_flag_host;
         ds[q].wait_timeout_ms = tl_upload_timeout_ms;
       }
     }
@@ -910,12 +919,9 @@ static pstgf_status_t form_batch_impl(const pstgf_wave_t *waves, int n_waves, vo
   }
   const int grid = (int)std::min<long long>(dstate.sm_count, total);
   const pstgf::RingGeo geo = ring_geometry(ds);
-  DevWave dummy;
-  std::memset(&dummy, 0, sizeof(dummy));
-  pstgf::rmat_persistent_kernel<true><<<grid, pstgf::NUM_THREADS, pstgf::smem_bytes_for(geo), s>>>(
-      dummy, reinterpret_cast<const DevWave *>(ws + off_waves), reinterpret_cast<const long long *>(ws + off_begin), nw,
-      total, reinterpret_cast<unsigned long long *>(ws), geo);
-  PSTGF_CUDA(cudaGetLastError());
+  pstgf::PersistentArgs pa{nullptr, reinterpret_cast<const DevWave *>(ws + off_waves), reinterpret_cast<const long long *>(ws + off_begin), nw,
+                           total, reinterpret_cast<unsigned long long *>(ws), geo, grid};
+  PSTGF_CUDA(pstgf::persistent_launch_family(launch_family(ds), true, pa, s));
   tl_launches = launches + 1;
   return PSTGF_OK;
 }
@@ -1097,7 +1103,10 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
   if (signalled) PSTGF_CUDA(host_call_flags(ds.device, &flags));
   const bool overlap_upload = signalled && (size_t)n_waves <= MAX_UPLOAD_WAVES;
   volatile unsigned int *abort_host = signalled ? flags.flags_host + 2 * MAX_CHUNK_SEGMENTS : nullptr;
-  if (signalled) *abort_host = 0u;
+  if (signalled) {
+    *abort_host = 0u;
+    PSTGF_CUDA(cudaMemsetAsync(flags.counters + 2 * MAX_CHUNK_SEGMENTS, 0, sizeof(unsigned int), res.s));   // the device's copy
+  }
   if (overlap_upload) PSTGF_CUDA(cudaMemsetAsync(flags.upload_counters, 0, sizeof(unsigned int) * (size_t)n_waves, res.s));
   std::vector<pstgf_wave_t> dev(waves, waves + n_waves);
   // poles [k0, k1) of all channels, or (by_channels, pole-contiguous W only) channels [k0, k1) with all their poles
@@ -1323,7 +1332,8 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
       completion.flag = flag.data();
       completion.rows_ready = rows_ready.data();
       completion.ready_counts_channels = ready_kind.data();
-      completion.abort_flag = flags.flags_dev + 2 * MAX_CHUNK_SEGMENTS;
+      completion.abort_flag = flags.counters + 2 * MAX_CHUNK_SEGMENTS;
+      completion.abort_flag_host = flags.flags_dev + 2 * MAX_CHUNK_SEGMENTS;
       completion.force_pair = force.data();
       st = form_batch_impl(sub.data(), (int)sub.size(), wsbuf[b], wsb, cs, &completion);
       if (st != PSTGF_OK) return st;

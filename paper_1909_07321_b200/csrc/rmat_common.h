@@ -86,6 +86,9 @@ constexpr int PAIR_MAX_CHAN = 96;        // 4656 pairs; P is 71 MB at n_poles = 
 constexpr int PAIR_MIN_E = 64;           // fewer energies than this do not fill an energy tile's eight warps
 constexpr int PT_M = 128, PT_MF = 64, PT_N = 128;
 constexpr int PAIR_PANELS = (PT_M + PT_N) / TN;             // 8
+// Item families a launch can hold; the persistent kernel is compiled once per value (a template parameter), so that a
+// launch of classic items only does not carry the code of the others.
+constexpr int FAM_CLASSIC = 0, FAM_SLAB = 1, FAM_PAIR = 2;
 
 // Shared memory of a CTA: [mbarriers | two ItemInfo slots | ring of n_stages stages]; the ring geometry is a launch
 // parameter (RingGeo) because slab tiles of edge 128 need 8 panels per stage instead of 5.
@@ -127,7 +130,8 @@ struct alignas(128) DevWave {
   unsigned int *done;      // optional completion counter of this wave (host-buffer call): += 1 per consumer warp and item
   unsigned int *done_flag; // ... and the (host-mapped) word that is set to 1 by the arrival that makes it done_target
   const unsigned int *rows_ready;   // optional (host-buffer call): how much of W has been uploaded so far, see the load warp
-  unsigned int *abort_flag;         // host-buffer call: set to 1 by a load warp whose wait for an upload timed out
+  unsigned int *abort_flag;         // host-buffer call: DEVICE word set to 1 by a load warp whose wait for an upload timed out
+  unsigned int *abort_flag_host;    // ... and the host-mapped word that warp sets as well (written once, never polled by the device)
   long long ldw;
   double inv2a;            // 1/(2a), PAPER.md:108 prefactor
   int n_chan, n_poles, n_E;

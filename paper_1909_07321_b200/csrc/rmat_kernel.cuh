@@ -119,7 +119,8 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
 // warp raises the launch's abort flag and stops waiting; every other load warp sees the flag at its next wait, the
 // launch drains, and the host turns the flag into PSTGF_ERR_TIMEOUT (the R of that call is then undefined).
 __device__ __forceinline__ void wait_rows_uploaded(const unsigned int *rows_ready, unsigned int need, unsigned int &seen,
-                                                   unsigned int *abort_flag, unsigned long long timeout_ns, int lane) {
+                                                   unsigned int *abort_flag, unsigned int *abort_flag_host,
+                                                   unsigned long long timeout_ns, int lane) {
   if (seen >= need) return;
   if (lane == 0) {
     unsigned int v;
@@ -128,10 +129,17 @@ __device__ __forceinline__ void wait_rows_uploaded(const unsigned int *rows_read
       asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(rows_ready) : "memory");
       if (v >= need) break;
       if (abort_flag != nullptr) {
+        // the flag that is polled lives in DEVICE memory: 148 load warps polling a word of mapped host memory
+        // fill the PCIe link with small reads and slow the very upload they are waiting for (measured: config 4's
+        // host call 149 -> 265 ms); the host's copy is written once, by the warp whose wait timed out
         unsigned int ab;
-        asm volatile("ld.relaxed.sys.global.u32 %0, [%1];" : "=r"(ab) : "l"(abort_flag) : "memory");
+        asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(ab) : "l"(abort_flag) : "memory");
         if (ab == 0u && global_timer_ns() - t0 > timeout_ns) {
-          atomicExch_system(abort_flag, 1u);
+          atomicExch(abort_flag, 1u);
+          if (abort_flag_host != nullptr) {
+            *reinterpret_cast<volatile unsigned int *>(abort_flag_host) = 1u;
+            __threadfence_system();
+          }
           ab = 1u;
         }
         if (ab != 0u) {
@@ -510,9 +518,10 @@ __device__ __forceinline__ void consume_pair(const ItemInfo &it, Pipe &ps, int w
 
 // The tile shapes are compile-time variants (no predicates inside the DMMA loop); ragged edges of
 // a wave pick the variant with fewer 8-wide blocks.
-template <bool TR>
+template <int FAM, bool TR>
 __device__ __forceinline__ void consume_item_layout(const ItemInfo &it, Pipe &ps, int warp, int lane) {
-  if (it.slab_T != 0) {
+  if constexpr (FAM >= FAM_SLAB) {
+   if (it.slab_T != 0) {
     const SlabShape sh = slab_shape(it.slab_T, it.slab_g);
     switch (sh.nr) {
       case 16: consume_slab<16, 2, 1, TR>(it, ps, warp, lane, sh.wc); break;
@@ -524,6 +533,7 @@ __device__ __forceinline__ void consume_item_layout(const ItemInfo &it, Pipe &ps
         break;
     }
     return;
+  }
   }
   if (warp >= it.n_valid_e) {
     consume_idle(it.n_kt, ps, lane);
@@ -560,15 +570,21 @@ __device__ __forceinline__ void consume_item_layout(const ItemInfo &it, Pipe &ps
   }
 }
 
+// FAM: the item families the launch can hold (rmat_common.h): a launch without pair items (without slab items)
+// runs a kernel that does not contain their code -- the mere presence of the pair consumer in the kernel cost the
+// classic items 1.4 % (config 5: 20.14 -> 20.42 ms, with identical SASS in the classic loops).
+template <int FAM>
 __device__ __forceinline__ void consume_item(const ItemInfo &it, Pipe &ps, int warp, int lane) {
-  if (it.kind == 2) {
-    if (it.nblk == 16) consume_pair<16>(it, ps, warp, lane);
-    else if (it.nblk == 8) consume_pair<8>(it, ps, warp, lane);
-    else consume_pair<4>(it, ps, warp, lane);
-    return;
+  if constexpr (FAM >= FAM_PAIR) {
+    if (it.kind == 2) {
+      if (it.nblk == 16) consume_pair<16>(it, ps, warp, lane);
+      else if (it.nblk == 8) consume_pair<8>(it, ps, warp, lane);
+      else consume_pair<4>(it, ps, warp, lane);
+      return;
+    }
   }
-  if (it.tr) consume_item_layout<true>(it, ps, warp, lane);
-  else consume_item_layout<false>(it, ps, warp, lane);
+  if (it.tr) consume_item_layout<FAM, true>(it, ps, warp, lane);
+  else consume_item_layout<FAM, false>(it, ps, warp, lane);
 }
 
 // ---- producer ----------------------------------------------------------------------------
@@ -667,7 +683,7 @@ __device__ __forceinline__ void stage_panel_plain_tr(double *dst, const DevWave 
   }
 }
 
-template <bool BATCH>
+template <bool BATCH, int FAM>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__restrict__ waves,
                        const long long *__restrict__ item_begin, int n_waves, long long n_items,
@@ -863,7 +879,7 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
         unsigned int rows_seen = rows_ready ? 0u : 0xffffffffu;
         if (rows_ready && w.ready_counts_channels) {
           const int last = max(row0 + i_boxes * TN, kind != 0 ? col0 + j_boxes * TN : 0);
-          wait_rows_uploaded(rows_ready, (unsigned int)min(last, w.n_chan), rows_seen, w.abort_flag, timeout_ns, lane);
+          wait_rows_uploaded(rows_ready, (unsigned int)min(last, w.n_chan), rows_seen, w.abort_flag, w.abort_flag_host, timeout_ns, lane);
           rows_seen = 0xffffffffu;
         }
         if (w.use_tma || pair) {
@@ -882,12 +898,12 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
           if (pair) map = lane < i_boxes ? &w.map_P : &w.map_D;
           const uint64_t policy = w.l2_keep ? keep_policy : normal_policy;
           const int n_poles = w.n_poles;
-          unsigned int *const abort_flag = w.abort_flag;
+          unsigned int *const abort_flag = w.abort_flag, *const abort_flag_host = w.abort_flag_host;
           const int draw_at = max(0, n_kt - DRAW_AHEAD);
           for (int kt = 0; kt < n_kt; ++kt) {
             if (kt == draw_at && counter != nullptr && lane == 0) next_drawn = atomicAdd(counter, 1ULL);
             if (rows_ready != nullptr)
-              wait_rows_uploaded(rows_ready, (unsigned int)min(kt * KT + KT, n_poles), rows_seen, abort_flag, timeout_ns, lane);
+              wait_rows_uploaded(rows_ready, (unsigned int)min(kt * KT + KT, n_poles), rows_seen, abort_flag, abort_flag_host, timeout_ns, lane);
             mbar_wait(ps.empty(), ps.phase ^ 1u);
             const uint32_t full = ps.full();
             if (lane == 0) mbar_arrive_expect_tx(full, tx_bytes);
@@ -900,7 +916,7 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
           if (counter != nullptr && lane == 0) next_drawn = atomicAdd(counter, 1ULL);
           for (int kt = 0; kt < n_kt; ++kt) {
             const int k0 = kt * KT;
-            wait_rows_uploaded(rows_ready, (unsigned int)min(k0 + KT, w.n_poles), rows_seen, w.abort_flag, timeout_ns, lane);
+            wait_rows_uploaded(rows_ready, (unsigned int)min(k0 + KT, w.n_poles), rows_seen, w.abort_flag, w.abort_flag_host, timeout_ns, lane);
             mbar_wait(ps.empty(), ps.phase ^ 1u);
             double *sd = reinterpret_cast<double *>(stages + (size_t)ps.stage * ps.stage_bytes) + D_DOUBLES;
             if (w.tr) {
@@ -1007,7 +1023,7 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
       mbar_wait(item_full0 + 8 * iq, iphase);
       const ItemInfo it = ring[iq];
       if (it.kind < 0) break;
-      consume_item(it, ps, warp, lane);
+      consume_item<FAM>(it, ps, warp, lane);
       if (it.done != nullptr) {
         // host-buffer call: the host copies a wave's R back as soon as its last item has been stored.  Every warp
         // makes its stores visible device-wide and counts itself in; the arrival that completes the wave raises
@@ -1025,61 +1041,6 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
       if (iq == 0) iphase ^= 1u;
     }
   }
-}
-
-// ---- pair form: scratch builder ---------------------------------------------------------------
-// P[(n,m)][k] = w_nk * w_mk for the pairs n <= m (no energy in it: once per wave; rows in the order of
-// pair_row_channels, which is also recorded in pair_nm) and D[e][k] = 1/(E_k - E_e) (no channel in it), both
-// [rows][pair_ld] with k contiguous, which is how the GEMM items' TMA boxes want them.
-// Grid (blocks, waves); block b takes rows b, b + gridDim.x, ... of the wave's n_E + n_pairs rows.
-template <bool BATCH>
-__global__ void __launch_bounds__(256)
-pair_build_kernel(const __grid_constant__ DevWave single, const DevWave *__restrict__ waves, int n_waves) {
- for (int p = blockIdx.y; p < n_waves; p += gridDim.y) {
-  const DevWave &w = BATCH ? waves[p] : single;
-  if (w.n_pairs <= 0) continue;
-  const int K = w.n_poles, C = w.n_chan, N = w.n_E;
-  const long long sn = w.tr ? 1 : w.ldw, sk = w.tr ? w.ldw : 1;       // element (n, k) of W at W[n * sn + k * sk]
-  for (int row = blockIdx.x; row < N + w.n_pairs; row += gridDim.x) {
-    if (row < N) {
-      const double E = __ldg(w.energies + row);
-      double *d = w.pair_D + (size_t)row * w.pair_ld;
-      for (int k = threadIdx.x; k < K; k += blockDim.x) d[k] = 1.0 / (__ldg(w.E_k + k) - E);
-    } else {
-      int n, m;
-      pair_row_channels(row - N, C, n, m);                       // (every thread: O(n_chan) integer steps)
-      if (threadIdx.x == 0) const_cast<unsigned int *>(w.pair_nm)[row - N] = (unsigned int)n | ((unsigned int)m << 16);
-      const double *wn = w.W + (size_t)n * sn, *wm = w.W + (size_t)m * sn;
-      double *pp = w.pair_P + (size_t)(row - N) * w.pair_ld;
-      for (int k = threadIdx.x; k < K; k += blockDim.x) pp[k] = __dmul_rn(wn[(size_t)k * sk], wm[(size_t)k * sk]);
-    }
-  }
- }
-}
-
-// ---- verification kernel: eq. 4 term by term, one thread per R element ----------------------
-__global__ void rmat_naive_kernel(const double *__restrict__ W, long long stride_n, long long stride_k,
-                                  const double *__restrict__ E_k, const double *__restrict__ energies, int n_chan,
-                                  int n_poles, long long n_elems, double a, const double *__restrict__ diag_add,
-                                  double *__restrict__ R_out) {
-  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= n_elems) return;
-  const long long cc = (long long)n_chan * n_chan;
-  const long long e = idx / cc;
-  const int rem = (int)(idx - e * cc);
-  const int n = rem / n_chan, m = rem - n * n_chan;
-  const double E = energies[e];
-  const double *wn = W + (size_t)n * stride_n, *wm = W + (size_t)m * stride_n;
-  double s = 0.0, c = 0.0;
-  for (int k = 0; k < n_poles; ++k) {
-    const double t = __ddiv_rn(__dmul_rn(wn[(size_t)k * stride_k], wm[(size_t)k * stride_k]), __dsub_rn(E_k[k], E));
-    const double u = __dadd_rn(s, t);
-    c = __dadd_rn(c, fabs(s) >= fabs(t) ? __dadd_rn(__dsub_rn(s, u), t) : __dadd_rn(__dsub_rn(t, u), s));
-    s = u;
-  }
-  double r = __ddiv_rn(__dadd_rn(s, c), __dmul_rn(2.0, a));
-  if (diag_add != nullptr && n == m) r = __dadd_rn(r, diag_add[e * n_chan + n]);
-  R_out[idx] = r;
 }
 
 }  // namespace pstgf
