@@ -296,6 +296,17 @@ pstgf_status_t pstgf_debug_set_slab_policy(int policy);
 pstgf_status_t pstgf_debug_set_pair_policy(int policy);
 
 /*
+ * A pair-form wave with at most 16 channels and little work in all (n_chan^2 n_poles n_E <= 2^29, e.g. BASELINE.json
+ * configs[0]) is done by a one-launch kernel without scratch when it is the only wave of a call
+ * (PSTGF_SMALL_AUTO); PSTGF_SMALL_NONE sends it through the persistent kernel like any pair-form wave,
+ * PSTGF_SMALL_ALWAYS drops the bound on the work.  Same bits either way.
+ */
+#define PSTGF_SMALL_AUTO 0
+#define PSTGF_SMALL_NONE 1
+#define PSTGF_SMALL_ALWAYS 2
+pstgf_status_t pstgf_debug_set_small_policy(int policy);
+
+/*
  * How pstgf_rmat_form_batch_host overlaps formation and copy-back.
  * PSTGF_HOST_PIPELINE_AUTO (default): one launch per device-sized chunk of R; every piece of at
  * most max_chunk_bytes has a completion counter the kernel bumps, the arrival that completes a piece raises a

@@ -113,6 +113,7 @@ pstgf_status_t check_wave(const pstgf_wave_t &w) {
 thread_local int tl_tail_policy = PSTGF_TAIL_AUTO;
 thread_local int tl_slab_policy = PSTGF_SLAB_AUTO;
 thread_local int tl_pair_policy = PSTGF_PAIRS_AUTO;
+thread_local int tl_small_policy = PSTGF_SMALL_AUTO;
 thread_local int tl_host_pipeline = PSTGF_HOST_PIPELINE_AUTO;
 thread_local unsigned int tl_upload_timeout_ms = 0;   // 0 = the kernel's default (2 s)
 thread_local int tl_stall_upload = 0;
@@ -147,15 +148,17 @@ void plan_wave(const pstgf_wave_t &w, DevWave &d, int l2_bytes) {
   d.l2_keep = (l2_bytes > 0 && w_bytes <= 0.5 * (double)l2_bytes) ? 1 : 0;
 }
 
-// A wave in the pair form has its 128-pair items in the "coarse" section and its 32-pair tail in the "fine" one.
+// A wave in the pair form has its 128-pair items in section 0, its 64-pair items in section 1 (where the slab items
+// of the symmetric form are) and its 32-pair items in section 2.
 long long coarse_items(const DevWave &d) {
-  return d.n_pairs > 0 ? (long long)d.pair_mt * d.pair_nt_coarse : (long long)d.n_tiles * d.n_eb_coarse;
+  return d.n_pairs > 0 ? pstgf::pair_section_items(d, 0) : (long long)d.n_tiles * d.n_eb_coarse;
 }
 long long slab_items(const DevWave &d) {
-  return d.n_pairs > 0 ? 0 : (long long)pstgf::slab_tiles(d.slab_nt) * (d.slab_g2 + d.slab_g1);
+  return d.n_pairs > 0 ? pstgf::pair_section_items(d, 1)
+                       : (long long)pstgf::slab_tiles(d.slab_nt) * (d.slab_g2 + d.slab_g1);
 }
 long long fine_items(const DevWave &d) {
-  return d.n_pairs > 0 ? (long long)d.pair_mtf * (d.pair_nt - d.pair_nt_coarse)
+  return d.n_pairs > 0 ? pstgf::pair_section_items(d, 2)
                        : (long long)pstgf::fine_tiles(d.n_j) * (d.n_eb - d.n_eb_coarse);
 }
 long long wave_items(const DevWave &d) { return coarse_items(d) + slab_items(d) + fine_items(d); }
@@ -174,6 +177,15 @@ bool wants_pair_form(int n_chan, int n_poles, int n_E) {
   if (n_chan <= 0 || n_poles <= 0 || n_chan > pstgf::PAIR_MAX_CHAN) return false;
   if (tl_pair_policy == PSTGF_PAIRS_ALWAYS) return n_E > 0;
   return n_E >= pstgf::PAIR_MIN_E;
+}
+// A pair-form wave that is tiny -- few channels and little work in all -- goes to the one-launch kernel of
+// rmat_small.cu (single-wave calls only).  It computes the pair form term for term, so this is a choice of speed, not
+// of bits: the persistent kernel needs a scratch-builder launch, a ring and 128-energy items, which cost such a wave
+// tens of microseconds.
+constexpr double SMALL_MAX_FLOP = 536870912.0;       // n_chan^2 n_poles n_E = 2^29, about 15 us of the FP64 pipe: measured crossover 6e8 - 1e9
+bool wants_small_kernel(int n_chan, int n_poles, int n_E) {
+  if (tl_small_policy == PSTGF_SMALL_NONE || n_chan > pstgf::SMALL_MAX_CHAN) return false;
+  return tl_small_policy == PSTGF_SMALL_ALWAYS || (double)n_chan * n_chan * (double)n_poles * (double)n_E <= SMALL_MAX_FLOP;
 }
 long long pair_count(int n_chan) { return (long long)n_chan * (n_chan + 1) / 2; }
 long long pair_ld(int n_poles) { return ((long long)n_poles + 1) & ~1LL; }
@@ -198,24 +210,70 @@ void plan_pairs(DevWave &d, unsigned char *scratch) {
   d.pair_rb = pstgf::pair_block_rows(d.n_chan);
   d.pair_mt = (d.n_pairs + pstgf::PT_M - 1) / pstgf::PT_M;
   d.pair_mtf = (d.n_pairs + pstgf::PT_MF - 1) / pstgf::PT_MF;
+  d.pair_mtff = (d.n_pairs + pstgf::PT_MFF - 1) / pstgf::PT_MFF;
   d.pair_nt = (d.n_E + pstgf::PT_N - 1) / pstgf::PT_N;
-  d.pair_nt_coarse = d.pair_nt;
+  d.pair_nt_coarse = d.pair_nt_mid = d.pair_nt;
   // no classic or slab items
   d.n_eb = d.n_eb_coarse = 0;
   d.slab_g2 = d.slab_g1 = 0;
   d.slab_e0 = d.n_E;
 }
 
-// Relative cost of a wave's pair items: row blocks per item (16, fewer in the last pair tile; 8 for fine items)
-double pair_last_tile_blocks(const DevWave &d) {
-  const int left = d.n_pairs - (d.pair_mt - 1) * pstgf::PT_M;
-  return left > 64 ? 16.0 : left > 32 ? 8.0 : 4.0;
+// Relative cost of a wave's pair items in row blocks of 8 pairs per item: 16 / 8 / 4 for the three tile heights
+// (fewer in a wave's last pair tile), times a factor for the shorter register tiles' inner loops.
+// Measured item times on config 2 (per-CTA timestamps, 64 k-tiles per item): 172.6 us for 16 row blocks, 97.8 us for 8,
+// 49.6 - 61.5 us for 4, i.e. 9.35 us per row block plus 23 us per item -- the short items reload the same 128 energies
+// of D for fewer pairs and run into the L2 -> SM bandwidth (3.5 TB/s chip-wide for 64-pair items).
+constexpr double PAIR_Q[3] = {1.0, 1.0, 1.0};
+constexpr double PAIR_ITEM_FIXED = 2.5;              // per item, in row blocks
+double pair_last_tile_blocks(const DevWave &d, int sec) {
+  const int rows = pstgf::PT_M >> sec;
+  const int left = d.n_pairs - ((d.n_pairs + rows - 1) / rows - 1) * rows;
+  return std::min<double>(rows / 8, left > 64 ? 16.0 : left > 32 ? 8.0 : 4.0);
+}
+int pair_tiles(const DevWave &d, int sec) { return sec == 0 ? d.pair_mt : sec == 1 ? d.pair_mtf : d.pair_mtff; }
+// Sets the section boundaries of a pair-form wave from item counts: the first n0 items of the 128-pair tiling are
+// section 0, then about n1 64-pair items (rounded up so that no energy tile is split three ways), the rest 32-pair.
+void pair_set_sections(DevWave &d, long long n0, long long n1) {
+  const int nt = d.pair_nt;
+  n0 = std::min<long long>(n0, (long long)d.pair_mt * nt);
+  d.pair_nt_coarse = (int)(n0 / d.pair_mt);
+  d.pair_x0 = (int)(n0 % d.pair_mt);
+  d.pair_x1 = 0;
+  if (d.pair_nt_coarse >= nt) {            // everything coarse
+    d.pair_nt_coarse = d.pair_nt_mid = nt;
+    d.pair_x0 = 0;
+    return;
+  }
+  const long long first = d.pair_x0 > 0 ? d.pair_mtf - 2 * d.pair_x0 : 0;    // the split energy tile's 64-pair items
+  const long long rest = std::max<long long>(0, n1 - first);
+  const int full = (int)std::min<long long>(rest / d.pair_mtf, nt - d.pair_nt_coarse - (d.pair_x0 > 0 ? 1 : 0));
+  d.pair_nt_mid = d.pair_nt_coarse + (d.pair_x0 > 0 ? 1 : 0) + full;
+  if (d.pair_nt_mid < nt) d.pair_x1 = (int)std::min<long long>(rest - (long long)full * d.pair_mtf, d.pair_mtf - 1);
 }
 
-// The tail of the launch's pair items -- about one round of the grid -- in 64-pair items (whole energy tiles), so
-// that the CTAs run dry together, like the fine tiles of the symmetric form.  One wave: the tail size with the
-// smallest simulated makespan; several waves: whole energy tiles from the end of the list until a round's worth of
-// work has been cut fine.
+// Item costs of a pair-form wave, item by item in the order the counter hands them out.
+void pair_item_costs(const DevWave &d, std::vector<std::pair<double, int>> &runs) {
+  runs.clear();
+  for (int sec = 0; sec < 3; ++sec) {
+    const long long n = pstgf::pair_section_items(d, sec);
+    const int rows = pstgf::PT_M >> sec, last_mt = pair_tiles(d, sec) - 1;
+    const double c_full = PAIR_Q[sec] * (rows / 8) + PAIR_ITEM_FIXED, c_last = PAIR_Q[sec] * pair_last_tile_blocks(d, sec) + PAIR_ITEM_FIXED;
+    for (long long i = 0; i < n; ++i) {
+      int mt, nt;
+      pstgf::pair_decode_item(d, sec, i, mt, nt);
+      const double c = mt == last_mt ? c_last : c_full;
+      if (!runs.empty() && runs.back().first == c) ++runs.back().second;
+      else runs.emplace_back(c, 1);
+    }
+  }
+}
+
+// The tail of the launch's pair items -- about one round of the grid -- in 64-pair and, at the very end, 32-pair items,
+// so that the CTAs run dry together, like the fine tiles of the symmetric form.  One wave: the section sizes (in
+// items: the boundaries may cut through an energy tile) with the smallest simulated makespan among those that end the
+// 128-pair section near a whole number of rounds of the grid; several waves: whole energy tiles from the end of the
+// list until a quarter of a round's worth of work has been cut into 32-pair items and a round's worth into 64-pair items.
 void plan_pair_tails(std::vector<DevWave> &ds, int grid) {
   if (tl_tail_policy == PSTGF_TAIL_NONE) return;
   std::vector<DevWave *> pw;
@@ -223,57 +281,67 @@ void plan_pair_tails(std::vector<DevWave> &ds, int grid) {
     if (d.n_pairs > 0) pw.push_back(&d);
   if (pw.empty()) return;
   if (tl_tail_policy == PSTGF_TAIL_ALL) {
-    for (DevWave *d : pw) d->pair_nt_coarse = 0;
+    for (DevWave *d : pw) {               // a bit of everything, with both boundaries inside an energy tile where there is room
+      const long long all = (long long)d->pair_mt * d->pair_nt;
+      pair_set_sections(*d, all / 3 + (d->pair_mt > 1 ? 1 : 0), (long long)d->pair_mtf * d->pair_nt / 3 + (d->pair_mtf > 1 ? 1 : 0));
+    }
     return;
   }
   if (pw.size() == 1 && ds.size() == 1) {
     DevWave &d = *pw[0];
-    if ((long long)d.pair_mt * d.pair_nt > 16LL * grid) {      // many rounds: one energy tile of fine items is tail enough
-      d.pair_nt_coarse = std::max(0, d.pair_nt - 1);
-      return;
-    }
-    // cached per shape: the simulation costs a millisecond of host time for a few thousand items
+    // cached per shape: the simulation costs a millisecond or two of host time for a few thousand items
     static std::mutex cache_mutex;
-    static std::map<std::tuple<int, int, int>, int> cache;      // (n_pairs, energy tiles, grid) -> fine energy tiles
+    static std::map<std::tuple<int, int, int>, std::pair<long long, long long>> cache;   // (n_pairs, energy tiles, grid) -> (n0, n1)
     const auto key = std::make_tuple(d.n_pairs, d.pair_nt, grid);
     {
       std::lock_guard<std::mutex> lock(cache_mutex);
       auto it = cache.find(key);
       if (it != cache.end()) {
-        d.pair_nt_coarse = d.pair_nt - it->second;
+        pair_set_sections(d, it->second.first, it->second.second);
         return;
       }
     }
-    const double c_last = pair_last_tile_blocks(d);
-    std::vector<std::pair<double, int>> runs;
-    int best_t = 0;
-    double best = 0.0;
-    for (int t = 0; t <= d.pair_nt; ++t) {
-      runs.clear();
-      if (d.pair_nt - t > 0) {
-        if (d.pair_mt > 1) runs.emplace_back(16.0, (d.pair_mt - 1) * (d.pair_nt - t));
-        runs.emplace_back(c_last, d.pair_nt - t);
-      }
-      if (t > 0) runs.emplace_back(8.0 * 1.08, d.pair_mtf * t);
-      const double m = simulate_makespan(runs, grid);
-      if (t == 0 || m < best * (1.0 - 1e-9)) {
-        best = m;
-        best_t = t;
-      }
+    const long long all = (long long)d.pair_mt * d.pair_nt;
+    std::vector<long long> c0, c1;
+    if (all > 64LL * grid) {              // many rounds: the last round and a half in 64-pair items, the last half round finer
+      c0.push_back(std::max<long long>(0, all - grid - grid / 2));
+      c1.push_back(2LL * grid);
+    } else {
+      // 128-pair sections that end up to a round short of the total, in steps of an eighth of a round; 64-pair
+      // sections of up to two rounds of the grid (two 64-pair items are one 128-pair item)
+      for (int i = 0; i <= 16; ++i) c0.push_back(std::max<long long>(0, all - (long long)i * grid / 8));
+      for (int i = 0; i <= 8; ++i) c1.push_back((long long)i * grid / 4);
     }
-    d.pair_nt_coarse = d.pair_nt - best_t;
+    std::vector<std::pair<double, int>> runs;
+    long long best_n0 = all, best_n1 = 0;
+    double best = -1.0;
+    for (long long n0 : c0)
+      for (long long n1 : c1) {
+        pair_set_sections(d, n0, n1);
+        pair_item_costs(d, runs);
+        const double m = simulate_makespan(runs, grid);
+        if (best < 0.0 || m < best * (1.0 - 1e-9)) {
+          best = m;
+          best_n0 = n0;
+          best_n1 = n1;
+        }
+      }
+    pair_set_sections(d, best_n0, best_n1);
     std::lock_guard<std::mutex> lock(cache_mutex);
-    cache[key] = best_t;
+    cache[key] = std::make_pair(best_n0, best_n1);
     return;
   }
-  double budget = 16.0 * grid;                                  // one round of full coarse items, in row blocks
-  for (size_t q = pw.size(); q-- > 0 && budget > 0.0;) {
+  double budget_fine = 4.0 * grid, budget_mid = 16.0 * grid;          // in row blocks
+  for (size_t q = pw.size(); q-- > 0 && budget_mid > 0.0;) {
     DevWave &d = *pw[q];
-    const double per_tile = 16.0 * (d.pair_mt - 1) + pair_last_tile_blocks(d);   // one energy tile of this wave
-    const int t = (int)std::min<double>((double)d.pair_nt, std::floor(budget / per_tile + 0.5));
-    if (t == 0) break;
-    d.pair_nt_coarse = d.pair_nt - t;
-    budget -= t * per_tile;
+    const double per_tile = 16.0 * (d.pair_mt - 1) + pair_last_tile_blocks(d, 0);   // one energy tile of this wave
+    const int t2 = budget_fine > 0.0 ? (int)std::min<double>((double)d.pair_nt, std::floor(budget_fine / per_tile + 0.5)) : 0;
+    budget_fine -= std::max(1, t2) * per_tile;                        // (a wave too big for it ends the 32-pair tail)
+    const int t1 = (int)std::min<double>((double)(d.pair_nt - t2), std::floor(budget_mid / per_tile + 0.5));
+    d.pair_nt_mid = d.pair_nt - t2;
+    d.pair_nt_coarse = d.pair_nt_mid - t1;
+    budget_mid -= (t1 + t2) * per_tile;
+    if (t1 + t2 == 0) break;
   }
 }
 
@@ -396,7 +464,7 @@ pstgf::RingGeo ring_geometry(const std::vector<DevWave> &ds) {
     int panels = 0;
     if (d.n_pairs > 0) panels = pstgf::PAIR_PANELS;
     else if (coarse_items(d) + fine_items(d) > 0) panels = pstgf::CLASSIC_PANELS;
-    if (slab_items(d) > 0) panels = std::max(panels, pstgf::slab_panels(d.slab_T));
+    if (d.n_pairs == 0 && slab_items(d) > 0) panels = std::max(panels, pstgf::slab_panels(d.slab_T));
     bytes = std::max(bytes, pstgf::stage_bytes_for(d.tr != 0 && d.n_pairs == 0, panels));
   }
   pstgf::RingGeo g;
@@ -707,6 +775,12 @@ pstgf_status_t pstgf_debug_set_pair_policy(int policy) {
   return PSTGF_OK;
 }
 
+pstgf_status_t pstgf_debug_set_small_policy(int policy) {
+  if (policy < PSTGF_SMALL_AUTO || policy > PSTGF_SMALL_ALWAYS) return PSTGF_ERR_INVALID_VALUE;
+  tl_small_policy = policy;
+  return PSTGF_OK;
+}
+
 pstgf_status_t pstgf_debug_set_slab_policy(int policy) {
   if (policy < PSTGF_SLAB_AUTO || policy > PSTGF_SLAB_T128) return PSTGF_ERR_INVALID_VALUE;
   tl_slab_policy = policy;
@@ -727,6 +801,11 @@ static pstgf_status_t form_single(const pstgf_wave_t &w, void *stream) {
   std::vector<DevWave> d(1);
   plan_wave(w, d[0], ds.l2_bytes);
   void *scratch = nullptr;
+  if (wants_pair_form(n_chan, n_poles, n_E) && wants_small_kernel(n_chan, n_poles, n_E)) {
+    PSTGF_CUDA(pstgf::small_launch(d[0], s));
+    tl_launches = 1;
+    return PSTGF_OK;
+  }
   if (wants_pair_form(n_chan, n_poles, n_E)) {
     // the pair form's scratch (P and D) is stream-ordered memory from the library's pool (kept between calls: the
     // device's default pool hands its memory back at every synchronise): allocated here, freed behind the launch
@@ -839,6 +918,17 @@ static pstgf_status_t form_batch_impl(const pstgf_wave_t *waves, int n_waves, vo
   std::stable_sort(order.begin(), order.end(),
                    [&](int x, int y) { return wave_item_cost(waves[x]) > wave_item_cost(waves[y]); });
   const int nw = (int)order.size();
+  if (nw == 1 && !completion) {
+    // one tiny wave: the one-launch kernel, as in the single-wave call (same bits: rmat_small.cu)
+    const pstgf_wave_t &w = waves[order[0]];
+    if (wants_pair_form(w.n_chan, w.n_poles, w.n_E) && wants_small_kernel(w.n_chan, w.n_poles, w.n_E)) {
+      DevWave d;
+      plan_wave(w, d, dstate.l2_bytes);
+      PSTGF_CUDA(pstgf::small_launch(d, s));
+      tl_launches = launches + 1;
+      return PSTGF_OK;
+    }
+  }
   // host image of the workspace: [counter | item_begin[3 nw + 1] | DevWave[nw]]; item sections are the coarse
   // items of every wave (largest first), then the slab items of every wave, then the fine items of every wave
   const size_t off_begin = WS_COUNTER_BYTES, off_waves = WS_COUNTER_BYTES + ws_item_begin_bytes(n_waves);

@@ -33,8 +33,9 @@
 //                    R[e][(n,m)] = (1/2a) sum_k P[(n,m)][k] * D[e][k],   P = w_nk w_mk,  D = 1/(E_k - E_e),
 //                with the n_chan (n_chan + 1) / 2 pairs n <= m as rows and the energies as columns: no block is
 //                cut by a diagonal and nothing is scaled inside the k loop.  P (once per wave) and D (once per
-//                energy) are written to scratch by a small kernel first; an item is (128 or 64 pairs) x 128 energies,
-//                each of the eight warps taking 16 energies (the WIDE register tile, 16 x 2 blocks).
+//                energy) are written to scratch by a small kernel first; an item is (128, 64 or 32 pairs) x 128
+//                energies, each of the eight warps taking 16 energies (the WIDE register tile, 16 x 2 blocks, or 8 x 2,
+//                4 x 2): 128-pair items first, then a tail of 64-pair and last of 32-pair items.
 // Only tiles on or above the diagonal exist ("half of the symmetric R-matrix"),
 // the mirror is written by the epilogue ("symmetrised").
 #pragma once
@@ -84,8 +85,12 @@ constexpr int slab_panels(int T) { return 2 * (T / TN); }   // 8, 4, 2 for slab 
 // Pair form (see above): pair tiles of 128 (coarse) or 64 (fine tail) rows of P, energy tiles of 128 rows of D.
 constexpr int PAIR_MAX_CHAN = 96;        // 4656 pairs; P is 71 MB at n_poles = 20 n_chan
 constexpr int PAIR_MIN_E = 64;           // fewer energies than this do not fill an energy tile's eight warps
-constexpr int PT_M = 128, PT_MF = 64, PT_N = 128;
+constexpr int PT_M = 128, PT_MF = 64, PT_MFF = 32, PT_N = 128;   // pair tile rows of section s: PT_M >> s
 constexpr int PAIR_PANELS = (PT_M + PT_N) / TN;             // 8
+// Tiny waves (pair form, at most SMALL_MAX_CHAN channels, little work in all) are done by a kernel of their own
+// (rmat_small.cu): one CTA per block of 8 energies, at most SMALL_MAX_WARPS warps that split the blocks of 8 pairs.
+constexpr int SMALL_MAX_CHAN = 16;       // 136 pairs: 17 blocks of 8
+constexpr int SMALL_MAX_WARPS = 6;
 // Item families a launch can hold; the persistent kernel is compiled once per value (a template parameter), so that a
 // launch of classic items only does not carry the code of the others.
 constexpr int FAM_CLASSIC = 0, FAM_SLAB = 1, FAM_PAIR = 2;
@@ -157,13 +162,60 @@ struct alignas(128) DevWave {
   long long pair_ld;       // even, >= n_poles
   int n_pairs;             // n_chan (n_chan + 1) / 2, or 0 when the wave is done in the SYRK form
   int pair_nt;             // energy tiles of PT_N
-  int pair_nt_coarse;      // energy tiles [0, pair_nt_coarse) are cut into pair tiles of PT_M rows, the rest (the tail) of PT_MF
-  int pair_mt, pair_mtf;   // pair tiles of PT_M / of PT_MF rows
+  int pair_nt_coarse;      // energy tiles [0, pair_nt_coarse) are cut into pair tiles of PT_M rows (section 0), ...
+  int pair_nt_mid;         // ... [pair_nt_coarse, pair_nt_mid) of PT_MF rows (section 1), the rest of PT_MFF rows (section 2)
+  int pair_mt, pair_mtf, pair_mtff;   // pair tiles of PT_M / PT_MF / PT_MFF rows
+  int pair_x0;             // the first pair_x0 128-pair tiles of energy tile pair_nt_coarse are section-0 items too (< pair_mt; 0 unless pair_nt_coarse < pair_nt_mid)
+  int pair_x1;             // the first pair_x1 64-pair tiles of energy tile pair_nt_mid are section-1 items too (< pair_mtf; 0 unless pair_nt_mid < pair_nt)
   int pair_nfb;            // n_chan / 8: channel blocks that are full
   int pair_rb;             // rows of P in the block section: 64 pair_nfb (pair_nfb - 1) / 2, see pair_row_channels
   const unsigned int *pair_nm;   // scratch [n_pairs]: n | m << 16 of every row of P (written by the scratch builder)
 };
 static_assert(sizeof(DevWave) == 640, "DevWave layout (alignas 128; the batch workspace holds an array of these)");
+
+// Pair form: the items of a wave, section by section.  Section s holds (PT_M >> s)-pair tiles: section 0 the energy
+// tiles [0, pair_nt_coarse) and the first pair_x0 tiles of energy tile pair_nt_coarse; section 1 the rest of that energy
+// tile (its 64-pair tiles from 2 pair_x0 on), the energy tiles up to pair_nt_mid and the first pair_x1 tiles of energy
+// tile pair_nt_mid; section 2 the rest.  The ragged boundaries let the planner end each section after any number of
+// items, not only after whole energy tiles: with 3.7 rounds of 128-pair items on the grid (config 2) that is worth 5 %.
+__host__ __device__ inline long long pair_section_items(const DevWave &w, int sec) {
+  if (sec == 0) return (long long)w.pair_mt * w.pair_nt_coarse + w.pair_x0;
+  const int x = sec == 1 ? w.pair_x0 : w.pair_x1, tiles = sec == 1 ? w.pair_mtf : w.pair_mtff;
+  const int first = sec == 1 ? w.pair_nt_coarse : w.pair_nt_mid, end = sec == 1 ? w.pair_nt_mid : w.pair_nt;
+  return (x > 0 ? tiles - 2 * x : 0) + (long long)tiles * (end - first - (x > 0 ? 1 : 0)) + (sec == 1 ? w.pair_x1 : 0);
+}
+// item of section sec -> (pair tile mt in units of PT_M >> sec rows, energy tile nt)
+__host__ __device__ inline void pair_decode_item(const DevWave &w, int sec, long long item, int &mt, int &nt) {
+  if (sec == 0) {
+    const long long reg = (long long)w.pair_mt * w.pair_nt_coarse;
+    if (item < reg) {                      // energy tile fastest: CTAs side by side share a P panel
+      mt = (int)(item / w.pair_nt_coarse);
+      nt = (int)(item - (long long)mt * w.pair_nt_coarse);
+    } else {
+      mt = (int)(item - reg);
+      nt = w.pair_nt_coarse;
+    }
+    return;
+  }
+  const int x = sec == 1 ? w.pair_x0 : w.pair_x1, tiles = sec == 1 ? w.pair_mtf : w.pair_mtff;
+  const int first = sec == 1 ? w.pair_nt_coarse : w.pair_nt_mid, end = sec == 1 ? w.pair_nt_mid : w.pair_nt;
+  const int first_cnt = x > 0 ? tiles - 2 * x : 0;
+  if (item < first_cnt) {
+    nt = first;
+    mt = 2 * x + (int)item;
+    return;
+  }
+  item -= first_cnt;
+  const int r0 = first + (x > 0 ? 1 : 0), n_reg = end - r0;
+  const long long reg = (long long)tiles * n_reg;
+  if (item < reg) {
+    mt = (int)(item / n_reg);
+    nt = r0 + (int)(item - (long long)mt * n_reg);
+  } else {
+    mt = (int)(item - reg);
+    nt = end;
+  }
+}
 
 // Host-side tile arithmetic (also used by the kernel's decoder).
 // WIDE tiles of row pair p: columns from 128 (p + 1) to the end, 16 at a time.

@@ -758,8 +758,9 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
             p = lo - sec * n_waves;
           } else {
             const bool sp = single.n_pairs > 0;
-            const long long n_coarse = sp ? (long long)single.pair_mt * single.pair_nt_coarse : (long long)single.n_tiles * single.n_eb_coarse;
-            const long long n_slab = sp ? 0 : (long long)slab_tiles(single.slab_nt) * (single.slab_g2 + single.slab_g1);
+            const long long n_coarse = sp ? pair_section_items(single, 0) : (long long)single.n_tiles * single.n_eb_coarse;
+            const long long n_slab = sp ? pair_section_items(single, 1)
+                                        : (long long)slab_tiles(single.slab_nt) * (single.slab_g2 + single.slab_g1);
             if (item >= n_coarse + n_slab) { sec = 2; item -= n_coarse + n_slab; }
             else if (item >= n_coarse) { sec = 1; item -= n_coarse; }
           }
@@ -768,17 +769,15 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
         int kind = -1, row0 = 0, col0 = 0, nblk = 0, nrb = 0, e_first = 0, n_valid = 0, n_kt = 0, slab_T = 0, slab_g = 0;
         if (!stop) {
           if (w.n_pairs > 0) {
-            // pair form: section 0 holds the wave's (128-pair tile, energy tile) items, section 2 its fine tail
-            // (64-pair tiles of the last energy tiles); energy tile fastest, so CTAs side by side share a P panel
-            const bool fine = sec == 2;
-            const int n_nt_sec = fine ? w.pair_nt - w.pair_nt_coarse : w.pair_nt_coarse;
-            const int mt = (int)(item / n_nt_sec);
-            const int nt = (int)(item - (long long)mt * n_nt_sec) + (fine ? w.pair_nt_coarse : 0);
+            // pair form: section s holds (PT_M >> s)-pair tiles: 128-pair items, then the tail in 64-pair and last in
+            // 32-pair items (rmat_common.h: pair_section_items)
+            int mt, nt;
+            pair_decode_item(w, sec, item, mt, nt);
             kind = 2;
-            row0 = mt * (fine ? PT_MF : PT_M);
+            row0 = mt * (PT_M >> sec);
             col0 = nt * PT_N;
             const int left = w.n_pairs - row0;
-            nblk = left > 64 && !fine ? 16 : left > 32 ? 8 : 4;
+            nblk = min(PT_M >> (sec + 3), left > 64 ? 16 : left > 32 ? 8 : 4);
             e_first = col0;
             n_valid = min(PT_N, w.n_E - col0);
           } else if (sec == 1) {

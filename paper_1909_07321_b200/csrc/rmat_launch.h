@@ -29,6 +29,10 @@ cudaError_t persistent_launch_f0(bool batch, const PersistentArgs &a, cudaStream
 cudaError_t persistent_launch_f1(bool batch, const PersistentArgs &a, cudaStream_t s);
 cudaError_t persistent_launch_f2(bool batch, const PersistentArgs &a, cudaStream_t s);
 
+// rmat_small.cu: eq. 4 for a tiny wave (pair form, n_chan <= SMALL_MAX_CHAN) in one launch; uses W, E_k, energies,
+// R_out, diag_add, ldw, inv2a, n_chan, n_poles, n_E and tr of `w`.
+cudaError_t small_launch(const DevWave &w, cudaStream_t s);
+
 inline cudaError_t persistent_prepare_all() {
   cudaError_t e = persistent_prepare_f0();
   if (e == cudaSuccess) e = persistent_prepare_f1();

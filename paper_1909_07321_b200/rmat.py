@@ -19,12 +19,13 @@ PSTGF_W_POLE_CONTIGUOUS, PSTGF_W_CHANNEL_CONTIGUOUS = 0, 1
 PSTGF_HOST_PIPELINE_AUTO, PSTGF_HOST_PIPELINE_CHUNKED = 0, 1
 PSTGF_SLAB_AUTO, PSTGF_SLAB_NONE, PSTGF_SLAB_T32, PSTGF_SLAB_T64, PSTGF_SLAB_T128 = 0, 1, 2, 3, 4
 PSTGF_PAIRS_AUTO, PSTGF_PAIRS_NONE, PSTGF_PAIRS_ALWAYS = 0, 1, 2
+PSTGF_SMALL_AUTO, PSTGF_SMALL_NONE, PSTGF_SMALL_ALWAYS = 0, 1, 2
 PSTGF_ERR_TIMEOUT, PSTGF_ERR_CAPTURE = 6, 7
 PSTGF_RMAT_VERSION = 200            # must equal include/pstgf_rmat.h; load() checks it against the library
 
 EXPORTS = ["pstgf_rmat_form", "pstgf_rmat_form_hdat", "pstgf_rmat_batch_workspace_bytes", "pstgf_rmat_form_batch",
            "pstgf_rmat_form_naive", "pstgf_rmat_form_batch_host", "pstgf_mesh_from_zscaled", "pstgf_rmat_finalize",
-           "pstgf_debug_set_tail_policy", "pstgf_debug_set_slab_policy", "pstgf_debug_set_pair_policy",
+           "pstgf_debug_set_tail_policy", "pstgf_debug_set_slab_policy", "pstgf_debug_set_pair_policy", "pstgf_debug_set_small_policy",
            "pstgf_debug_set_host_pipeline",
            "pstgf_debug_set_upload_timeout_ms", "pstgf_debug_stall_upload", "pstgf_last_launch_count",
            "pstgf_status_string", "pstgf_last_cuda_error", "pstgf_version"]
@@ -81,7 +82,7 @@ def load(build_if_missing: bool = False):
     lib.pstgf_rmat_form_batch.restype = i
     lib.pstgf_rmat_form_batch_host.argtypes = [ctypes.POINTER(pstgf_wave_t), i, sz, vp]
     lib.pstgf_rmat_form_batch_host.restype = i
-    for name in ("pstgf_debug_set_tail_policy", "pstgf_debug_set_slab_policy", "pstgf_debug_set_pair_policy",
+    for name in ("pstgf_debug_set_tail_policy", "pstgf_debug_set_slab_policy", "pstgf_debug_set_pair_policy", "pstgf_debug_set_small_policy",
                  "pstgf_debug_set_host_pipeline",
                  "pstgf_debug_stall_upload"):
         getattr(lib, name).argtypes = [i]
@@ -246,6 +247,11 @@ def pstgf_debug_set_slab_policy(policy: int) -> None:
 def pstgf_debug_set_pair_policy(policy: int) -> None:
     """Thread-local: which waves take the GEMM-over-channel-pairs form (PSTGF_PAIRS_AUTO / _NONE / _ALWAYS)."""
     _check(load().pstgf_debug_set_pair_policy(int(policy)))
+
+
+def pstgf_debug_set_small_policy(policy: int) -> None:
+    """Thread-local: whether a tiny pair-form wave takes the one-launch kernel (PSTGF_SMALL_AUTO / _NONE / _ALWAYS); same bits."""
+    _check(load().pstgf_debug_set_small_policy(int(policy)))
 
 
 def pstgf_debug_set_host_pipeline(mode: int) -> None:

@@ -111,7 +111,7 @@ def test_argument_errors_need_no_device(lib):
     assert lib.pstgf_rmat_form_naive(ctypes.byref(w), None) == 2                        # misaligned diag_add
     assert lib.pstgf_rmat_form_naive(None, None) == 1
     for name, bad in (("pstgf_debug_set_tail_policy", 5), ("pstgf_debug_set_slab_policy", 9), ("pstgf_debug_set_pair_policy", 3),
-                      ("pstgf_debug_set_host_pipeline", 3)):
+                      ("pstgf_debug_set_small_policy", 3), ("pstgf_debug_set_host_pipeline", 3)):
         f = getattr(lib, name)
         f.argtypes, f.restype = [i], i
         assert f(bad) == 1 and f(0) == 0

@@ -332,6 +332,50 @@ def test_pair_form_edge_shapes(rmat, oracle, pair_policy, tail_policy, C, K, N):
     assert np.array_equal(Rh.numpy(), results[0])
 
 
+SMALL_SHAPES = [(1, 5, 64), (7, 161, 65), (8, 160, 1000), (9, 500, 100), (12, 323, 77), (15, 61, 128), (16, 333, 71), (16, 20, 64)]
+
+
+@pytest.mark.parametrize("C,K,N", SMALL_SHAPES)
+def test_small_wave_kernel(rmat, oracle, C, K, N):
+    """A tiny pair-form wave (n_chan <= 16, little work) is done by the one-launch kernel of rmat_small.cu in the
+    single-wave calls: one launch, <= 1e-13 against the oracle, and bitwise what the persistent kernel's pair items
+    give for the same wave in a batch call (several pole chunks of 160, a ragged last chunk, a ragged last energy
+    block, both memory orders of W, the diagonal addend)."""
+    from paper_1909_07321_b200 import inputs
+    w = inputs.make_wave(13000 + 17 * C + N, C, K, N)
+    da = np.random.default_rng(C * N).normal(0.0, 0.05, (N, C))
+    Wd, Wt, Ek, en, dad = _dev(w.W), _dev(w.W.T), _dev(w.E_k), _dev(w.energies), _dev(da)
+    R = rmat.pstgf_rmat_form(Wd, Ek, en, w.a)
+    assert rmat.pstgf_last_launch_count() == 1
+    Rh = rmat.pstgf_rmat_form_hdat(Wt, Ek, en, w.a)
+    assert rmat.pstgf_last_launch_count() == 1
+    torch.cuda.synchronize()
+    R, Rh = R.cpu().numpy(), Rh.cpu().numpy()
+    _check(R, oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads()))
+    assert np.array_equal(R, Rh)
+    # the same wave in a batch beside another one (persistent kernel, pair items): bitwise the same
+    other = inputs.make_wave(78, 40, 60, 70)
+    Rb = torch.full((N, C, C), float("nan"), dtype=torch.float64, device="cuda")
+    Ro = torch.empty((other.n_E, 40, 40), dtype=torch.float64, device="cuda")
+    keep = [(_dev(other.W), _dev(other.E_k), _dev(other.energies), other.a, Ro), (Wd, Ek, en, w.a, Rb)]
+    arr = rmat.make_wave_array(keep)
+    ws = torch.empty(rmat.pstgf_rmat_batch_workspace_bytes(arr), dtype=torch.uint8, device="cuda")
+    rmat.pstgf_rmat_form_batch(arr, ws)
+    assert rmat.pstgf_last_launch_count() == 2
+    torch.cuda.synchronize()
+    assert np.array_equal(Rb.cpu().numpy(), R)
+    # a batch of this one wave takes the one-launch kernel too, here with the diagonal addend
+    Rd = torch.full((N, C, C), float("nan"), dtype=torch.float64, device="cuda")
+    one = rmat.make_wave_array([(Wd, Ek, en, w.a, Rd, rmat.PSTGF_W_POLE_CONTIGUOUS, dad)])
+    rmat.pstgf_rmat_form_batch(one, ws)
+    assert rmat.pstgf_last_launch_count() == 1
+    torch.cuda.synchronize()
+    Rd = Rd.cpu().numpy()
+    _check(Rd, oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads(), diag_add=da))
+    idx, off = np.arange(C), ~np.eye(C, dtype=bool)
+    assert np.array_equal(Rd[:, off], R[:, off]) and np.array_equal(Rd[:, idx, idx], R[:, idx, idx] + da)
+
+
 def test_pair_form_is_chosen_by_shape_alone(rmat, oracle):
     """Default policy: a wave takes the pair form iff n_chan <= 96 and n_E >= 64, whatever else is in the batch, so
     single, batch and host calls agree bitwise; the host call cuts the wave into energy ranges of fewer than 64
