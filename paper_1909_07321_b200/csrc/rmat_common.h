@@ -118,7 +118,10 @@ struct SlabShape {
 __host__ __device__ inline SlabShape slab_shape(int T, int g) {
   if (T == 128) return SlabShape{8, 16, 2};                 // g = 1 only: 8 warps x (16 x 2 blocks), the WIDE register tile
   if (T == 64) return g == 1 ? SlabShape{4, 4, 2} : SlabShape{4, 8, 2};
-  return g == 1 ? SlabShape{4, 2, 1} : SlabShape{2, 2, 2};  // T == 32
+  // T == 32: 2 x 2 warps of 2 x 2 blocks for either group size.  With one energy that leaves four of the eight warps
+  // idle, on purpose: 8 warps of 2 x 1 blocks issue 4 LDS.64 per 2 DMMA each, which is all of the SM's shared-memory
+  // bandwidth (ncu: 48 % of its peak at 52 % DMMA utilisation); 2 x 2 blocks need 5 per 4.
+  return SlabShape{2, 2, 2};
 }
 
 // One partial wave as the kernel sees it.  Built on the host, lives in kernel parameter

@@ -241,8 +241,17 @@ __device__ __forceinline__ void consume_off(const ItemInfo &it, Pipe &ps, int wa
     for (int bi = 0; bi < NRB; ++bi) {
       const int r = it.row0 + bi * 8 + g;
       const double v0 = acc[bi][bj][0] * s, v1 = acc[bi][bj][1] * s;
-      if (c < C) { __stcs(R + (size_t)r * C + c, v0); __stcs(R + (size_t)c * C + r, v0); }
-      if (c + 1 < C) { __stcs(R + (size_t)r * C + c + 1, v1); __stcs(R + (size_t)(c + 1) * C + r, v1); }
+      // R[r][c], R[r][c+1] are neighbours: one 16-byte store when the address allows it (always, for an even n_chan
+      // and a 16-byte aligned R_out); the mirror elements R[c][r], R[c+1][r] are a row apart
+      double *direct = R + (size_t)r * C + c;
+      if (c + 1 < C && (reinterpret_cast<uintptr_t>(direct) & 15u) == 0) {
+        __stcs(reinterpret_cast<double2 *>(direct), make_double2(v0, v1));
+        __stcs(R + (size_t)c * C + r, v0);
+        __stcs(R + (size_t)(c + 1) * C + r, v1);
+      } else {
+        if (c < C) { __stcs(direct, v0); __stcs(R + (size_t)c * C + r, v0); }
+        if (c + 1 < C) { __stcs(direct + 1, v1); __stcs(R + (size_t)(c + 1) * C + r, v1); }
+      }
     }
   }
 }
@@ -527,10 +536,7 @@ __device__ __forceinline__ void consume_item_layout(const ItemInfo &it, Pipe &ps
       case 16: consume_slab<16, 2, 1, TR>(it, ps, warp, lane, sh.wc); break;
       case 8: consume_slab<8, 2, 1, TR>(it, ps, warp, lane, sh.wc); break;
       case 4: consume_slab<4, 2, 1, TR>(it, ps, warp, lane, sh.wc); break;
-      default:
-        if (sh.ncw == 2) consume_slab<2, 2, 1, TR>(it, ps, warp, lane, sh.wc);
-        else consume_slab<2, 1, 1, TR>(it, ps, warp, lane, sh.wc);
-        break;
+      default: consume_slab<2, 2, 1, TR>(it, ps, warp, lane, sh.wc); break;
     }
     return;
   }
