@@ -817,7 +817,8 @@ static pstgf_status_t form_single(const pstgf_wave_t &w, void *stream) {
     st = encode_pair_maps(d[0]);
     if (st == PSTGF_OK) {
       const int rows = d[0].n_E + d[0].n_pairs;
-      pstgf::pair_build_kernel<false><<<dim3((unsigned)std::min(rows, 8 * ds.sm_count), 1), 256, 0, s>>>(d[0], nullptr, 1);
+      const int chunks = (rows + pstgf::PAIR_BUILD_ROWS - 1) / pstgf::PAIR_BUILD_ROWS;
+      pstgf::pair_build_kernel<false><<<dim3((unsigned)std::min(chunks, 8 * ds.sm_count), 1), 256, 0, s>>>(d[0], nullptr, 1);
       if (cudaGetLastError() != cudaSuccess) st = PSTGF_ERR_CUDA;
     }
     if (st != PSTGF_OK) {
@@ -1029,7 +1030,7 @@ static pstgf_status_t form_batch_impl(const pstgf_wave_t *waves, int n_waves, vo
     // P and D of every pair-form wave in one launch (grid.y = the waves; the others return at once)
     DevWave none;
     std::memset(&none, 0, sizeof(none));
-    const int bx = std::max(1, std::min(max_build_rows, std::max(8, 8 * dstate.sm_count / nw)));
+    const int bx = std::max(1, std::min((max_build_rows + pstgf::PAIR_BUILD_ROWS - 1) / pstgf::PAIR_BUILD_ROWS, std::max(2, 8 * dstate.sm_count / nw)));
     pstgf::pair_build_kernel<true><<<dim3((unsigned)bx, (unsigned)std::min(nw, 65535)), 256, 0, s>>>(none, reinterpret_cast<const DevWave *>(ws + off_waves), nw);
     PSTGF_CUDA(cudaGetLastError());
     ++launches;
