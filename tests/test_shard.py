@@ -103,3 +103,24 @@ def test_two_ranks_gloo_reassemble_the_whole_mesh():
         pr.join(120)
         assert pr.exitcode == 0
     assert ret.get(timeout=10) is True
+
+
+@pytest.mark.parametrize("scaling,world", [("weak", 2), ("weak", 4), ("strong", 2), ("strong", 8)])
+def test_bench_job_is_partitioned_exactly(scaling, world):
+    """bench.py --gpus N: the ranks' shares (shard.plan over the job's meshes) are a disjoint cover of the job --
+    weak scaling multiplies the mesh by N, strong scaling keeps the configuration's own mesh -- so that
+    value = job energies / max-over-ranks time counts every energy once."""
+    import argparse
+    import bench
+    args = argparse.Namespace(config=1, n_E=0, scaling=scaling)
+    job = bench.job_workload(args, world)
+    base = bench.job_workload(args, 1)
+    assert job.n_energies() == (world if scaling == "weak" else 1) * base.n_energies()
+    for p, w in enumerate(job.waves):
+        seen = np.zeros(w.n_E, dtype=int)
+        for r in range(world):
+            for q, idx in shard.plan([x.n_E for x in job.waves], r, world):
+                if q == p:
+                    seen[idx] += 1
+        assert np.all(seen == 1)
+    assert bench.workload_description(1, job) == bench.workload_description(1, bench.job_workload(args, world))
