@@ -653,12 +653,15 @@ def test_R_out_in_mapped_host_memory(rmat):
         assert torch.equal(d[4].cpu(), Rh)
 
 
-def test_single_wave_call_in_a_cuda_graph(rmat, oracle):
+@pytest.mark.parametrize("C,K,N", [(137, 260, 27), (48, 300, 200), (8, 160, 100)])
+def test_single_wave_call_in_a_cuda_graph(rmat, oracle, C, K, N):
     """Under stream capture the single-wave call must not touch its counter pool (a replayed launch would
     reuse a slot it no longer owns): it falls back to round-robin item assignment.  Captured once, replayed
-    several times, also while ordinary launches are in flight; same bits as the eager call."""
+    several times, also while ordinary launches are in flight; same bits as the eager call.  The three shapes
+    take the symmetric form, the pair form (scratch from the library's stream-ordered pool: allocation and
+    free nodes in the graph) and the one-launch kernel for tiny waves."""
     from paper_1909_07321_b200 import inputs
-    w = inputs.make_wave(4711, 137, 260, 27)
+    w = inputs.make_wave(4711, C, K, N)
     Wd, Ek, en = _dev(w.W), _dev(w.E_k), _dev(w.energies)
     R_ref = oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads())
     eager = rmat.pstgf_rmat_form(Wd, Ek, en, w.a)
