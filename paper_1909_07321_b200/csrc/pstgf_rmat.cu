@@ -155,7 +155,7 @@ long long coarse_items(const DevWave &d) {
 }
 long long slab_items(const DevWave &d) {
   return d.n_pairs > 0 ? pstgf::pair_section_items(d, 1)
-                       : (long long)pstgf::slab_tiles(d.slab_nt) * (d.slab_g2 + d.slab_g1);
+                       : (long long)pstgf::slab_tiles(d.slab_nt) * pstgf::slab_groups(d.slab_g4, d.slab_g2, d.slab_g1);
 }
 long long fine_items(const DevWave &d) {
   return d.n_pairs > 0 ? pstgf::pair_section_items(d, 2)
@@ -215,7 +215,7 @@ void plan_pairs(DevWave &d, unsigned char *scratch) {
   d.pair_nt_coarse = d.pair_nt_mid = d.pair_nt;
   // no classic or slab items
   d.n_eb = d.n_eb_coarse = 0;
-  d.slab_g2 = d.slab_g1 = 0;
+  d.slab_g4 = d.slab_g2 = d.slab_g1 = 0;
   d.slab_e0 = d.n_E;
 }
 
@@ -370,61 +370,75 @@ double simulate_makespan(const std::vector<std::pair<double, int>> &runs, int gr
 }
 
 // ---- slab section: the energies that do not fill a block of 8 ------------------------------------
-// An item's time is set by its busiest warp: blocks per warp and k-step (SlabShape: nr x ncw), times a factor for
-// the quality of the warp's inner loop (fewer DMMAs per fragment load and per scaling multiply in the small
-// shapes; fitted to the B200 sweeps of bench.py --n-E), plus a fixed cost per item (epilogue, ring refill) in
-// units of k-tiles.
+// Time of a slab item per k-tile, in SM clocks: the slower of
+//  - its busiest SM sub-partition's DMMAs: blocks per warp (SlabShape: nr x ncw) x warps per sub-partition x 5 k-steps
+//    x 16 clk, times a factor for the quality of the warp's inner loop (fewer DMMAs per fragment load and per scaling
+//    multiply in the small shapes; fitted to the B200 sweeps of bench.py --n-E), and
+//  - its panels coming out of L2: with every SM loading, L2 delivers 4.2 TB/s chip-wide, 15 B/clk per SM (measured:
+//    one energy at 512 x 10240 on tiles of edge 32 runs at 634 clk per k-tile for 10 KB of panels),
+// plus a fixed cost per item (epilogue, ring refill) of three k-tiles.
+constexpr double L2_BYTES_PER_CLK_PER_SM = 15.0;
 double slab_item_cost(int T, int g, int n_kt) {
   const pstgf::SlabShape sh = pstgf::slab_shape(T, g);
   const int blocks = sh.nr * sh.ncw;
-  const double quality = blocks >= 32 ? 1.0 : blocks >= 16 ? 1.04 : blocks >= 8 ? 1.10 : blocks >= 4 ? 1.15 : 1.25;
-  return blocks * quality * ((double)n_kt + 3.0);
+  const double quality = blocks >= 32 ? 1.0 : blocks >= 16 ? 1.04 : blocks >= 8 ? 1.10 : 1.15;
+  const double warps_per_smsp = (T == 32 && g == 1) ? 1.0 : 2.0;          // (edge 32 with one energy keeps four warps idle)
+  const double compute = blocks * warps_per_smsp * 80.0 * quality;
+  const double l2 = pstgf::slab_panels(T) * (double)pstgf::BOX_BYTES / L2_BYTES_PER_CLK_PER_SM;
+  return std::max(compute, l2) * ((double)n_kt + 3.0);
 }
 
+struct SlabPlan {
+  int T, g4, g2, g1;
+};
 std::mutex g_slab_mutex;
-std::map<std::tuple<int, int, int, int>, int> g_slab_cache;   // (n_chan, remainder, n_kt bucket, grid) -> T
+std::map<std::tuple<int, int, int, int, int>, SlabPlan> g_slab_cache;   // (n_chan, remainder, n_kt bucket, grid, forced edge) -> plan
 
-// Tile edge of a wave's slab items: the candidate with the smallest simulated makespan of the slab items alone.
-// Large tiles have the better inner loop and the smaller L2 traffic, small tiles give the grid enough items.
-int best_slab_edge(int n_chan, int r, int n_kt, int grid) {
-  const auto key = std::make_tuple(n_chan, r, std::min(n_kt, 64), grid);
+// Tile edge and energy groups of a wave's slab items: the candidate with the smallest simulated makespan of the slab
+// items alone.  Large tiles have the better inner loop and the smaller L2 traffic, small tiles give the grid enough
+// items; groups of four or two energies share the tile's panels (tiles of edge 128 take one energy at a time), and a
+// group of four may hold three.
+SlabPlan best_slab_plan(int n_chan, int r, int n_kt, int grid, int forced_T) {
+  const auto key = std::make_tuple(n_chan, r, std::min(n_kt, 64), grid, forced_T);
   {
     std::lock_guard<std::mutex> lock(g_slab_mutex);
     auto it = g_slab_cache.find(key);
     if (it != g_slab_cache.end()) return it->second;
   }
-  int best_T = 32;
-  double best = 0.0;
+  SlabPlan best_plan{32, 0, 0, r};
+  double best = -1.0;
   std::vector<std::pair<double, int>> runs;
   for (int T : {128, 64, 32}) {
+    if (forced_T != 0 && T != forced_T) continue;
     const int nt = (n_chan + T - 1) / T;
     const long long tiles = pstgf::slab_tiles(nt);
-    const int g2 = T == 128 ? 0 : r / 2, g1 = T == 128 ? r : r % 2;
-    double m;
-    if (tiles * (g2 + g1) > 16LL * grid) {
-      // plenty of items: the makespan is the work divided by the grid, no need to simulate
-      m = (double)tiles * (g2 * slab_item_cost(T, 2, n_kt) + g1 * slab_item_cost(T, 1, n_kt)) / grid;
-    } else {
-      runs.clear();
-      // group-fastest order inside a tile; all tiles cost the same in this model (edge tiles are cheaper in fact)
-      if (g2 > 0 && g1 > 0) {
-        for (long long t = 0; t < tiles; ++t) {
-          runs.emplace_back(slab_item_cost(T, 2, n_kt), g2);
-          runs.emplace_back(slab_item_cost(T, 1, n_kt), g1);
-        }
+    for (int g4 = 0; g4 <= (T == 128 ? 0 : (r + 3) / 4); ++g4) {
+      const int rem = std::max(0, r - 4 * g4);
+      if (g4 > 0 && 4 * g4 - r > 1) continue;                            // a group of four holds four or three energies
+      const int g2 = T == 128 ? 0 : rem / 2, g1 = T == 128 ? rem : rem % 2;
+      const double c4 = g4 ? slab_item_cost(T, 4, n_kt) : 0.0, c2 = g2 ? slab_item_cost(T, 2, n_kt) : 0.0,
+                   c1 = g1 ? slab_item_cost(T, 1, n_kt) : 0.0;
+      double m;
+      if (tiles * (g4 + g2 + g1) > 16LL * grid) {
+        // plenty of items: the makespan is the work divided by the grid, no need to simulate
+        m = (double)tiles * (g4 * c4 + g2 * c2 + g1 * c1) / grid;
       } else {
-        runs.emplace_back(slab_item_cost(T, g2 > 0 ? 2 : 1, n_kt), (int)(tiles * (g2 + g1)));
+        runs.clear();
+        // group-major order, groups of four first; all tiles cost the same in this model (edge tiles are cheaper in fact)
+        if (g4) runs.emplace_back(c4, (int)(tiles * g4));
+        if (g2) runs.emplace_back(c2, (int)(tiles * g2));
+        if (g1) runs.emplace_back(c1, (int)(tiles * g1));
+        m = simulate_makespan(runs, grid);
       }
-      m = simulate_makespan(runs, grid);
-    }
-    if (best == 0.0 || m < best * (1.0 - 1e-9)) {
-      best = m;
-      best_T = T;
+      if (best < 0.0 || m < best * (1.0 - 1e-9)) {
+        best = m;
+        best_plan = SlabPlan{T, g4, g2, g1};
+      }
     }
   }
   std::lock_guard<std::mutex> lock(g_slab_mutex);
-  g_slab_cache[key] = best_T;
-  return best_T;
+  g_slab_cache[key] = best_plan;
+  return best_plan;
 }
 
 void plan_slabs(std::vector<DevWave> &ds, int grid) {
@@ -433,15 +447,16 @@ void plan_slabs(std::vector<DevWave> &ds, int grid) {
   for (DevWave &d : ds) {
     const int r = d.n_E % pstgf::EB;
     if (r == 0 || d.n_pairs > 0) continue;
-    int T = policy == PSTGF_SLAB_T32 ? 32 : policy == PSTGF_SLAB_T64 ? 64 : policy == PSTGF_SLAB_T128 ? 128
-                                                                           : best_slab_edge(d.n_chan, r, d.n_kt, grid);
+    const int forced = policy == PSTGF_SLAB_T32 ? 32 : policy == PSTGF_SLAB_T64 ? 64 : policy == PSTGF_SLAB_T128 ? 128 : 0;
+    const SlabPlan sp = best_slab_plan(d.n_chan, r, d.n_kt, grid, forced);
     d.n_eb = d.n_E / pstgf::EB;
     d.n_eb_coarse = d.n_eb;
     d.slab_e0 = d.n_eb * pstgf::EB;
-    d.slab_T = T;
-    d.slab_nt = (d.n_chan + T - 1) / T;
-    d.slab_g2 = T == 128 ? 0 : r / 2;       // tiles of edge 128 take one energy at a time (8 warps x 16 x 2 blocks)
-    d.slab_g1 = T == 128 ? r : r % 2;
+    d.slab_T = sp.T;
+    d.slab_nt = (d.n_chan + sp.T - 1) / sp.T;
+    d.slab_g4 = sp.g4;
+    d.slab_g2 = sp.g2;
+    d.slab_g1 = sp.g1;
   }
 }
 

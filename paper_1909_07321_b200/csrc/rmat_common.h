@@ -22,7 +22,7 @@
 //                the same result).
 //   slab tiles   the energies that do not fill a block of 8 (n_E mod 8, and every energy of a call with
 //                n_E < 8: PSTGF calls RINIT once per (wave, energy)) are taken in groups
-//                of g = 2 or 1 energies, and the eight consumer warps split the TILE instead of the energy
+//                of g = 4, 2 or 1 energies, and the eight consumer warps split the TILE instead of the energy
 //                block: square tiles S(i, j), j >= i, of edge T = 128, 64 or 32 chosen by the planner so that
 //                there are enough items for the grid; the 8 / g warps of one energy each take a slab of the
 //                tile (SlabShape below).  Same operands, same k order: same bits as inside a block of 8.
@@ -117,12 +117,15 @@ struct SlabShape {
 };
 __host__ __device__ inline SlabShape slab_shape(int T, int g) {
   if (T == 128) return SlabShape{8, 16, 2};                 // g = 1 only: 8 warps x (16 x 2 blocks), the WIDE register tile
-  if (T == 64) return g == 1 ? SlabShape{4, 4, 2} : SlabShape{4, 8, 2};
-  // T == 32: 2 x 2 warps of 2 x 2 blocks for either group size.  With one energy that leaves four of the eight warps
+  if (T == 64) return g == 1 ? SlabShape{4, 4, 2} : g == 2 ? SlabShape{4, 8, 2} : SlabShape{2, 8, 4};
+  // T == 32: 2 x 2 warps of 2 x 2 blocks for one or two energies.  With one energy that leaves four of the eight warps
   // idle, on purpose: 8 warps of 2 x 1 blocks issue 4 LDS.64 per 2 DMMA each, which is all of the SM's shared-memory
-  // bandwidth (ncu: 48 % of its peak at 52 % DMMA utilisation); 2 x 2 blocks need 5 per 4.
-  return SlabShape{2, 2, 2};
+  // bandwidth (ncu: 48 % of its peak at 52 % DMMA utilisation); 2 x 2 blocks need 5 per 4.  Four energies: two warps
+  // of 4 x 2 blocks each.
+  return g == 4 ? SlabShape{2, 4, 2} : SlabShape{2, 2, 2};
 }
+// slab groups of a wave: all of them, and the number of energies in front of group gi
+__host__ __device__ inline int slab_groups(int g4, int g2, int g1) { return g4 + g2 + g1; }
 
 // One partial wave as the kernel sees it.  Built on the host, lives in kernel parameter
 // space (single-wave call) or in the caller's workspace (batch call).
@@ -154,7 +157,7 @@ struct alignas(128) DevWave {
   int ready_counts_channels;   // what rows_ready counts: 0 poles uploaded, 1 channels (rows of a pole-contiguous W)
   int tr;                  // 1: W is channel-contiguous [n_poles][ldw] (H.DAT record order), map box [KT][TR_PITCH]
   int slab_e0;             // first energy handled by slab items (8 n_eb, or n_E when there are none)
-  int slab_g2, slab_g1;    // groups of two energies, then groups of one
+  int slab_g4, slab_g2, slab_g1;   // groups of four energies (the last of them may hold three), then of two, then of one
   int slab_T;              // tile edge of the slab items: 128, 64 or 32
   int slab_nt;             // ceil(n_chan / slab_T): slab tiles = slab_nt (slab_nt + 1) / 2
   int l2_keep;             // W fits half of L2: load it with the evict_last policy so that R's stores do not push it out
@@ -174,7 +177,7 @@ struct alignas(128) DevWave {
   int pair_rb;             // rows of P in the block section: 64 pair_nfb (pair_nfb - 1) / 2, see pair_row_channels
   const unsigned int *pair_nm;   // scratch [n_pairs]: n | m << 16 of every row of P (written by the scratch builder)
 };
-static_assert(sizeof(DevWave) == 640, "DevWave layout (alignas 128; the batch workspace holds an array of these)");
+static_assert(sizeof(DevWave) == 768, "DevWave layout (alignas 128; the batch workspace holds an array of these)");
 
 // Pair form: the items of a wave, section by section.  Section s holds (PT_M >> s)-pair tiles: section 0 the energy
 // tiles [0, pair_nt_coarse) and the first pair_x0 tiles of energy tile pair_nt_coarse; section 1 the rest of that energy

@@ -344,7 +344,7 @@ __device__ __forceinline__ void consume_slab(const ItemInfo &it, Pipe &ps, int w
     nrc[c] = it.col0 + cb * 8 < C ? max(0, min(NR, lim - rb0)) : 0;
     any = any || nrc[c] > 0;
   }
-  if (!any) {
+  if (!any || e_slot >= it.n_valid_e) {                      // nothing wanted, or the empty fourth slot of a group of three
     consume_idle(it.n_kt, ps, lane);
     return;
   }
@@ -534,7 +534,10 @@ __device__ __forceinline__ void consume_item_layout(const ItemInfo &it, Pipe &ps
     const SlabShape sh = slab_shape(it.slab_T, it.slab_g);
     switch (sh.nr) {
       case 16: consume_slab<16, 2, 1, TR>(it, ps, warp, lane, sh.wc); break;
-      case 8: consume_slab<8, 2, 1, TR>(it, ps, warp, lane, sh.wc); break;
+      case 8:
+        if (sh.ncw == 4) consume_slab<8, 4, 1, TR>(it, ps, warp, lane, sh.wc);
+        else consume_slab<8, 2, 1, TR>(it, ps, warp, lane, sh.wc);
+        break;
       case 4: consume_slab<4, 2, 1, TR>(it, ps, warp, lane, sh.wc); break;
       default: consume_slab<2, 2, 1, TR>(it, ps, warp, lane, sh.wc); break;
     }
@@ -766,7 +769,7 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
             const bool sp = single.n_pairs > 0;
             const long long n_coarse = sp ? pair_section_items(single, 0) : (long long)single.n_tiles * single.n_eb_coarse;
             const long long n_slab = sp ? pair_section_items(single, 1)
-                                        : (long long)slab_tiles(single.slab_nt) * (single.slab_g2 + single.slab_g1);
+                                        : (long long)slab_tiles(single.slab_nt) * slab_groups(single.slab_g4, single.slab_g2, single.slab_g1);
             if (item >= n_coarse + n_slab) { sec = 2; item -= n_coarse + n_slab; }
             else if (item >= n_coarse) { sec = 1; item -= n_coarse; }
           }
@@ -787,14 +790,25 @@ rmat_persistent_kernel(const __grid_constant__ DevWave single, const DevWave *__
             e_first = col0;
             n_valid = min(PT_N, w.n_E - col0);
           } else if (sec == 1) {
-            const int n_groups = w.slab_g2 + w.slab_g1;
-            const int tile = (int)(item / n_groups);
-            const int gi = (int)(item - (long long)tile * n_groups);
+            // group-major: all tiles of the first group, then of the next -- the groups of four energies come first, so
+            // the longest items do (largest-first list scheduling)
+            const int n_st = slab_tiles(w.slab_nt);
+            const int gi = (int)(item / n_st);
+            const int tile = (int)(item - (long long)gi * n_st);
             decode_tile_slab(w, tile, kind, row0, col0);
             slab_T = w.slab_T;
-            slab_g = gi < w.slab_g2 ? 2 : 1;
-            e_first = w.slab_e0 + (gi < w.slab_g2 ? 2 * gi : 2 * w.slab_g2 + (gi - w.slab_g2));
-            n_valid = slab_g;
+            // groups of four energies first, then of two, then of one
+            if (gi < w.slab_g4) {
+              slab_g = 4;
+              e_first = w.slab_e0 + 4 * gi;
+            } else if (gi < w.slab_g4 + w.slab_g2) {
+              slab_g = 2;
+              e_first = w.slab_e0 + 4 * w.slab_g4 + 2 * (gi - w.slab_g4);
+            } else {
+              slab_g = 1;
+              e_first = w.slab_e0 + 4 * w.slab_g4 + 2 * w.slab_g2 + (gi - w.slab_g4 - w.slab_g2);
+            }
+            n_valid = min(slab_g, w.n_E - e_first);             // (a group of four may hold three)
           } else {
             const bool fine = sec == 2;
             const int n_eb_sec = fine ? w.n_eb - w.n_eb_coarse : w.n_eb_coarse;
