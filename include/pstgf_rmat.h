@@ -139,16 +139,20 @@ typedef struct {
  *   energies [n_E]           energies, same units and origin as E_k
  *   a                        R-matrix radius r0 in a.u., finite and > 0
  *   R_out    [n_E][n_chan][n_chan]
- * One persistent kernel launch (plus a zero-fill when n_poles == 0); work
+ * One persistent kernel launch (a memset when n_poles == 0; a small scratch-
+ * builder launch ahead of it for a wave in the pair form, see
+ * pstgf_rmat_form_batch; ONE small launch in all for a tiny pair-form wave of
+ * at most 16 channels); work
  * items (energy block, upper-triangle tile) are drawn by the CTAs from an
  * atomic counter.  PSTGF forms R once per (partial wave, energy) (loop over
  * E -> RINIT; one energy per processor at :694): a call
  * with few energies (and the n_E mod 8 energies of any call) is cut into
- * items in which the CTA's eight compute warps share ONE or TWO energies and
- * split the tile instead, so n_E = 1 is a first-class
+ * items in which the CTA's eight compute warps share FOUR, TWO or ONE energies
+ * and split the tile instead, so n_E = 1 is a first-class
  * shape.  The counter lives in a pool of 64 slots (8 KiB of device
- * memory per device, allocated by the library at the first call -- the only
- * device allocation of the DEVICE-pointer calls); when 64 launches are in
+ * memory per device, allocated by the library at the first call -- beside the
+ * pair form's stream-ordered scratch the only device allocation of the
+ * DEVICE-pointer calls); when 64 launches are in
  * flight at once, or `stream` is being captured into a CUDA graph, items are
  * assigned round-robin instead.  Results do not depend on the assignment.
  */
@@ -167,7 +171,7 @@ pstgf_status_t pstgf_rmat_form_hdat(const double *Wt, long long ldw, const doubl
 
 /*
  * Bytes of device workspace pstgf_rmat_form_batch needs for these waves: the
- * tables (a few hundred bytes per wave) plus, for every wave that is done in
+ * tables (about 800 bytes per wave) plus, for every wave that is done in
  * the pair form (n_chan <= 96 with at least 64 energies, see
  * pstgf_rmat_form_batch), 8 * n_poles * (n_chan (n_chan + 1) / 2 + n_E) bytes
  * of scratch.  `waves` is the HOST array that will be passed to the batch call
@@ -177,7 +181,9 @@ pstgf_status_t pstgf_rmat_form_hdat(const double *Wt, long long ldw, const doubl
 size_t pstgf_rmat_batch_workspace_bytes(const pstgf_wave_t *waves, int n_waves);
 
 /*
- * Eq. 4 for every wave of a ragged batch in ONE persistent kernel launch.
+ * Eq. 4 for every wave of a ragged batch in ONE persistent kernel launch (two,
+ * the pair-form waves first, for a batch that mixes pair-form waves with
+ * others; plus their scratch builder).
  * `waves` is a HOST array of n_waves structs with DEVICE pointers.
  * `workspace` is DEVICE memory, 256-byte aligned, at least
  * pstgf_rmat_batch_workspace_bytes() long; it holds the wave table (with one
@@ -270,8 +276,8 @@ pstgf_status_t pstgf_rmat_finalize(void);
 pstgf_status_t pstgf_debug_set_tail_policy(int policy);
 
 /*
- * The n_E mod 8 energies that do not fill a block of 8 are taken two or one at
- * a time by "slab" items whose eight warps split a square tile.
+ * The n_E mod 8 energies that do not fill a block of 8 are taken four, two or
+ * one at a time by "slab" items whose eight warps split a square tile.
  * PSTGF_SLAB_AUTO (default) picks the tile edge (128, 64 or 32) that gives
  * the grid enough items; PSTGF_SLAB_NONE leaves the remainder to a partly
  * idle block of 8 (the round-1 behaviour); _T32/_T64/_T128 force an edge.

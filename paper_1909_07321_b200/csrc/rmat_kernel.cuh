@@ -6,7 +6,9 @@
 // panels; warps 9..11 build the pole scaling d_e[k] = 1/(E_k - E_e) of every
 // stage in shared memory (S1; the denominator of eq. 4).  Warps 0..7 are consumers.  On a classic
 // item each takes one energy of the item's block of 8; on a slab item (the energies that do not fill a block of
-// 8, taken two or one at a time) the warps of one energy split the tile between them.  Either way they contract
+// 8, taken four, two or one at a time) the warps of one energy split the tile between them; on a pair item (a wave
+// with few channels as the GEMM over channel pairs, rmat_common.h) each takes 16 of the item's 128 energies.  Classic
+// and slab items contract
 // acc[n][m] += W[n][k] * (W[m][k] * d_e[k]) on the FP64 tensor pipe (mma.sync m8n8k4 -> DMMA.8x8x4) over
 // upper-triangle tiles only (S3) and write R and its mirror scaled by 1/(2a) (S4).
 // Producer and consumers are coupled by an mbarrier full/empty ring that runs on across item boundaries, so the
@@ -315,7 +317,7 @@ __device__ __forceinline__ void consume_diag(const ItemInfo &it, Pipe &ps, int w
   }
 }
 
-// Slab item: a square tile S(i, j) of edge T for a group of g = 2 or 1 energies.  The 8 / g warps of one energy
+// Slab item: a square tile S(i, j) of edge T for a group of g = 4, 2 or 1 energies.  The 8 / g warps of one energy
 // form a grid of wr x wc warps over the tile (SlabShape); this warp computes row blocks [rb0, rb0 + NR) x column
 // blocks [cb0, cb0 + NCW) of 8 x 8.  The DMMA loop has no predicates: a warp whose slab is cut by the diagonal or by
 // the edge of the matrix computes all of its register tile and stores only what is wanted (nrc[c] row blocks of
@@ -530,19 +532,19 @@ __device__ __forceinline__ void consume_pair(const ItemInfo &it, Pipe &ps, int w
 template <int FAM, bool TR>
 __device__ __forceinline__ void consume_item_layout(const ItemInfo &it, Pipe &ps, int warp, int lane) {
   if constexpr (FAM >= FAM_SLAB) {
-   if (it.slab_T != 0) {
-    const SlabShape sh = slab_shape(it.slab_T, it.slab_g);
-    switch (sh.nr) {
-      case 16: consume_slab<16, 2, 1, TR>(it, ps, warp, lane, sh.wc); break;
-      case 8:
-        if (sh.ncw == 4) consume_slab<8, 4, 1, TR>(it, ps, warp, lane, sh.wc);
-        else consume_slab<8, 2, 1, TR>(it, ps, warp, lane, sh.wc);
-        break;
-      case 4: consume_slab<4, 2, 1, TR>(it, ps, warp, lane, sh.wc); break;
-      default: consume_slab<2, 2, 1, TR>(it, ps, warp, lane, sh.wc); break;
+    if (it.slab_T != 0) {
+      const SlabShape sh = slab_shape(it.slab_T, it.slab_g);
+      switch (sh.nr) {
+        case 16: consume_slab<16, 2, 1, TR>(it, ps, warp, lane, sh.wc); break;
+        case 8:
+          if (sh.ncw == 4) consume_slab<8, 4, 1, TR>(it, ps, warp, lane, sh.wc);
+          else consume_slab<8, 2, 1, TR>(it, ps, warp, lane, sh.wc);
+          break;
+        case 4: consume_slab<4, 2, 1, TR>(it, ps, warp, lane, sh.wc); break;
+        default: consume_slab<2, 2, 1, TR>(it, ps, warp, lane, sh.wc); break;
+      }
+      return;
     }
-    return;
-  }
   }
   if (warp >= it.n_valid_e) {
     consume_idle(it.n_kt, ps, lane);
