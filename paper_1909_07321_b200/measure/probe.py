@@ -21,6 +21,8 @@ def load():
         lib.pstgf_fp64_probe.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_void_p,
                                          ctypes.POINTER(ctypes.c_double), ctypes.c_void_p]
         lib.pstgf_fp64_probe.restype = ctypes.c_int
+        lib.pstgf_i8_probe.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]
+        lib.pstgf_i8_probe.restype = ctypes.c_double
         _lib = lib
     return _lib
 
@@ -39,3 +41,18 @@ def fp64_probe(kind: int, iters: int, blocks: int, threads: int, sink: torch.Ten
     if rc != 0:
         raise RuntimeError(f"pstgf_fp64_probe failed (rc={rc})")
     return float(flop.value)
+
+
+def i8_probe(iters: int, blocks: int, sink: torch.Tensor, stream=None) -> float:
+    """Enqueue the INT8 tensor-pipe probe (tcgen05.mma kind::i8, 128 x 256 x 32, operands resident in shared memory, one
+    CTA per SM); returns the INT8 operations of the launch.  Context for DESIGN.md 11.6, not used by the product."""
+    lib = load()
+    if sink.dtype != torch.int32 or not sink.is_cuda or sink.numel() < blocks:
+        raise ValueError("sink must be a CUDA int32 tensor of at least `blocks` elements")
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    with torch.cuda.device(sink.device):
+        ops = float(lib.pstgf_i8_probe(int(iters), int(blocks), sink.data_ptr(), int(stream.cuda_stream)))
+    if ops < 0:
+        raise RuntimeError("pstgf_i8_probe failed to launch")
+    return ops
