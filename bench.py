@@ -66,6 +66,9 @@ def parse_args():
     ap.add_argument("--scaling", choices=["weak", "strong"], default="weak",
                     help="N > 1 ranks: weak = the configuration with an N times finer mesh (per-rank work fixed, default); "
                          "strong = the configuration as it is, its energy blocks split over the ranks (total work fixed)")
+    ap.add_argument("--probe-i8", action="store_true",
+                    help="also run the INT8 tensor-pipe probe (tcgen05.mma kind::i8, measure/i8_probe.cu) and report its rate "
+                         "under context.int8_tensor_pops: the number behind DESIGN.md 11.6, not a path of the library")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
@@ -512,6 +515,19 @@ def run_cuda(args):
             torch.cuda.synchronize()
             best_ms = min(best_ms, e0.elapsed_time(e1))
         probe["dmma_dependent_latency_clk"] = best_ms * 1e-3 * peaks["sm_max_mhz"] * 1e6 / (it_chain * 32)
+    context = None
+    if rank == 0 and args.probe_i8:
+        isink = torch.zeros(sms, dtype=torch.int32, device="cuda")
+        best = 0.0
+        for _ in range(4):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            ops = probe_lib.i8_probe(4000, sms, isink)
+            e1.record()
+            torch.cuda.synchronize()
+            best = max(best, ops / (e0.elapsed_time(e1) * 1e-3) / 1e15)
+        context = {"int8_tensor_pops": best, "kind": "tcgen05.mma.cta_group::1.kind::i8 128x256x32, operands in shared memory, "
+                                                        "accumulators in TMEM, one CTA per SM (burst, best of 4)"}
     # Peak: the FP64 tensor (DMMA) rate measured live by the probe above (burst, this kernel is timed alone);
     # MEASURED_PEAKS.json has no FP64 entry.  The guide's rule (another dtype's measured peak x nominal ratio)
     # gives a LOWER figure because the bf16 measurement is power-limited (1335 MHz) while FP64 runs at 1965 MHz;
@@ -593,7 +609,7 @@ def run_cuda(args):
                         "sha256": wl_job.sha256()[:16]},
                 "tflops_counted": wl_job.counted_flop() * args.steps / (total_ms_max * 1e-3) / 1e12,
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,
-                **({"prior_art": prior} if prior else {}),
+                **({"prior_art": prior} if prior else {}), **({"context": context} if context else {}),
                 "clocks": clocks, "wall_s_timed_region": wall, "step_ms_min_max": [min(step_ms), max(step_ms)]}
         print(json.dumps(line), flush=True)
     if world > 1:

@@ -124,6 +124,7 @@ def test_product_library_holds_no_measurement_code(lib):
     assert not hasattr(lib, "pstgf_fp64_probe")
     from paper_1909_07321_b200 import build
     assert hasattr(ctypes.CDLL(build.PROBE_LIB), "pstgf_fp64_probe")
+    assert hasattr(ctypes.CDLL(build.PROBE_LIB), "pstgf_i8_probe") and not hasattr(lib, "pstgf_i8_probe")
 
 
 def test_mesh_from_zscaled(lib):

@@ -990,3 +990,23 @@ def test_paper_scale_wave_sampled(rmat, oracle):
     num = (Rs - Rn).abs().flatten(1).max(dim=1).values
     den = Rn.abs().flatten(1).max(dim=1).values
     assert float((num / den).max()) <= TOL_TIGHT
+
+
+def test_measurement_probes_run():
+    """The bench-side probes (libpstgf_probe.so, not the product): the FP64 pipe probes behind the roofline denominator
+    and the INT8 tensor-pipe probe (tcgen05.mma kind::i8 with TMEM accumulators) behind DESIGN.md 11.6 launch, finish
+    and report the operations they performed."""
+    from paper_1909_07321_b200.measure import probe
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    sink = torch.empty(sms * 4 * 256, dtype=torch.float64, device="cuda")
+    for kind in (0, 1, 2):
+        assert probe.fp64_probe(kind, 10, sms * 2, 256, sink) > 0
+    isink = torch.zeros(sms, dtype=torch.int32, device="cuda")
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    probe.i8_probe(50, sms, isink)
+    e0.record()
+    ops = probe.i8_probe(2000, sms, isink)
+    e1.record()
+    torch.cuda.synchronize()
+    assert ops == 2.0 * 128 * 256 * 32 * 8 * 2000 * sms
+    assert ops / (e0.elapsed_time(e1) * 1e-3) > 1e15          # above 1 POP/s: the tensor pipe, not an emulation
