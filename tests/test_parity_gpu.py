@@ -716,7 +716,9 @@ def test_host_call_signalled_pipeline(rmat, oracle):
 def test_random_shapes_layouts_policies(rmat, tail_policy):
     """Seeded fuzz: random batches of 1-4 waves with random shapes (n_chan 1..700), leading dimensions, memory
     orders of W and scheduling policies, single-wave or batch call, every energy against the term-by-term device
-    kernel (itself checked against the oracle above).  The bound is 1e-12 rather than 1e-13 because a wave with
+    kernel (itself checked against the oracle above).  The draw covers every item family: classic and slab items,
+    pair-form waves (n_chan <= 96 with >= 64 energies: about one wave in six), tiny waves through the one-launch kernel,
+    mixed batches that go out as two launches.  The bound is 1e-12 rather than 1e-13 because a wave with
     one or two channels has no large diagonal to normalise by: cancellation in a single sum shows directly."""
     from paper_1909_07321_b200 import inputs
     rng = np.random.default_rng(20260101)
