@@ -66,6 +66,11 @@ def parse_args():
     ap.add_argument("--scaling", choices=["weak", "strong"], default="weak",
                     help="N > 1 ranks: weak = the configuration with an N times finer mesh (per-rank work fixed, default); "
                          "strong = the configuration as it is, its energy blocks split over the ranks (total work fixed)")
+    ap.add_argument("--variant", choices=["dmma", "sliced"], default="dmma",
+                    help="dmma: the library's path (default).  sliced: pstgf_rmat_form_sliced, the INT8 tcgen05 VARIANT of "
+                         "SURVEY.md 8f-4 (single-wave configs only; results agree with FP64 sums to ~1e-12, see the header); "
+                         "a comparison line, not the product's number")
+    ap.add_argument("--slices", type=int, default=7, help="digits per element for --variant sliced (7: ~1e-12, 8: ~1e-14)")
     ap.add_argument("--probe-i8", action="store_true",
                     help="also run the INT8 tensor-pipe probe (tcgen05.mma kind::i8, measure/i8_probe.cu) and report its rate "
                          "under context.int8_tensor_pops: the number behind DESIGN.md 11.6, not a path of the library")
@@ -438,7 +443,19 @@ def run_cuda(args):
         ws = torch.empty(rmat.pstgf_rmat_batch_workspace_bytes(arr), dtype=torch.uint8, device="cuda")
     flush_buf = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
 
+    sliced = args.variant == "sliced"
+    if sliced:
+        if not single or hdat:
+            raise SystemExit("--variant sliced: single-wave configs with pole-contiguous W only")
+        w0 = wl.waves[0]
+        sliced_ws = torch.empty(int(rmat.load().pstgf_rmat_sliced_workspace_bytes(w0.n_chan, w0.n_poles, w0.n_E, args.slices)),
+                                dtype=torch.uint8, device="cuda")
+
     def step():
+        if sliced:
+            W, E_k, en, a, R, _ = dev_waves[0]
+            rmat.pstgf_rmat_form_sliced(W, E_k, en, a, n_slices=args.slices, R_out=R, workspace=sliced_ws)
+            return 1 + 2 * -(-w0.n_E // max(1, min(w0.n_E, (1 << 30) // (args.slices * (-(-w0.n_chan // 128) * 128) * (-(-w0.n_poles // 64) * 64)))))
         if single:
             W, E_k, en, a, R, _ = dev_waves[0]
             (rmat.pstgf_rmat_form_hdat if hdat else rmat.pstgf_rmat_form)(W, E_k, en, a, R_out=R)
@@ -543,18 +560,18 @@ def run_cuda(args):
     roofline = {"bound": "tensor", "achieved": achieved_tflops, "peak": peak, "unit": "TFLOP/s",
                 "frac": achieved_tflops / peak, "traffic": None, "peak_source": peak_source,
                 "peak_rule_bf16_x_ratio": peak_rule, "peak_nominal_fp64": peak_nominal,
-                "kernel": "rmat_persistent_kernel", "flop_per_launch": flop,
+                "kernel": "rmat_persistent_kernel" if not sliced else "slice_kernel + sliced_gemm_kernel (variant)", "flop_per_launch": flop,
                 "t_roof_ms": 1e3 * max(t_fp64, t_hbm), "hbm_write_gbs": wl.r_bytes() / (kern_ms * 1e-3) / 1e9,
                 "hbm_peak_gbs": peaks["hbm_gbs"]}
     if probe:
         roofline["fp64_probe_tflops"] = probe
-    roofline["traffic"] = ncu_traffic(args.config) if not args.n_E else None
+    roofline["traffic"] = ncu_traffic(args.config) if not (args.n_E or sliced) else None
     roofline["traffic_source"] = ("committed ncu --set full capture (profiles/traffic.csv): DRAM bytes read + written "
                                   "per launch; not measured in this run") if roofline["traffic"] is not None else None
 
     # ---- end to end: HOST buffers through the C ABI, copies inside the timed region ----
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not sliced:
         host = []
         for w in wl.waves:
             hW = torch.from_numpy(np.ascontiguousarray(w.W.T) if hdat else w.W).pin_memory()
@@ -606,6 +623,7 @@ def run_cuda(args):
                 "config": job_description,           # the same dict as --impl reference prints
                 "run": {"n_energies_per_rank": n_e, "l2": "flushed between timed steps (512 MiB write)",
                         "w_layout": args.w_layout, "tail_policy": args.tail_policy, "slab_policy": args.slab_policy,
+                        "variant": args.variant if not sliced else f"sliced (INT8 tcgen05, {args.slices} slices): NOT the product's path",
                         "sha256": wl_job.sha256()[:16]},
                 "tflops_counted": wl_job.counted_flop() * args.steps / (total_ms_max * 1e-3) / 1e12,
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,

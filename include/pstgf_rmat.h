@@ -215,6 +215,22 @@ pstgf_status_t pstgf_rmat_form_batch(const pstgf_wave_t *waves, int n_waves, voi
 pstgf_status_t pstgf_rmat_form_naive(const pstgf_wave_t *wave, void *stream);
 
 /*
+ * VARIANT, never chosen by the calls above: eq. 4 for ONE wave (HOST struct, DEVICE pointers, pole-contiguous W)
+ * evaluated on the INT8 tensor pipe (tcgen05.mma kind::i8, INT32 accumulators in tensor memory) instead of the FP64
+ * tensor pipe, by slicing W and W diag(1/(E_k - E_e)) into n_slices signed 7-bit digits per element with one
+ * power-of-two scale per row and summing the n_slices (n_slices + 1) / 2 leading digit products exactly (SURVEY.md
+ * 8f-4).  The result is NOT an IEEE FP64 sum of the terms of eq. 4: it agrees with one to about
+ * 1e-12 of max|R| per energy with 7 slices and 1e-14 with 8 (6 miss north_star's 1e-11); both triangles are written
+ * and bitwise equal, diag_add is honoured.  n_slices in [2, 8]; n_poles * n_slices < 2^19 (INT32 accumulators).
+ * `workspace` is DEVICE memory, 256-byte aligned, of pstgf_rmat_sliced_workspace_bytes() (the digit arrays: n_slices
+ * bytes per element of W, once for W and once per energy of a chunk of at most 1 GiB).  Asynchronous on `stream`;
+ * measured slower than pstgf_rmat_form on this chip, provided for comparison.
+ */
+size_t pstgf_rmat_sliced_workspace_bytes(int n_chan, int n_poles, int n_E, int n_slices);
+pstgf_status_t pstgf_rmat_form_sliced(const pstgf_wave_t *wave, int n_slices, void *workspace, size_t workspace_bytes,
+                                      void *stream);
+
+/*
  * End-to-end convenience over HOST buffers: `waves` holds HOST pointers
  * (pinned memory recommended; pageable memory works but copies synchronously).
  * Inputs are copied to the device on `stream`, R is formed on streams of the

@@ -10,13 +10,13 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libpstgf_rmat.so")
-SOURCES = [os.path.join(CSRC, "pstgf_rmat.cu"), os.path.join(CSRC, "rmat_launch.cu"), os.path.join(CSRC, "rmat_small.cu")]
+SOURCES = [os.path.join(CSRC, "pstgf_rmat.cu"), os.path.join(CSRC, "rmat_launch.cu"), os.path.join(CSRC, "rmat_small.cu"), os.path.join(CSRC, "rmat_sliced.cu")]
 HEADERS = [os.path.join(CSRC, "rmat_common.h"), os.path.join(CSRC, "rmat_kernel.cuh"), os.path.join(CSRC, "rmat_aux.cuh"), os.path.join(CSRC, "rmat_launch.h"),
            os.path.join(os.path.dirname(_HERE), "include", "pstgf_rmat.h")]
 # translation units of libpstgf_rmat.so: (source, extra flags).  The persistent kernel is compiled once per item
 # family set (csrc/rmat_launch.h), each in its own unit so that the units build side by side.
 UNITS = [(SOURCES[0], []), (SOURCES[1], ["-DPSTGF_FAM=0"]), (SOURCES[1], ["-DPSTGF_FAM=1"]), (SOURCES[1], ["-DPSTGF_FAM=2"]),
-         (SOURCES[2], [])]
+         (SOURCES[2], []), (SOURCES[3], [])]
 PROBE_LIB = os.path.join(_HERE, "libpstgf_probe.so")
 PROBE_SOURCES = [os.path.join(_HERE, "measure", "fp64_probe.cu"), os.path.join(_HERE, "measure", "i8_probe.cu")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -24,7 +24,7 @@ PSTGF_ERR_TIMEOUT, PSTGF_ERR_CAPTURE = 6, 7
 PSTGF_RMAT_VERSION = 200            # must equal include/pstgf_rmat.h; load() checks it against the library
 
 EXPORTS = ["pstgf_rmat_form", "pstgf_rmat_form_hdat", "pstgf_rmat_batch_workspace_bytes", "pstgf_rmat_form_batch",
-           "pstgf_rmat_form_naive", "pstgf_rmat_form_batch_host", "pstgf_mesh_from_zscaled", "pstgf_rmat_finalize",
+           "pstgf_rmat_form_naive", "pstgf_rmat_form_sliced", "pstgf_rmat_sliced_workspace_bytes", "pstgf_rmat_form_batch_host", "pstgf_mesh_from_zscaled", "pstgf_rmat_finalize",
            "pstgf_debug_set_tail_policy", "pstgf_debug_set_slab_policy", "pstgf_debug_set_pair_policy", "pstgf_debug_set_small_policy",
            "pstgf_debug_set_host_pipeline",
            "pstgf_debug_set_upload_timeout_ms", "pstgf_debug_stall_upload", "pstgf_last_launch_count",
@@ -76,6 +76,10 @@ def load(build_if_missing: bool = False):
     lib.pstgf_rmat_form_hdat.restype = i
     lib.pstgf_rmat_form_naive.argtypes = [ctypes.POINTER(pstgf_wave_t), vp]
     lib.pstgf_rmat_form_naive.restype = i
+    lib.pstgf_rmat_form_sliced.argtypes = [ctypes.POINTER(pstgf_wave_t), i, vp, sz, vp]
+    lib.pstgf_rmat_form_sliced.restype = i
+    lib.pstgf_rmat_sliced_workspace_bytes.argtypes = [i, i, i, i]
+    lib.pstgf_rmat_sliced_workspace_bytes.restype = sz
     lib.pstgf_rmat_batch_workspace_bytes.argtypes = [ctypes.POINTER(pstgf_wave_t), i]
     lib.pstgf_rmat_batch_workspace_bytes.restype = sz
     lib.pstgf_rmat_form_batch.argtypes = [ctypes.POINTER(pstgf_wave_t), i, vp, sz, vp]
@@ -189,6 +193,21 @@ def pstgf_rmat_form_naive(W, E_k, energies, a: float, R_out=None, stream=None,
     w = _wave_struct(W, E_k, energies, a, R_out, layout, diag_add)
     with torch.cuda.device(W.device):
         _check(lib.pstgf_rmat_form_naive(ctypes.byref(w), _stream_ptr(stream)))
+    return R_out
+
+
+def pstgf_rmat_form_sliced(W, E_k, energies, a: float, n_slices: int = 7, R_out=None, workspace=None, stream=None,
+                           diag_add=None) -> torch.Tensor:
+    """The INT8-sliced VARIANT of eq. 4 (tcgen05.mma kind::i8; not an IEEE FP64 sum, see the header); pole-contiguous W."""
+    lib = load()
+    if R_out is None:
+        R_out = torch.empty((energies.shape[0], W.shape[0], W.shape[0]), dtype=torch.float64, device=W.device)
+    w = _wave_struct(W, E_k, energies, a, R_out, PSTGF_W_POLE_CONTIGUOUS, diag_add)
+    need = int(lib.pstgf_rmat_sliced_workspace_bytes(w.n_chan, w.n_poles, w.n_E, int(n_slices)))
+    if workspace is None:
+        workspace = torch.empty(max(need, 1024), dtype=torch.uint8, device=W.device)
+    with torch.cuda.device(W.device):
+        _check(lib.pstgf_rmat_form_sliced(ctypes.byref(w), int(n_slices), workspace.data_ptr(), workspace.numel(), _stream_ptr(stream)))
     return R_out
 
 

@@ -1012,3 +1012,52 @@ def test_measurement_probes_run():
     torch.cuda.synchronize()
     assert ops == 2.0 * 128 * 256 * 32 * 8 * 2000 * sms
     assert ops / (e0.elapsed_time(e1) * 1e-3) > 1e15          # above 1 POP/s: the tensor pipe, not an emulation
+
+
+SLICED_SHAPES = [(1, 5, 1, 7), (8, 64, 2, 7), (64, 128, 3, 7), (130, 300, 5, 7), (200, 777, 4, 7), (257, 513, 3, 7), (64, 1280, 9, 8),
+                 (129, 2050, 2, 8)]
+
+
+@pytest.mark.parametrize("C,K,N,S", SLICED_SHAPES)
+def test_sliced_variant_matches_the_oracle(rmat, oracle, C, K, N, S):
+    """pstgf_rmat_form_sliced (SURVEY.md 8f-4): eq. 4 on the INT8 tensor pipe (tcgen05.mma kind::i8, TMEM accumulators)
+    from signed 7-bit digits of W and W diag(1/(E_k - E)).  Not an IEEE FP64 sum: the bound is north_star's 1e-11 per
+    energy (measured ~2e-13 with 7 slices, ~4e-15 with 8), asserted at 5e-12 / 1e-13; both triangles bitwise equal; the
+    diagonal addend honoured exactly; several row tiles, ragged tiles in both directions, poles not a multiple of 64."""
+    from paper_1909_07321_b200 import inputs
+    w = inputs.make_wave(15000 + 7 * C + N, C, K, N)
+    da = np.random.default_rng(C + K).normal(0.0, 0.05, (N, C))
+    Wd, Ek, en = _dev(w.W), _dev(w.E_k), _dev(w.energies)
+    R = rmat.pstgf_rmat_form_sliced(Wd, Ek, en, w.a, n_slices=S)
+    Rd = rmat.pstgf_rmat_form_sliced(Wd, Ek, en, w.a, n_slices=S, diag_add=_dev(da))
+    torch.cuda.synchronize()
+    R, Rd = R.cpu().numpy(), Rd.cpu().numpy()
+    ref = oracle.rmat_form(w.W, w.E_k, w.energies, w.a, threads=_threads())
+    err = _rel_err_per_energy(R, ref)
+    assert err.max() <= (5e-12 if S == 7 else 1e-13), err.max()
+    assert np.array_equal(R, R.transpose(0, 2, 1))
+    idx, off = np.arange(C), ~np.eye(C, dtype=bool)
+    assert np.array_equal(Rd[:, off], R[:, off]) and np.array_equal(Rd[:, idx, idx], R[:, idx, idx] + da)
+
+
+def test_sliced_variant_config2_and_errors(rmat, oracle):
+    """Config 2 through the sliced variant on sampled energies (the one nearest a pole included), six slices missing
+    1e-11 as DESIGN.md 11.6 says, and the argument errors of the call."""
+    from paper_1909_07321_b200 import inputs
+    w = inputs.make_config(2).waves[0]
+    idx = inputs.sample_energy_indices(w)
+    Wd, Ek = _dev(w.W), _dev(w.E_k)
+    ref = oracle.rmat_form(w.W, w.E_k, w.energies[idx], w.a, threads=_threads())
+    errs = {}
+    for S in (6, 7, 8):
+        R = rmat.pstgf_rmat_form_sliced(Wd, Ek, _dev(w.energies[idx]), w.a, n_slices=S)
+        torch.cuda.synchronize()
+        errs[S] = float(_rel_err_per_energy(R.cpu().numpy(), ref).max())
+    assert errs[8] <= 1e-13 and errs[7] <= 5e-12 and errs[6] > errs[7] > errs[8], errs
+    lib = rmat.load()
+    one = rmat.make_wave_array([(Wd, Ek, _dev(w.energies[idx]), w.a, torch.empty((len(idx), 64, 64), dtype=torch.float64, device="cuda"))])
+    ws = torch.empty(1 << 20, dtype=torch.uint8, device="cuda")
+    assert lib.pstgf_rmat_form_sliced(one, 7, ws.data_ptr(), ws.numel(), None) == 3          # workspace too small
+    assert lib.pstgf_rmat_form_sliced(one, 9, ws.data_ptr(), ws.numel(), None) == 1          # n_slices out of range
+    assert lib.pstgf_rmat_form_sliced(None, 7, ws.data_ptr(), ws.numel(), None) == 1
+    assert lib.pstgf_rmat_sliced_workspace_bytes(64, 1280, 8, 7) > 0 and lib.pstgf_rmat_sliced_workspace_bytes(64, 1280, 8, 1) == 0
