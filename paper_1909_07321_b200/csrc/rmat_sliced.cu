@@ -391,9 +391,10 @@ pstgf_status_t pstgf_rmat_form_sliced(const pstgf_wave_t *wave, int n_slices, vo
   if (!encode_bytes_map(&mapA, dA, (long long)S * L.Cp, L.Kp, TILE_M) ||
       !encode_bytes_map(&mapB, dB, (long long)L.chunk * S * L.Cp, L.Kp, TILE_N))
     return PSTGF_ERR_CUDA;
-  // the slicing kernel keeps a row in shared memory between its two passes when it fits
+  // the slicing kernel keeps a row in shared memory between its two passes when that does not cost occupancy (a row of
+  // config 5 is 80 KB: two blocks per SM, measured 12.6 ms per step against 8.8 ms with the divisions done twice)
   const size_t row_bytes = sizeof(double) * (size_t)w.n_poles;
-  const bool cache = row_bytes <= 200 * 1024;
+  const bool cache = row_bytes <= 16 * 1024;
   if (cache && cudaFuncSetAttribute(slice_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)row_bytes) != cudaSuccess) return PSTGF_ERR_CUDA;
   auto slice = [&](dim3 grid, const double *Ek, const double *en, int8_t *digits, double *scales) {
     if (cache) slice_kernel<true><<<grid, 256, row_bytes, s>>>(w.W, w.ldw, Ek, en, w.n_chan, w.n_poles, S, L.Cp, L.Kp, digits, scales);

@@ -196,6 +196,10 @@ def pstgf_rmat_form_naive(W, E_k, energies, a: float, R_out=None, stream=None,
     return R_out
 
 
+def pstgf_rmat_sliced_workspace_bytes(n_chan: int, n_poles: int, n_E: int, n_slices: int = 7) -> int:
+    return int(load().pstgf_rmat_sliced_workspace_bytes(int(n_chan), int(n_poles), int(n_E), int(n_slices)))
+
+
 def pstgf_rmat_form_sliced(W, E_k, energies, a: float, n_slices: int = 7, R_out=None, workspace=None, stream=None,
                            diag_add=None) -> torch.Tensor:
     """The INT8-sliced VARIANT of eq. 4 (tcgen05.mma kind::i8; not an IEEE FP64 sum, see the header); pole-contiguous W."""
