@@ -71,7 +71,7 @@
 extern "C" {
 #endif
 
-#define PSTGF_RMAT_VERSION 200 /* major*100 + minor; 2.x: pstgf_wave_t grew diag_add (72 bytes) */
+#define PSTGF_RMAT_VERSION 201 /* major*100 + minor; 2.x: pstgf_wave_t grew diag_add (72 bytes); 2.01: pstgf_rmat_form_static */
 
 typedef enum {
   PSTGF_OK = 0,
@@ -81,7 +81,8 @@ typedef enum {
   PSTGF_ERR_UNSUPPORTED_DEVICE = 4, /* no CUDA device, or the current device is not compute capability 10.x */
   PSTGF_ERR_CUDA = 5,               /* a CUDA runtime/driver call failed; see pstgf_last_cuda_error() */
   PSTGF_ERR_TIMEOUT = 6,            /* pstgf_rmat_form_batch_host: the launch gave up waiting for an upload of W; R_out undefined */
-  PSTGF_ERR_CAPTURE = 7             /* the stream is being captured and this call cannot be (see above) */
+  PSTGF_ERR_CAPTURE = 7,            /* the stream is being captured and this call cannot be (see above) */
+  PSTGF_ERR_STATIC_LIMIT = 8        /* pstgf_rmat_form_static: the wave needs more scratch than PSTGF_STATIC_SCRATCH_BYTES */
 } pstgf_status_t;
 
 /*
@@ -168,6 +169,54 @@ pstgf_status_t pstgf_rmat_form(const double *W, long long ldw, const double *E_k
 pstgf_status_t pstgf_rmat_form_hdat(const double *Wt, long long ldw, const double *E_k,
                                     const double *energies, int n_chan, int n_poles, int n_E,
                                     double a, double *R_out, void *stream);
+
+/*
+ * pstgf_rmat_form for callers that cannot allocate device memory.
+ *
+ * Who that is: code running where a cudaMalloc / cudaFree is forbidden or harmful.  A process whose device memory
+ * is handed out in full at start-up to one arena (a framework's caching allocator, a job that several MPI ranks
+ * share one GPU for -- PSTGF's own set-up, Fig. 2 -- each with a fixed slice) has nothing left for a
+ * library to take, and a failed allocation deep inside a formation is an error the caller cannot plan for.  A
+ * latency-bound loop of one RINIT call per energy cannot afford cudaMalloc / cudaFree either:
+ * both may synchronise the whole device.  And a host thread that already holds its framework's allocator lock, or
+ * runs as a stream callback, must not enter the CUDA allocator at all.  pstgf_rmat_form does allocate: its work
+ * counters come from cudaMalloc at the first call, the pair form's P and D from a memory pool at every call.
+ *
+ * This call allocates nothing, frees nothing and creates no pool or event.  Its scratch is a fixed array of
+ * PSTGF_STATIC_SCRATCH_BYTES (16 MiB) compiled into the library's device image: EVERY GPU on which a process uses
+ * libpstgf_rmat.so gives up that much memory from the moment the library's module is loaded until the process
+ * exits, whether this call is ever made or not.  That is the price, and the reason the array is modest.
+ *
+ * Arguments, layout, alignment rules, planning and kernels are those of pstgf_rmat_form; so are the bits of
+ * R_out (the tests compare the two calls bitwise).  DEVICE: W, E_k, energies, R_out -- all the caller's.
+ *
+ * Limit.  A wave that goes the pair form (n_chan <= 96 and n_E >= 64, unless it is tiny enough for the
+ * one-launch kernel) needs 8 * ld * (n_chan (n_chan + 1) / 2 + n_E) bytes, ld = n_poles rounded up to even, plus
+ * 4 bytes per channel pair, each of the three parts rounded up to 256 bytes; that must fit in
+ * PSTGF_STATIC_SCRATCH_BYTES - 256.  E.g. 24 x 480 with 2000 energies (8.8 MB) fits, BASELINE.json's 64 x 1280 x 4096
+ * (63 MB) does not.  A larger wave is refused with PSTGF_ERR_STATIC_LIMIT before anything is enqueued and R_out
+ * is untouched; nothing is cut down silently.  (pstgf_debug_set_pair_policy(PSTGF_PAIRS_NONE) sends such a wave
+ * through the symmetric form, which needs no scratch; a few ulp apart, see there.)  Waves in the symmetric form
+ * use only the 16-byte work counter and are accepted at any size.
+ *
+ * First call on a device.  It asks the runtime once for the array's device address (cudaGetSymbolAddress, with the
+ * caller's current device current; the result is remembered per device) and, like every call of this library,
+ * raises the kernels' shared-memory limit once.  Make that first call on each device ahead of time, outside any
+ * stream capture; later calls only enqueue: one 16-byte memset of the work counter when the launch has more items
+ * than CTAs, the scratch builder for a pair-form wave, the persistent kernel.  pstgf_last_launch_count() counts
+ * the memset as one.
+ *
+ * Sharing.  There is ONE array per device and every call of pstgf_rmat_form_static on that device uses it, from
+ * any thread and on any stream.  Two calls whose kernels can run on the GPU at the same time (different streams
+ * without an event between them, or two host threads) overwrite each other's P, D and counter: wrong R, no error.
+ * Keep such calls on one stream, or order them with events.  The array keeps the previous call's contents; the
+ * call clears the counter and rewrites every scratch element it later reads, so nothing carries over into R.
+ * pstgf_rmat_finalize neither frees nor resets the array (there is nothing to free).
+ */
+#define PSTGF_STATIC_SCRATCH_BYTES 16777216
+pstgf_status_t pstgf_rmat_form_static(const double *W, long long ldw, const double *E_k,
+                                      const double *energies, int n_chan, int n_poles, int n_E,
+                                      double a, double *R_out, void *stream);
 
 /*
  * Bytes of device workspace pstgf_rmat_form_batch needs for these waves: the

@@ -774,6 +774,37 @@ int acquire_counter(int dev, cudaStream_t s, unsigned long long **out) {
   return -1;
 }
 
+// ---- library-resident scratch of pstgf_rmat_form_static ------------------------------------------
+// pstgf_rmat_form_static (include/pstgf_rmat.h) is the single-wave call for callers that must not allocate device
+// memory.  What pstgf_rmat_form takes from cudaMalloc (the work-counter pool) and from cudaMallocFromPoolAsync (P, D and
+// the pair table of a pair-form wave) lives here instead: one array of PSTGF_STATIC_SCRATCH_BYTES that is part of the
+// module's image, so every device that loads libpstgf_rmat.so carries it from module load to process exit, used or not.
+//   [0, 256)                               the launch's work counter (two words used)
+//   [256, PSTGF_STATIC_SCRATCH_BYTES)      pair-form scratch, laid out by plan_pairs as in the other calls
+// In host code `g_static_scratch` is only a handle for the runtime (a host-side shadow symbol), never a device
+// address: the device address is asked for once per device with cudaGetSymbolAddress and that is what kernels get.
+}  // namespace
+static __device__ __align__(256) unsigned char g_static_scratch[PSTGF_STATIC_SCRATCH_BYTES];
+namespace {
+constexpr size_t STATIC_COUNTER_BYTES = 256;
+std::mutex g_static_mutex;
+unsigned char *g_static_addr[64] = {nullptr};
+
+// Device address of g_static_scratch on device `dev`, which must be the CURRENT device (cudaGetSymbolAddress answers
+// for the current device's copy of the module).  Looked up at the first call per device, remembered afterwards.
+pstgf_status_t static_scratch_address(int dev, unsigned char **out) {
+  if (dev < 0 || dev >= 64) return PSTGF_ERR_UNSUPPORTED_DEVICE;
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  if (!g_static_addr[dev]) {
+    void *p = nullptr;
+    PSTGF_CUDA(cudaGetSymbolAddress(&p, g_static_scratch));
+    if (!p || (reinterpret_cast<uintptr_t>(p) & 255u) != 0) return PSTGF_ERR_CUDA;
+    g_static_addr[dev] = static_cast<unsigned char *>(p);
+  }
+  *out = g_static_addr[dev];
+  return PSTGF_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -880,6 +911,71 @@ pstgf_status_t pstgf_rmat_form_hdat(const double *Wt, long long ldw, const doubl
                                     int n_chan, int n_poles, int n_E, double a, double *R_out, void *stream) {
   pstgf_wave_t w{n_chan, n_poles, n_E, PSTGF_W_CHANNEL_CONTIGUOUS, ldw, a, Wt, E_k, energies, R_out, nullptr};
   return form_single(w, stream);
+}
+
+// pstgf_rmat_form without any device allocation: the same plan, the same kernels and therefore the same bits, with
+// the scratch and the work counter in g_static_scratch.  No cudaMalloc*, cudaFree*, memory pool or event is touched.
+pstgf_status_t pstgf_rmat_form_static(const double *W, long long ldw, const double *E_k, const double *energies,
+                                      int n_chan, int n_poles, int n_E, double a, double *R_out, void *stream) {
+  const pstgf_wave_t w{n_chan, n_poles, n_E, PSTGF_W_POLE_CONTIGUOUS, ldw, a, W, E_k, energies, R_out, nullptr};
+  tl_launches = 0;
+  pstgf_status_t st = check_wave(w);
+  if (st != PSTGF_OK) return st;
+  if (n_chan == 0 || n_E == 0) return PSTGF_OK;
+  const bool pair = wants_pair_form(n_chan, n_poles, n_E);
+  const bool small = pair && wants_small_kernel(n_chan, n_poles, n_E);      // one launch, no scratch at all
+  // the size check needs no device: too large a wave is refused before any CUDA call
+  if (pair && !small && pair_scratch_bytes(n_chan, n_poles, n_E) > (size_t)PSTGF_STATIC_SCRATCH_BYTES - STATIC_COUNTER_BYTES)
+    return PSTGF_ERR_STATIC_LIMIT;
+  DeviceState ds;
+  st = device_state(ds);
+  if (st != PSTGF_OK) return st;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  if (n_poles == 0) return zero_fill(w, s);
+  std::vector<DevWave> d(1);
+  plan_wave(w, d[0], ds.l2_bytes);
+  if (small) {
+    PSTGF_CUDA(pstgf::small_launch(d[0], s));
+    tl_launches = 1;
+    return PSTGF_OK;
+  }
+  unsigned char *base = nullptr;
+  st = static_scratch_address(ds.device, &base);       // the first call on this device looks the address up
+  if (st != PSTGF_OK) return st;
+  int launches = 0;
+  if (pair) {
+    // P, D and the pair table are written in full by the builder before the GEMM items read them, so what the last
+    // call left in the array does not matter
+    plan_pairs(d[0], base + STATIC_COUNTER_BYTES);
+    plan_pair_tails(d, ds.sm_count);
+    st = encode_pair_maps(d[0]);
+    if (st != PSTGF_OK) return st;
+    const int rows = d[0].n_E + d[0].n_pairs;
+    const int chunks = (rows + pstgf::PAIR_BUILD_ROWS - 1) / pstgf::PAIR_BUILD_ROWS;
+    pstgf::pair_build_kernel<false><<<dim3((unsigned)std::min(chunks, 8 * ds.sm_count), 1), 256, 0, s>>>(d[0], nullptr, 1);
+    PSTGF_CUDA(cudaGetLastError());
+    ++launches;
+  } else {
+    plan_slabs(d, ds.sm_count);
+    plan_tails(d, ds.sm_count);
+    st = encode_map(d[0]);
+    if (st != PSTGF_OK) return st;
+  }
+  const long long n_items = wave_items(d[0]);
+  const int grid = (int)std::min<long long>(ds.sm_count, n_items);
+  const pstgf::RingGeo geo = ring_geometry(d);
+  unsigned long long *counter = nullptr;
+  if (n_items > grid) {
+    // the work counter must start at zero: cleared on the stream ahead of every launch (a launch that ran to its end
+    // leaves it zeroed, one that was cut short does not)
+    counter = reinterpret_cast<unsigned long long *>(base);
+    PSTGF_CUDA(cudaMemsetAsync(counter, 0, 2 * sizeof(unsigned long long), s));
+    ++launches;
+  }
+  pstgf::PersistentArgs pa{&d[0], nullptr, nullptr, 1, n_items, counter, geo, grid};
+  PSTGF_CUDA(pstgf::persistent_launch_family(launch_family(d), false, pa, s));
+  tl_launches = launches + 1;
+  return PSTGF_OK;
 }
 
 size_t pstgf_rmat_batch_workspace_bytes(const pstgf_wave_t *waves, int n_waves) {
@@ -1599,6 +1695,7 @@ const char *pstgf_status_string(pstgf_status_t status) {
     case PSTGF_ERR_CUDA: return "PSTGF_ERR_CUDA: a CUDA call failed, see pstgf_last_cuda_error()";
     case PSTGF_ERR_TIMEOUT: return "PSTGF_ERR_TIMEOUT: the launch gave up waiting for an upload of W; R_out is undefined";
     case PSTGF_ERR_CAPTURE: return "PSTGF_ERR_CAPTURE: this call cannot be captured into a CUDA graph";
+    case PSTGF_ERR_STATIC_LIMIT: return "PSTGF_ERR_STATIC_LIMIT: pstgf_rmat_form_static: the wave's pair-form scratch exceeds PSTGF_STATIC_SCRATCH_BYTES";
   }
   return "unknown pstgf_status_t";
 }

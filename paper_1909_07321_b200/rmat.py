@@ -20,10 +20,11 @@ PSTGF_HOST_PIPELINE_AUTO, PSTGF_HOST_PIPELINE_CHUNKED = 0, 1
 PSTGF_SLAB_AUTO, PSTGF_SLAB_NONE, PSTGF_SLAB_T32, PSTGF_SLAB_T64, PSTGF_SLAB_T128 = 0, 1, 2, 3, 4
 PSTGF_PAIRS_AUTO, PSTGF_PAIRS_NONE, PSTGF_PAIRS_ALWAYS = 0, 1, 2
 PSTGF_SMALL_AUTO, PSTGF_SMALL_NONE, PSTGF_SMALL_ALWAYS = 0, 1, 2
-PSTGF_ERR_TIMEOUT, PSTGF_ERR_CAPTURE = 6, 7
-PSTGF_RMAT_VERSION = 200            # must equal include/pstgf_rmat.h; load() checks it against the library
+PSTGF_ERR_TIMEOUT, PSTGF_ERR_CAPTURE, PSTGF_ERR_STATIC_LIMIT = 6, 7, 8
+PSTGF_STATIC_SCRATCH_BYTES = 16 << 20   # include/pstgf_rmat.h
+PSTGF_RMAT_VERSION = 201            # must equal include/pstgf_rmat.h; load() checks it against the library
 
-EXPORTS = ["pstgf_rmat_form", "pstgf_rmat_form_hdat", "pstgf_rmat_batch_workspace_bytes", "pstgf_rmat_form_batch",
+EXPORTS = ["pstgf_rmat_form", "pstgf_rmat_form_hdat", "pstgf_rmat_form_static", "pstgf_rmat_batch_workspace_bytes", "pstgf_rmat_form_batch",
            "pstgf_rmat_form_naive", "pstgf_rmat_form_sliced", "pstgf_rmat_sliced_workspace_bytes", "pstgf_rmat_form_batch_host", "pstgf_mesh_from_zscaled", "pstgf_rmat_finalize",
            "pstgf_debug_set_tail_policy", "pstgf_debug_set_slab_policy", "pstgf_debug_set_pair_policy", "pstgf_debug_set_small_policy",
            "pstgf_debug_set_host_pipeline",
@@ -74,6 +75,8 @@ def load(build_if_missing: bool = False):
     lib.pstgf_rmat_form.restype = i
     lib.pstgf_rmat_form_hdat.argtypes = [vp, ll, vp, vp, i, i, i, d, vp, vp]
     lib.pstgf_rmat_form_hdat.restype = i
+    lib.pstgf_rmat_form_static.argtypes = [vp, ll, vp, vp, i, i, i, d, vp, vp]
+    lib.pstgf_rmat_form_static.restype = i
     lib.pstgf_rmat_form_naive.argtypes = [ctypes.POINTER(pstgf_wave_t), vp]
     lib.pstgf_rmat_form_naive.restype = i
     lib.pstgf_rmat_form_sliced.argtypes = [ctypes.POINTER(pstgf_wave_t), i, vp, sz, vp]
@@ -168,6 +171,21 @@ def pstgf_rmat_form(W, E_k, energies, a: float, R_out=None, stream=None) -> torc
     with torch.cuda.device(W.device):
         _check(lib.pstgf_rmat_form(w.W, w.ldw, w.E_k, w.energies, w.n_chan, w.n_poles, w.n_E, w.a, w.R_out,
                                    _stream_ptr(stream)))
+    return R_out
+
+
+def pstgf_rmat_form_static(W, E_k, energies, a: float, R_out, stream=None) -> torch.Tensor:
+    """pstgf_rmat_form for callers that cannot allocate device memory (no room left beside their own arena, a loop
+    that cannot stand cudaMalloc's device-wide synchronisation, a thread inside its framework's allocator): the
+    library's scratch is a 16 MiB array built into its device image instead.  ``R_out`` is required -- this binding
+    allocates nothing either.  Same bits as pstgf_rmat_form; a pair-form wave whose scratch exceeds the array raises
+    PstgfError with status PSTGF_ERR_STATIC_LIMIT.  All calls on a device share the one array: keep them ordered
+    on the GPU (one stream, or events)."""
+    lib = load()
+    w = _wave_struct(W, E_k, energies, a, R_out)
+    with torch.cuda.device(W.device):
+        _check(lib.pstgf_rmat_form_static(w.W, w.ldw, w.E_k, w.energies, w.n_chan, w.n_poles, w.n_E, w.a, w.R_out,
+                                          _stream_ptr(stream)))
     return R_out
 
 

@@ -77,7 +77,7 @@ def test_version_and_status_strings(lib):
     m = re.search(r"#define\s+PSTGF_RMAT_VERSION\s+(\d+)", open(HEADER).read())
     assert lib.pstgf_version() == int(m.group(1))
     seen = set()
-    for code in range(8):
+    for code in range(9):
         s = lib.pstgf_status_string(code).decode()
         assert s and s not in seen
         seen.add(s)
@@ -97,6 +97,13 @@ def test_argument_errors_need_no_device(lib):
     assert lib.pstgf_rmat_form(fake + 4, 6, fake, fake, 4, 6, 1, 20.0, fake, None) == 2  # misaligned
     assert lib.pstgf_rmat_form(fake, 6, fake, fake, 0, 6, 1, 20.0, fake, None) == 0     # n_chan == 0: nothing to do
     assert lib.pstgf_rmat_form(fake, 6, fake, fake, 4, 6, 0, 20.0, fake, None) == 0     # n_E == 0
+    # the no-allocation call: same checks, and a wave beyond its built-in scratch is refused before any CUDA call
+    lib.pstgf_rmat_form_static.argtypes = [vp, ll, vp, vp, i, i, i, d, vp, vp]
+    lib.pstgf_rmat_form_static.restype = i
+    assert lib.pstgf_rmat_form_static(fake, 6, fake, fake, 4, 6, 1, 0.0, fake, None) == 1       # a <= 0
+    assert lib.pstgf_rmat_form_static(fake + 4, 6, fake, fake, 4, 6, 1, 20.0, fake, None) == 2  # misaligned
+    assert lib.pstgf_rmat_form_static(fake, 6, fake, fake, 4, 6, 0, 20.0, fake, None) == 0      # n_E == 0
+    assert lib.pstgf_rmat_form_static(fake, 1280, fake, fake, 64, 1280, 4096, 20.0, fake, None) == 8   # 63 MB of pair scratch > 16 MiB
     # H.DAT record order: the leading dimension runs over channels
     lib.pstgf_rmat_form_hdat.argtypes = [vp, ll, vp, vp, i, i, i, d, vp, vp]
     lib.pstgf_rmat_form_hdat.restype = i
