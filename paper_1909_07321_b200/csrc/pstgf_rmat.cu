@@ -39,6 +39,13 @@ pstgf_status_t cuda_fail(cudaError_t e) {
     if (e_ != cudaSuccess) return cuda_fail(e_);          \
   } while (0)
 
+}  // namespace
+void pstgf::set_last_call_state(int launches, int cuda_error) {
+  tl_launches = launches;
+  tl_cuda_error = cuda_error;
+}
+namespace {
+
 // ---- device / driver state -----------------------------------------------------------------
 typedef CUresult (*encode_tiled_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                     const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,

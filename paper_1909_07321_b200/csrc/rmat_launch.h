@@ -33,6 +33,10 @@ cudaError_t persistent_launch_f2(bool batch, const PersistentArgs &a, cudaStream
 // R_out, diag_add, ldw, inv2a, n_chan, n_poles, n_E and tr of `w`.
 cudaError_t small_launch(const DevWave &w, cudaStream_t s);
 
+// pstgf_rmat.cu: the calling thread's "launches of the last call" / "cudaError_t of the last failure" (what
+// pstgf_last_launch_count and pstgf_last_cuda_error report), for entry points that live in other units.
+void set_last_call_state(int launches, int cuda_error);
+
 inline cudaError_t persistent_prepare_all() {
   cudaError_t e = persistent_prepare_f0();
   if (e == cudaSuccess) e = persistent_prepare_f1();

@@ -17,10 +17,12 @@
 #include <stdint.h>
 
 #include <algorithm>
+#include <cfloat>
 #include <cmath>
 #include <mutex>
 
 #include "../../include/pstgf_rmat.h"
+#include "rmat_launch.h"
 
 namespace {
 
@@ -55,7 +57,7 @@ __global__ void __launch_bounds__(256) slice_kernel(const double *__restrict__ W
     for (int k = threadIdx.x; k < n_poles; k += blockDim.x) {
       const double x = E_k ? w[k] * (1.0 / (E_k[k] - E)) : w[k];
       if (CACHE) xrow[k] = x;
-      m = fmax(m, fabs(x));
+      m = fabs(x) <= DBL_MAX ? fmax(m, fabs(x)) : INFINITY;       // inf or NaN (an energy on a pole): fmax alone would drop a NaN
     }
   red[threadIdx.x] = m;
   __syncthreads();
@@ -64,9 +66,12 @@ __global__ void __launch_bounds__(256) slice_kernel(const double *__restrict__ W
     __syncthreads();
   }
   m = red[0];
+  // a row with a non-finite element has no digits: they are written as zeros and the row's scale as NaN, which the
+  // epilogue multiplies into every R element the row enters (IEEE inf/NaN there, as the header promises)
+  const bool bad = !(m <= DBL_MAX);
   int ex = 0;
-  if (m > 0.0 && isfinite(m)) (void)frexp(m, &ex);          // m = f 2^ex, f in [0.5, 1): |x| < 2^ex
-  const double scale = ldexp(1.0, ex), inv = ldexp(1.0, -ex);
+  if (m > 0.0 && !bad) (void)frexp(m, &ex);                 // m = f 2^ex, f in [0.5, 1): |x| < 2^ex
+  const double scale = bad ? __longlong_as_double(0x7ff8000000000000LL) : ldexp(1.0, ex), inv = ldexp(1.0, -ex);
   if (threadIdx.x == 0) scales[(size_t)e * Cp + row] = scale;
   for (long long k4 = (long long)threadIdx.x * 4; k4 < Kp; k4 += (long long)blockDim.x * 4) {
     uint32_t word[SL_MAX];
@@ -78,7 +83,7 @@ __global__ void __launch_bounds__(256) slice_kernel(const double *__restrict__ W
       double r = 0.0;
       if (in_row && k < n_poles) {
         const double x = CACHE ? xrow[k] : (E_k ? w[k] * (1.0 / (E_k[k] - E)) : w[k]);
-        r = x * inv * 64.0;
+        r = bad ? 0.0 : x * inv * 64.0;
       }
 #pragma unroll
       for (int i = 0; i < SL_MAX; ++i) {
@@ -188,6 +193,7 @@ sliced_gemm_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 0) {
+    __syncwarp();                                            // lane 0 comes out of the barrier set-up: .sync.aligned wants the warp converged
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_slot)), "r"(512u) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
@@ -304,7 +310,10 @@ sliced_gemm_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_consta
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
-  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512u) : "memory");
+  if (warp == 0) {
+    __syncwarp();                                            // lane 0 ran the producer loop on its own
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512u) : "memory");
+  }
 }
 
 // ---- host ----------------------------------------------------------------------------------------
@@ -336,6 +345,7 @@ SlicedLayout sliced_layout(int n_chan, int n_poles, int n_E, int S) {
   const size_t per_op = (size_t)S * (size_t)L.Cp * (size_t)L.Kp;             // digits of one operand at one energy
   const size_t budget = (size_t)1 << 30;                                     // B digits of a chunk: at most 1 GiB
   L.chunk = (int)std::max<size_t>(1, std::min<size_t>((size_t)std::max(n_E, 1), budget / std::max<size_t>(per_op, 1)));
+  L.chunk = std::min(L.chunk, 65535);                                        // the slicing launch has one grid.y per energy
   auto al = [](size_t x) { return (x + 1023) & ~(size_t)1023; };
   L.off_sA = 0;
   L.off_sB = al(L.off_sA + sizeof(double) * (size_t)L.Cp);
@@ -355,6 +365,7 @@ size_t pstgf_rmat_sliced_workspace_bytes(int n_chan, int n_poles, int n_E, int n
 }
 
 pstgf_status_t pstgf_rmat_form_sliced(const pstgf_wave_t *wave, int n_slices, void *workspace, size_t workspace_bytes, void *stream) {
+  pstgf::set_last_call_state(0, 0);
   if (!wave) return PSTGF_ERR_INVALID_VALUE;
   const pstgf_wave_t &w = *wave;
   if (w.n_chan < 0 || w.n_poles < 0 || w.n_E < 0 || !(w.a > 0.0) || !std::isfinite(w.a)) return PSTGF_ERR_INVALID_VALUE;
@@ -386,22 +397,25 @@ pstgf_status_t pstgf_rmat_form_sliced(const pstgf_wave_t *wave, int n_slices, vo
   int8_t *dA = reinterpret_cast<int8_t *>(ws + L.off_A), *dB = reinterpret_cast<int8_t *>(ws + L.off_B);
   const int S = n_slices;
   const int smem = STAGES * S * (TILE_M + TILE_N) * KB + 1024;
-  if (cudaFuncSetAttribute(sliced_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return PSTGF_ERR_CUDA;
+  auto fail = [](cudaError_t e) { pstgf::set_last_call_state(0, (int)e); (void)cudaGetLastError(); return PSTGF_ERR_CUDA; };
+  cudaError_t ce = cudaFuncSetAttribute(sliced_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if (ce != cudaSuccess) return fail(ce);
   CUtensorMap mapA, mapB;
   if (!encode_bytes_map(&mapA, dA, (long long)S * L.Cp, L.Kp, TILE_M) ||
       !encode_bytes_map(&mapB, dB, (long long)L.chunk * S * L.Cp, L.Kp, TILE_N))
-    return PSTGF_ERR_CUDA;
+    return fail(cudaErrorInvalidValue);
   // the slicing kernel keeps a row in shared memory between its two passes when that does not cost occupancy (a row of
   // config 5 is 80 KB: two blocks per SM, measured 12.6 ms per step against 8.8 ms with the divisions done twice)
   const size_t row_bytes = sizeof(double) * (size_t)w.n_poles;
   const bool cache = row_bytes <= 16 * 1024;
-  if (cache && cudaFuncSetAttribute(slice_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)row_bytes) != cudaSuccess) return PSTGF_ERR_CUDA;
+  if (cache && (ce = cudaFuncSetAttribute(slice_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)row_bytes)) != cudaSuccess) return fail(ce);
   auto slice = [&](dim3 grid, const double *Ek, const double *en, int8_t *digits, double *scales) {
     if (cache) slice_kernel<true><<<grid, 256, row_bytes, s>>>(w.W, w.ldw, Ek, en, w.n_chan, w.n_poles, S, L.Cp, L.Kp, digits, scales);
     else slice_kernel<false><<<grid, 256, 0, s>>>(w.W, w.ldw, Ek, en, w.n_chan, w.n_poles, S, L.Cp, L.Kp, digits, scales);
   };
   // digits of A = W, once
   slice(dim3((unsigned)L.Cp, 1), nullptr, nullptr, dA, sA);
+  int launches = 1;
   for (int e0 = 0; e0 < w.n_E; e0 += L.chunk) {
     const int ne = std::min(L.chunk, w.n_E - e0);
     // digits of B_e = W diag(1 / (E_k - E_e)) for the chunk's energies, then the contraction
@@ -423,8 +437,12 @@ pstgf_status_t pstgf_rmat_form_sliced(const pstgf_wave_t *wave, int n_slices, vo
     for (int I = 0; I < g.n_ti; ++I) g.tiles_per_e += std::max(0, g.n_tj - 2 * I);
     const long long items = (long long)g.tiles_per_e * ne;
     sliced_gemm_kernel<<<(unsigned)std::min<long long>(sms, items), GEMM_THREADS, smem, s>>>(mapA, mapB, g);
+    launches += 2;
   }
-  return cudaGetLastError() == cudaSuccess ? PSTGF_OK : PSTGF_ERR_CUDA;
+  ce = cudaGetLastError();
+  if (ce != cudaSuccess) return fail(ce);
+  pstgf::set_last_call_state(launches, 0);
+  return PSTGF_OK;
 }
 
 }  // extern "C"
