@@ -1061,3 +1061,47 @@ def test_sliced_variant_config2_and_errors(rmat, oracle):
     assert lib.pstgf_rmat_form_sliced(one, 9, ws.data_ptr(), ws.numel(), None) == 1          # n_slices out of range
     assert lib.pstgf_rmat_form_sliced(None, 7, ws.data_ptr(), ws.numel(), None) == 1
     assert lib.pstgf_rmat_sliced_workspace_bytes(64, 1280, 8, 7) > 0 and lib.pstgf_rmat_sliced_workspace_bytes(64, 1280, 8, 1) == 0
+
+
+def test_sliced_variant_energy_on_a_pole_and_launch_count(rmat, oracle):
+    """An energy that equals a pole makes a term of eq. 4 infinite: the sliced variant must hand back IEEE inf/NaN for
+    that energy (a non-finite row has no digits; its scale is NaN) and leave the other energies alone; and the call
+    reports its launches (one slicing launch for W, then a slicing and a GEMM launch per chunk of energies)."""
+    from paper_1909_07321_b200 import inputs
+    w = inputs.make_wave(15999, 64, 128, 3)
+    en = w.energies.copy()
+    en[1] = w.E_k[5]
+    R = rmat.pstgf_rmat_form_sliced(_dev(w.W), _dev(w.E_k), _dev(en), w.a, n_slices=8)
+    assert rmat.pstgf_last_launch_count() == 3
+    torch.cuda.synchronize()
+    R = R.cpu().numpy()
+    assert not np.isfinite(R[1]).any()
+    ref = oracle.rmat_form(w.W, w.E_k, en[[0, 2]], w.a, threads=_threads())
+    assert _rel_err_per_energy(R[[0, 2]], ref).max() <= 1e-13
+
+
+def test_sliced_variant_config5_sampled(rmat, oracle):
+    """The sliced variant at the size DESIGN.md 6.5 quotes it on: config 5 (512 x 10240), 7 and 8 slices, on the sampled
+    energies of the full-size parity tests -- first, last, the one NEAREST A POLE (clearance 1e-3 Ryd), 5 seeded -- plus
+    enough evenly spaced ones to need a second chunk of energies (29 fit the 1 GiB digit budget).  The error is measured
+    against max |R| of the energy; the digits of a row of W diag(d_e) are relative to that row's largest element, so an
+    energy close to a pole coarsens the other terms of the row by the ratio of the pole term to them, and max |R| grows
+    by the same pole term: the bound in this measure holds down to the clearance, which is what is asserted."""
+    from paper_1909_07321_b200 import inputs
+    w = inputs.make_config(5).waves[0]
+    idx = np.unique(np.concatenate([inputs.sample_energy_indices(w), np.linspace(0, w.n_E - 1, 34).astype(np.int64)]))
+    assert len(idx) > 29
+    near = int(np.argmin(inputs.min_pole_distance(w.energies, w.E_k)))
+    assert near in idx
+    Wd, Ek, en = _dev(w.W), _dev(w.E_k), _dev(w.energies[idx])
+    ref = oracle.rmat_form(w.W, w.E_k, w.energies[idx], w.a, threads=_threads())
+    for S, tol in ((7, 5e-12), (8, 1e-13)):
+        R = rmat.pstgf_rmat_form_sliced(Wd, Ek, en, w.a, n_slices=S)
+        launches = rmat.pstgf_last_launch_count()
+        torch.cuda.synchronize()
+        assert launches >= 5, launches                       # more than one chunk: > 1 GEMM launch
+        R = R.cpu().numpy()
+        err = _rel_err_per_energy(R, ref)
+        assert err.max() <= tol, (S, float(err.max()), int(idx[int(err.argmax())]))
+        assert np.array_equal(R, R.transpose(0, 2, 1))
+
