@@ -1105,3 +1105,25 @@ def test_sliced_variant_config5_sampled(rmat, oracle):
         assert err.max() <= tol, (S, float(err.max()), int(idx[int(err.argmax())]))
         assert np.array_equal(R, R.transpose(0, 2, 1))
 
+
+def test_host_call_signalled_pipeline_with_pair_form_waves(rmat):
+    """A pair-form wave big enough for the signalled route of the host call (96^2 x 6000 x 1280 = 7e10 counted FLOP,
+    above the 2 ms threshold), cut into ten 128-energy pieces by a small max_chunk_bytes, beside a symmetric-form
+    wave: two launch groups in one chunk, completion targets of pair items, pieces copied back in completion order.
+    Bitwise equal to the device batch call (the form is chosen on the whole wave, so every piece goes the wave's way)."""
+    from paper_1909_07321_b200 import inputs
+    waves = [inputs.make_wave(90, 96, 6000, 1280), inputs.make_wave(91, 200, 4000, 64)]
+    host = []
+    for w in waves:
+        R = torch.full((w.n_E, w.n_chan, w.n_chan), np.nan, dtype=torch.float64).pin_memory()
+        host.append((torch.from_numpy(w.W).pin_memory(), torch.from_numpy(w.E_k).pin_memory(),
+                     torch.from_numpy(w.energies).pin_memory(), w.a, R))
+    rmat.pstgf_rmat_form_batch_host(host, max_chunk_bytes=96 * 96 * 8 * 128)
+    # signalled: one scratch-builder launch and one launch per group for the whole job (chunked: a set per piece)
+    assert rmat.pstgf_last_launch_count() == 3
+    dev = _form_batch(rmat, waves)
+    for h, d in zip(host, dev):
+        assert torch.equal(h[4], d.cpu())
+    w = waves[0]
+    Rn = rmat.pstgf_rmat_form_naive(_dev(w.W), _dev(w.E_k), _dev(w.energies[:40]), w.a).cpu().numpy()
+    _check(host[0][4].numpy()[:40], Rn)
