@@ -531,7 +531,7 @@ def run_cuda(args):
             e1.record()
             torch.cuda.synchronize()
             best_ms = min(best_ms, e0.elapsed_time(e1))
-        probe["dmma_dependent_latency_clk"] = best_ms * 1e-3 * peaks["sm_max_mhz"] * 1e6 / (it_chain * 32)
+        dmma_latency_clk = best_ms * 1e-3 * peaks["sm_max_mhz"] * 1e6 / (it_chain * 32)
     context = None
     if rank == 0 and args.probe_i8:
         isink = torch.zeros(sms, dtype=torch.int32, device="cuda")
@@ -564,7 +564,8 @@ def run_cuda(args):
                 "t_roof_ms": 1e3 * max(t_fp64, t_hbm), "hbm_write_gbs": wl.r_bytes() / (kern_ms * 1e-3) / 1e9,
                 "hbm_peak_gbs": peaks["hbm_gbs"]}
     if probe:
-        roofline["fp64_probe_tflops"] = probe
+        roofline["fp64_probe_tflops"] = probe                       # TFLOP/s per probe kind, nothing else
+        roofline["dmma_dependent_latency_clk"] = dmma_latency_clk   # a latency in SM clocks: a key of its own
     roofline["traffic"] = ncu_traffic(args.config) if not (args.n_E or sliced) else None
     roofline["traffic_source"] = ("committed ncu --set full capture (profiles/traffic.csv): DRAM bytes read + written "
                                   "per launch; not measured in this run") if roofline["traffic"] is not None else None
