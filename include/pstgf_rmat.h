@@ -25,8 +25,12 @@
  *  - Device memory owned by the library.  The DEVICE-pointer calls allocate
  *    none, but for the 8 KiB counter pool of pstgf_rmat_form (once per
  *    device) and that call's stream-ordered scratch for few-channel waves
- *    (freed behind the launch); the batch call keeps its tables and scratch
- *    in the caller's workspace.
+ *    (P plus at most 128 MiB of D whatever n_E is, freed behind the last
+ *    launch; the pool it comes from keeps at most 256 MiB across a
+ *    synchronise and returns the rest to the device; if the scratch cannot
+ *    be had the wave is done in the symmetric form, which needs none);
+ *    pstgf_rmat_form_static allocates nothing at all; the batch call keeps
+ *    its tables and scratch in the caller's workspace.
  *    pstgf_rmat_form_batch_host stages through a memory pool of its own (one
  *    per device) and keeps 33 KiB of completion words per calling thread.
  *    pstgf_rmat_finalize() frees all of it.
@@ -248,8 +252,13 @@ size_t pstgf_rmat_batch_workspace_bytes(const pstgf_wave_t *waves, int n_waves);
  * small launch): tiles of an n_chan x n_chan matrix that small are mostly
  * diagonal blocks, which the symmetric form computes in full.  pstgf_rmat_form
  * does the same with stream-ordered scratch of its own (cudaMallocAsync on
- * `stream`, freed behind the launch).  The choice depends on the wave's shape
- * only, so a wave gives the same bits through every call.
+ * `stream`, freed behind the last launch): P once, the reciprocals for at most
+ * 128 MiB worth of energies at a time -- a longer mesh goes out as several
+ * (builder, GEMM) launch pairs over energy ranges.  The host-buffer call
+ * builds P once per wave and shares it between the wave's pieces.  The choice
+ * depends on the wave's shape only, so a wave gives the same bits through
+ * every call (the one exception: pstgf_rmat_form falls back to the symmetric
+ * form, a few ulp apart, when the device has no memory left for the scratch).
  */
 pstgf_status_t pstgf_rmat_form_batch(const pstgf_wave_t *waves, int n_waves, void *workspace,
                                      size_t workspace_bytes, void *stream);

@@ -196,23 +196,32 @@ bool wants_small_kernel(int n_chan, int n_poles, int n_E) {
 }
 long long pair_count(int n_chan) { return (long long)n_chan * (n_chan + 1) / 2; }
 long long pair_ld(int n_poles) { return ((long long)n_poles + 1) & ~1LL; }
+size_t pair_D_bytes(int n_poles, int n_E) { return (((size_t)n_E * (size_t)pair_ld(n_poles) * 8) + 255) & ~(size_t)255; }
 size_t pair_scratch_bytes(int n_chan, int n_poles, int n_E) {        // P, D, the (n, m) table: each 256-byte aligned
   const size_t ld = (size_t)pair_ld(n_poles);
   const size_t p = (((size_t)pair_count(n_chan) * ld * 8) + 255) & ~(size_t)255;
-  const size_t d = (((size_t)n_E * ld * 8) + 255) & ~(size_t)255;
   const size_t t = (((size_t)pair_count(n_chan) * 4) + 255) & ~(size_t)255;
-  return p + d + t;
+  return p + pair_D_bytes(n_poles, n_E) + t;
 }
 // Cuts a wave into pair items; `scratch` is where its P and D go.  Every energy tile starts out coarse (128-pair
 // items); plan_pair_tails then cuts the tail of the launch into 64-pair items.
-void plan_pairs(DevWave &d, unsigned char *scratch) {
+// With kept_P / kept_nm (P and the pair table of this wave, built earlier from all of W -- they hold no energy) the
+// scratch takes D alone (pair_D_bytes) and the builder is told to leave P be.
+void plan_pairs(DevWave &d, unsigned char *scratch, double *kept_P = nullptr, const unsigned int *kept_nm = nullptr) {
   d.n_pairs = (int)pair_count(d.n_chan);
   d.pair_ld = pair_ld(d.n_poles);
-  d.pair_P = reinterpret_cast<double *>(scratch);
-  const size_t p_bytes = (((size_t)d.n_pairs * (size_t)d.pair_ld * 8) + 255) & ~(size_t)255;
-  const size_t d_bytes = (((size_t)d.n_E * (size_t)d.pair_ld * 8) + 255) & ~(size_t)255;
-  d.pair_D = reinterpret_cast<double *>(scratch + p_bytes);
-  d.pair_nm = reinterpret_cast<const unsigned int *>(scratch + p_bytes + d_bytes);
+  if (kept_P) {
+    d.pair_P = kept_P;
+    d.pair_nm = kept_nm;
+    d.pair_D = reinterpret_cast<double *>(scratch);
+    d.pair_keep_P = 1;
+  } else {
+    d.pair_P = reinterpret_cast<double *>(scratch);
+    const size_t p_bytes = (((size_t)d.n_pairs * (size_t)d.pair_ld * 8) + 255) & ~(size_t)255;
+    const size_t d_bytes = (((size_t)d.n_E * (size_t)d.pair_ld * 8) + 255) & ~(size_t)255;
+    d.pair_D = reinterpret_cast<double *>(scratch + p_bytes);
+    d.pair_nm = reinterpret_cast<const unsigned int *>(scratch + p_bytes + d_bytes);
+  }
   d.pair_nfb = d.n_chan / 8;
   d.pair_rb = pstgf::pair_block_rows(d.n_chan);
   d.pair_mt = (d.n_pairs + pstgf::PT_M - 1) / pstgf::PT_M;
@@ -673,13 +682,19 @@ pstgf_status_t zero_fill(const pstgf_wave_t &w, cudaStream_t s) {
 // Device memory of the host call, and the single-wave call's pair-form scratch, come from a pool the library owns (one per device, release threshold =
 // never, freed by pstgf_rmat_finalize): the default pool hands its memory back at every synchronise, and
 // re-growing it costs tens of milliseconds per call.
+// The single-wave call's pair-form scratch has a pool of its own that keeps at most SCRATCH_POOL_KEEP bytes across a
+// synchronise (what a run of RINIT calls on one wave reuses) and hands the rest back to the device, so that a caller's
+// own allocator can have it.
 std::mutex g_pool_mutex;
 cudaMemPool_t g_pool[64] = {nullptr};
+cudaMemPool_t g_scratch_pool[64] = {nullptr};
+constexpr unsigned long long SCRATCH_POOL_KEEP = 256ULL << 20;
 
-cudaError_t library_pool(int dev, cudaMemPool_t *out) {
+cudaError_t library_pool(int dev, cudaMemPool_t *out, bool scratch = false) {
   std::lock_guard<std::mutex> lock(g_pool_mutex);
   if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
-  if (!g_pool[dev]) {
+  cudaMemPool_t *pools = scratch ? g_scratch_pool : g_pool;
+  if (!pools[dev]) {
     cudaMemPoolProps props;
     std::memset(&props, 0, sizeof(props));
     props.allocType = cudaMemAllocationTypePinned;
@@ -689,12 +704,12 @@ cudaError_t library_pool(int dev, cudaMemPool_t *out) {
     cudaMemPool_t pool;
     cudaError_t e = cudaMemPoolCreate(&pool, &props);
     if (e != cudaSuccess) return e;
-    unsigned long long keep = ~0ULL;
+    unsigned long long keep = scratch ? SCRATCH_POOL_KEEP : ~0ULL;
     e = cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
     if (e != cudaSuccess) { cudaMemPoolDestroy(pool); return e; }
-    g_pool[dev] = pool;
+    pools[dev] = pool;
   }
-  *out = g_pool[dev];
+  *out = pools[dev];
   return cudaSuccess;
 }
 
@@ -706,14 +721,14 @@ size_t ws_tables_bytes(int n_waves) {
 }
 // tables, then the scratch (P, D) of every wave that is done in the pair form; force_pair, if given, overrides the
 // per-wave choice (the host call cuts waves into energy ranges and wants every range to go the way of the whole wave)
-size_t ws_bytes(const pstgf_wave_t *waves, int n_waves, const unsigned char *force_pair = nullptr) {
+size_t ws_bytes(const pstgf_wave_t *waves, int n_waves, const unsigned char *force_pair = nullptr, double *const *kept_P = nullptr) {
   size_t b = ws_tables_bytes(n_waves);
   if (waves)
     for (int p = 0; p < n_waves; ++p) {
       const pstgf_wave_t &w = waves[p];
       if (w.n_chan <= 0 || w.n_E <= 0 || w.n_poles <= 0) continue;
       const bool pair = force_pair ? force_pair[p] != 0 : wants_pair_form(w.n_chan, w.n_poles, w.n_E);
-      if (pair) b += pair_scratch_bytes(w.n_chan, w.n_poles, w.n_E);
+      if (pair) b += (kept_P && kept_P[p]) ? pair_D_bytes(w.n_poles, w.n_E) : pair_scratch_bytes(w.n_chan, w.n_poles, w.n_E);
     }
   return b;
 }
@@ -840,6 +855,87 @@ pstgf_status_t pstgf_debug_set_slab_policy(int policy) {
   return PSTGF_OK;
 }
 
+// One persistent launch of a single-wave plan on `s`, with a work counter from the pool when there are more items
+// than CTAs.
+static pstgf_status_t launch_single(std::vector<DevWave> &d, const DeviceState &ds, cudaStream_t s) {
+  const long long n_items = wave_items(d[0]);
+  const int grid = (int)std::min<long long>(ds.sm_count, n_items);
+  const pstgf::RingGeo geo = ring_geometry(d);
+  std::lock_guard<std::mutex> lock(g_counter_mutex);
+  unsigned long long *counter = nullptr;
+  // no more items than CTAs: item b goes to CTA b, no counter needed (one L2 round trip less for the tiny calls)
+  const int slot = n_items <= grid ? -1 : acquire_counter(ds.device, s, &counter);
+  pstgf::PersistentArgs pa{&d[0], nullptr, nullptr, 1, n_items, counter, geo, grid};
+  PSTGF_CUDA(pstgf::persistent_launch_family(launch_family(d), false, pa, s));
+  if (slot >= 0) {
+    CounterPool &cp = g_counters[ds.device];
+    PSTGF_CUDA(cudaEventRecord(cp.ev[slot], s));
+    cp.armed[slot] = true;
+  }
+  return PSTGF_OK;
+}
+
+// The pair form of the single-wave call.  Scratch is stream-ordered memory from the library's scratch pool, allocated
+// here and freed behind the last launch: P and the pair table once, D for at most PAIR_D_RANGE_BYTES worth of energies
+// at a time -- a long mesh goes out as several (builder, GEMM) launch pairs over energy ranges that start on energy-tile
+// boundaries, all reading the one P, so the scratch does not grow with n_E (a 64 x 1280 wave with 10^6 energies would
+// otherwise want 10 GB of D).  Every R element is still one thread's sum in the fixed k order: same bits as one launch.
+// *no_memory is set, and nothing has been enqueued, when the scratch cannot be had; the caller then takes the
+// symmetric form, which needs none.
+constexpr size_t PAIR_D_RANGE_BYTES = (size_t)128 << 20;
+static pstgf_status_t form_single_pairs(const pstgf_wave_t &w, const DeviceState &ds, cudaStream_t s, bool *no_memory) {
+  *no_memory = false;
+  const size_t row_bytes = (size_t)pair_ld(w.n_poles) * 8;
+  int range = w.n_E;
+  if (pair_D_bytes(w.n_poles, w.n_E) > PAIR_D_RANGE_BYTES)
+    range = std::max<long long>(pstgf::PT_N, (long long)(PAIR_D_RANGE_BYTES / row_bytes) / pstgf::PT_N * pstgf::PT_N);
+  range = std::min(range, w.n_E);
+  cudaMemPool_t pool;
+  PSTGF_CUDA(library_pool(ds.device, &pool, true));
+  void *scratch = nullptr;
+  const cudaError_t ae = cudaMallocFromPoolAsync(&scratch, pair_scratch_bytes(w.n_chan, w.n_poles, range), pool, s);
+  if (ae != cudaSuccess) {
+    (void)cudaGetLastError();
+    if (ae != cudaErrorMemoryAllocation) return cuda_fail(ae);
+    *no_memory = true;
+    return PSTGF_OK;
+  }
+  pstgf_status_t st = PSTGF_OK;
+  int launches = 0;
+  double *kept_P = nullptr;
+  const unsigned int *kept_nm = nullptr;
+  for (int e0 = 0; e0 < w.n_E && st == PSTGF_OK; e0 += range) {
+    pstgf_wave_t part = w;
+    part.n_E = std::min(range, w.n_E - e0);
+    part.energies = w.energies + e0;
+    part.R_out = w.R_out + (size_t)e0 * w.n_chan * w.n_chan;
+    if (w.diag_add) part.diag_add = w.diag_add + (size_t)e0 * w.n_chan;
+    std::vector<DevWave> d(1);
+    plan_wave(part, d[0], ds.l2_bytes);
+    if (e0 == 0) {
+      plan_pairs(d[0], static_cast<unsigned char *>(scratch));     // the first range is a full one: P | D[range] | table
+      kept_P = d[0].pair_P;
+      kept_nm = d[0].pair_nm;
+    } else {                                                       // later ranges: the same P and table, D in the same place
+      plan_pairs(d[0], reinterpret_cast<unsigned char *>(kept_P) + ((((size_t)pair_count(w.n_chan) * row_bytes) + 255) & ~(size_t)255),
+                 kept_P, kept_nm);
+    }
+    plan_pair_tails(d, ds.sm_count);
+    st = encode_pair_maps(d[0]);
+    if (st != PSTGF_OK) break;
+    const int rows = d[0].n_E + (d[0].pair_keep_P ? 0 : d[0].n_pairs);
+    const int chunks = (rows + pstgf::PAIR_BUILD_ROWS - 1) / pstgf::PAIR_BUILD_ROWS;
+    pstgf::pair_build_kernel<false><<<dim3((unsigned)std::min(chunks, 8 * ds.sm_count), 1), 256, 0, s>>>(d[0], nullptr, 1);
+    const cudaError_t le = cudaGetLastError();
+    if (le != cudaSuccess) { st = cuda_fail(le); break; }
+    st = launch_single(d, ds, s);
+    launches += 2;
+  }
+  cudaFreeAsync(scratch, s);
+  if (st == PSTGF_OK) tl_launches = launches;
+  return st;
+}
+
 static pstgf_status_t form_single(const pstgf_wave_t &w, void *stream) {
   const int n_chan = w.n_chan, n_poles = w.n_poles, n_E = w.n_E;
   tl_launches = 0;
@@ -853,58 +949,24 @@ static pstgf_status_t form_single(const pstgf_wave_t &w, void *stream) {
   if (n_poles == 0) return zero_fill(w, s);
   std::vector<DevWave> d(1);
   plan_wave(w, d[0], ds.l2_bytes);
-  void *scratch = nullptr;
   if (wants_pair_form(n_chan, n_poles, n_E) && wants_small_kernel(n_chan, n_poles, n_E)) {
     PSTGF_CUDA(pstgf::small_launch(d[0], s));
     tl_launches = 1;
     return PSTGF_OK;
   }
   if (wants_pair_form(n_chan, n_poles, n_E)) {
-    // the pair form's scratch (P and D) is stream-ordered memory from the library's pool (kept between calls: the
-    // device's default pool hands its memory back at every synchronise): allocated here, freed behind the launch
-    cudaMemPool_t pool;
-    PSTGF_CUDA(library_pool(ds.device, &pool));
-    PSTGF_CUDA(cudaMallocFromPoolAsync(&scratch, pair_scratch_bytes(n_chan, n_poles, n_E), pool, s));
-    plan_pairs(d[0], static_cast<unsigned char *>(scratch));
-    plan_pair_tails(d, ds.sm_count);
-    st = encode_pair_maps(d[0]);
-    if (st == PSTGF_OK) {
-      const int rows = d[0].n_E + d[0].n_pairs;
-      const int chunks = (rows + pstgf::PAIR_BUILD_ROWS - 1) / pstgf::PAIR_BUILD_ROWS;
-      pstgf::pair_build_kernel<false><<<dim3((unsigned)std::min(chunks, 8 * ds.sm_count), 1), 256, 0, s>>>(d[0], nullptr, 1);
-      if (cudaGetLastError() != cudaSuccess) st = PSTGF_ERR_CUDA;
-    }
-    if (st != PSTGF_OK) {
-      cudaFreeAsync(scratch, s);
-      return st;
-    }
-    ++tl_launches;
-  } else {
-    plan_slabs(d, ds.sm_count);
-    plan_tails(d, ds.sm_count);
-    st = encode_map(d[0]);
-    if (st != PSTGF_OK) return st;
+    bool no_memory = false;
+    st = form_single_pairs(w, ds, s, &no_memory);
+    if (!no_memory) return st;
+    // no device memory for P and D: the symmetric form below needs none (a few ulp apart, see the header)
   }
-  const int build_launches = tl_launches;
-  const long long n_items = wave_items(d[0]);
-  const int grid = (int)std::min<long long>(ds.sm_count, n_items);
-  const pstgf::RingGeo geo = ring_geometry(d);
-  {
-    std::lock_guard<std::mutex> lock(g_counter_mutex);
-    unsigned long long *counter = nullptr;
-    // no more items than CTAs: item b goes to CTA b, no counter needed (one L2 round trip less for the tiny calls)
-    const int slot = n_items <= grid ? -1 : acquire_counter(ds.device, s, &counter);
-    pstgf::PersistentArgs pa{&d[0], nullptr, nullptr, 1, n_items, counter, geo, grid};
-    const cudaError_t le = pstgf::persistent_launch_family(launch_family(d), false, pa, s);
-    if (scratch) cudaFreeAsync(scratch, s);
-    PSTGF_CUDA(le);
-    if (slot >= 0) {
-      CounterPool &cp = g_counters[ds.device];
-      PSTGF_CUDA(cudaEventRecord(cp.ev[slot], s));
-      cp.armed[slot] = true;
-    }
-  }
-  tl_launches = build_launches + 1;
+  plan_slabs(d, ds.sm_count);
+  plan_tails(d, ds.sm_count);
+  st = encode_map(d[0]);
+  if (st != PSTGF_OK) return st;
+  st = launch_single(d, ds, s);
+  if (st != PSTGF_OK) return st;
+  tl_launches = 1;
   return PSTGF_OK;
 }
 
@@ -998,6 +1060,8 @@ struct BatchCompletion {
   unsigned int *abort_flag = nullptr;                // in: zeroed DEVICE word the load warps poll and set when an upload wait times out
   unsigned int *abort_flag_host = nullptr;           // in: host-mapped word the warp that timed out sets as well
   const unsigned char *force_pair = nullptr;         // in, optional: per input wave, 1 = pair form, 0 = SYRK form
+  double *const *kept_P = nullptr;                   // in, optional: per input wave, its P built earlier (null = build it here) ...
+  const unsigned int *const *kept_nm = nullptr;      // ... and the pair table that goes with it
   std::vector<int> order;                // out: input wave indices in the order the launch completes them
   std::vector<long long> items;          // out: items of each input wave (arrivals = items * EB)
 };
@@ -1013,7 +1077,8 @@ static pstgf_status_t form_batch_impl(const pstgf_wave_t *waves, int n_waves, vo
     if (st != PSTGF_OK) return st;
   }
   const unsigned char *force_pair = completion ? completion->force_pair : nullptr;
-  if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) != 0 || workspace_bytes < ws_bytes(waves, n_waves, force_pair))
+  double *const *kept_P = completion ? completion->kept_P : nullptr;
+  if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) != 0 || workspace_bytes < ws_bytes(waves, n_waves, force_pair, kept_P))
     return PSTGF_ERR_WORKSPACE;
   DeviceState dstate;
   pstgf_status_t st = device_state(dstate);
@@ -1074,9 +1139,14 @@ static pstgf_status_t form_batch_impl(const pstgf_wave_t *waves, int n_waves, vo
     const pstgf_wave_t &w = waves[order[q]];
     plan_wave(w, ds[q], dstate.l2_bytes);
     if (is_pair(order[q])) {
-      plan_pairs(ds[q], ws + scratch_off);
-      scratch_off += pair_scratch_bytes(w.n_chan, w.n_poles, w.n_E);
-      max_build_rows = std::max(max_build_rows, ds[q].n_E + ds[q].n_pairs);
+      if (kept_P && kept_P[order[q]]) {                  // the host call built this wave's P once for all its energy ranges
+        plan_pairs(ds[q], ws + scratch_off, kept_P[order[q]], completion->kept_nm[order[q]]);
+        scratch_off += pair_D_bytes(w.n_poles, w.n_E);
+      } else {
+        plan_pairs(ds[q], ws + scratch_off);
+        scratch_off += pair_scratch_bytes(w.n_chan, w.n_poles, w.n_E);
+      }
+      max_build_rows = std::max(max_build_rows, ds[q].n_E + (ds[q].pair_keep_P ? 0 : ds[q].n_pairs));
       st = encode_pair_maps(ds[q]);
       if (st != PSTGF_OK) return st;
     }
@@ -1366,6 +1436,9 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
   // waves done in the pair form: decided on the WHOLE wave (every energy range of it then goes the same way, so the
   // host call gives the bits of the device calls), and their W is uploaded before the launches (P is built from all of it)
   std::vector<unsigned char> pair_wave((size_t)n_waves, 0);
+  std::vector<double *> kept_P((size_t)n_waves, nullptr);
+  std::vector<const unsigned int *> kept_nm((size_t)n_waves, nullptr);
+  int p_launches = 0;
   for (int p = 0; p < n_waves; ++p) pair_wave[(size_t)p] = wants_pair_form(waves[p].n_chan, waves[p].n_poles, waves[p].n_E) ? 1 : 0;
   for (int p = 0; p < n_waves; ++p) {
     const pstgf_wave_t &w = waves[p];
@@ -1398,6 +1471,22 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
     dev[p].E_k = static_cast<double *>(dEk);
     dev[p].energies = static_cast<double *>(dEn);
     if (!overlap_upload || pair_wave[(size_t)p]) PSTGF_CUDA(upload_W(p, 0, w.n_poles, false));
+    if (pair_wave[(size_t)p]) {
+      // P = w_n w_m and the pair table hold no energy: built ONCE per wave here, behind its W on `stream`, and shared
+      // by every energy range (segment) of the wave in every chunk; the segments' own scratch is D alone
+      void *dP;
+      PSTGF_CUDA(dev_alloc(pair_scratch_bytes(w.n_chan, w.n_poles, 0), &dP));
+      DevWave d;
+      plan_wave(dev[p], d, ds.l2_bytes);
+      d.n_E = 0;                                         // rows of P only
+      plan_pairs(d, static_cast<unsigned char *>(dP));
+      kept_P[(size_t)p] = d.pair_P;
+      kept_nm[(size_t)p] = d.pair_nm;
+      const int chunks_p = (d.n_pairs + pstgf::PAIR_BUILD_ROWS - 1) / pstgf::PAIR_BUILD_ROWS;
+      pstgf::pair_build_kernel<false><<<dim3((unsigned)std::min(chunks_p, 8 * ds.sm_count), 1), 256, 0, res.s>>>(d, nullptr, 1);
+      PSTGF_CUDA(cudaGetLastError());
+      ++p_launches;
+    }
   }
   // Two ways to overlap the copy-back with the formation (pstgf_debug_set_host_pipeline):
   //  signalled  ONE launch forms a whole chunk (as much of R as the device budget allows); its segments (a wave's
@@ -1474,7 +1563,7 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
     for (const auto &ch : chunks) {
       size_t b = ws_tables_bytes((int)max_segs);
       for (const Segment &g : ch)
-        if (pair_wave[(size_t)g.wave]) b += pair_scratch_bytes(waves[g.wave].n_chan, waves[g.wave].n_poles, g.ne);
+        if (pair_wave[(size_t)g.wave]) b += pair_D_bytes(waves[g.wave].n_poles, g.ne);
       wsb = std::max(wsb, b);
     }
     cudaError_t e = cudaSuccess;
@@ -1527,7 +1616,9 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
       }
     }
   }
-  int launches = 0;
+  int launches = p_launches;
+  std::vector<double *> sub_P;
+  std::vector<const unsigned int *> sub_nm;
   std::vector<pstgf_wave_t> sub;
   std::vector<unsigned int *> done, flag;
   std::vector<const unsigned int *> rows_ready;
@@ -1544,6 +1635,8 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
     rows_ready.clear();
     ready_kind.clear();
     force.clear();
+    sub_P.clear();
+    sub_nm.clear();
     const size_t f0 = (size_t)b * MAX_CHUNK_SEGMENTS;
     for (const Segment &g : chunks[c]) {
       pstgf_wave_t w = dev[g.wave];
@@ -1553,6 +1646,8 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
       w.R_out = reinterpret_cast<double *>(static_cast<unsigned char *>(rbuf[b]) + g.off);
       sub.push_back(w);
       force.push_back(pair_wave[(size_t)g.wave]);
+      sub_P.push_back(kept_P[(size_t)g.wave]);
+      sub_nm.push_back(kept_nm[(size_t)g.wave]);
       if (signalled) {
         done.push_back(flags.counters + f0 + (sub.size() - 1));
         flag.push_back(flags.flags_dev + f0 + (sub.size() - 1));
@@ -1577,6 +1672,8 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
       completion.abort_flag = flags.counters + 2 * MAX_CHUNK_SEGMENTS;
       completion.abort_flag_host = flags.flags_dev + 2 * MAX_CHUNK_SEGMENTS;
       completion.force_pair = force.data();
+      completion.kept_P = sub_P.data();
+      completion.kept_nm = sub_nm.data();
       st = form_batch_impl(sub.data(), (int)sub.size(), wsbuf[b], wsb, cs, &completion);
       if (st != PSTGF_OK) return st;
       launches += tl_launches;
@@ -1605,6 +1702,8 @@ pstgf_status_t pstgf_rmat_form_batch_host(const pstgf_wave_t *waves, int n_waves
     } else {
       BatchCompletion plain;
       plain.force_pair = force.data();
+      plain.kept_P = sub_P.data();
+      plain.kept_nm = sub_nm.data();
       st = form_batch_impl(sub.data(), (int)sub.size(), wsbuf[b], wsb, cs, &plain);
       if (st != PSTGF_OK) return st;
       launches += tl_launches;
@@ -1673,9 +1772,12 @@ pstgf_status_t pstgf_rmat_finalize(void) {
   {
     std::lock_guard<std::mutex> lock(g_pool_mutex);
     for (int dev = 0; dev < 64; ++dev) {
-      if (!g_pool[dev] || !on_device(dev)) continue;
-      cudaMemPoolDestroy(g_pool[dev]);
-      g_pool[dev] = nullptr;
+      if ((!g_pool[dev] && !g_scratch_pool[dev]) || !on_device(dev)) continue;
+      for (cudaMemPool_t *pools : {g_pool, g_scratch_pool})
+        if (pools[dev]) {
+          cudaMemPoolDestroy(pools[dev]);
+          pools[dev] = nullptr;
+        }
     }
   }
   {

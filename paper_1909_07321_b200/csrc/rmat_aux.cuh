@@ -22,7 +22,7 @@ pair_build_kernel(const __grid_constant__ DevWave single, const DevWave *__restr
   for (int p = blockIdx.y; p < n_waves; p += gridDim.y) {
     const DevWave &w = BATCH ? waves[p] : single;
     if (w.n_pairs <= 0) continue;
-    const int K = w.n_poles, C = w.n_chan, N = w.n_E, rows = N + w.n_pairs;
+    const int K = w.n_poles, C = w.n_chan, N = w.n_E, rows = N + (w.pair_keep_P ? 0 : w.n_pairs);   // D rows, then (unless kept) P rows
     const long long sn = w.tr ? 1 : w.ldw, sk = w.tr ? w.ldw : 1;       // element (n, k) of W at W[n * sn + k * sk]
     for (int r0 = blockIdx.x * PAIR_BUILD_ROWS; r0 < rows; r0 += gridDim.x * PAIR_BUILD_ROWS) {
       const int nr = min(PAIR_BUILD_ROWS, rows - r0);

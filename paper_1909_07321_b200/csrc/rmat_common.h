@@ -175,6 +175,7 @@ struct alignas(128) DevWave {
   int pair_x1;             // the first pair_x1 64-pair tiles of energy tile pair_nt_mid are section-1 items too (< pair_mtf; 0 unless pair_nt_mid < pair_nt)
   int pair_nfb;            // n_chan / 8: channel blocks that are full
   int pair_rb;             // rows of P in the block section: 64 pair_nfb (pair_nfb - 1) / 2, see pair_row_channels
+  int pair_keep_P;         // 1: P and pair_nm are there already (built once for the wave, shared by its energy ranges): the scratch builder writes D only
   const unsigned int *pair_nm;   // scratch [n_pairs]: n | m << 16 of every row of P (written by the scratch builder)
 };
 static_assert(sizeof(DevWave) == 768, "DevWave layout (alignas 128; the batch workspace holds an array of these)");

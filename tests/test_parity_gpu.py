@@ -1119,11 +1119,30 @@ def test_host_call_signalled_pipeline_with_pair_form_waves(rmat):
         host.append((torch.from_numpy(w.W).pin_memory(), torch.from_numpy(w.E_k).pin_memory(),
                      torch.from_numpy(w.energies).pin_memory(), w.a, R))
     rmat.pstgf_rmat_form_batch_host(host, max_chunk_bytes=96 * 96 * 8 * 128)
-    # signalled: one scratch-builder launch and one launch per group for the whole job (chunked: a set per piece)
-    assert rmat.pstgf_last_launch_count() == 3
+    # signalled: P of the pair-form wave once, then one D-builder launch and one launch per group for the whole job
+    # (chunked: a set per piece)
+    assert rmat.pstgf_last_launch_count() == 4
     dev = _form_batch(rmat, waves)
     for h, d in zip(host, dev):
         assert torch.equal(h[4], d.cpu())
     w = waves[0]
     Rn = rmat.pstgf_rmat_form_naive(_dev(w.W), _dev(w.E_k), _dev(w.energies[:40]), w.a).cpu().numpy()
     _check(host[0][4].numpy()[:40], Rn)
+
+
+def test_single_wave_pair_scratch_is_bounded(rmat):
+    """pstgf_rmat_form on a pair-form wave with a long mesh: D = 1/(E_k - E_e) for all 40 000 energies would be 154 MB,
+    so the call goes out as two (builder, GEMM) launch pairs over energy ranges that share one P, and the scratch stays
+    at P + 128 MiB whatever n_E is.  Bitwise equal to the batch call, which keeps all of D in the caller's workspace;
+    sampled energies against the term-by-term kernel."""
+    from paper_1909_07321_b200 import inputs
+    w = inputs.make_wave(92, 24, 480, 40000)
+    Wd, Ek, en = _dev(w.W), _dev(w.E_k), _dev(w.energies)
+    R = rmat.pstgf_rmat_form(Wd, Ek, en, w.a)
+    assert rmat.pstgf_last_launch_count() == 4
+    (Rb,) = _form_batch(rmat, [w])
+    torch.cuda.synchronize()
+    assert torch.equal(R, Rb)
+    pick = [0, 1, 34943, 34944, 34945, 39999]              # both sides of the range boundary
+    Rn = rmat.pstgf_rmat_form_naive(Wd, Ek, _dev(w.energies[pick]), w.a).cpu().numpy()
+    _check(R.cpu().numpy()[pick], Rn)
