@@ -97,10 +97,16 @@ def rmat_form(W, E_k, energies, a: float, threads: int = 1, diag_add=None) -> np
 def rmat_entries(W, E_k, energies, a: float, e_idx, n_idx, m_idx, threads: int = 1) -> np.ndarray:
     """R[e_idx[s], n_idx[s], m_idx[s]] of eq. 4, entry by entry (for waves too large to form densely).
 
-    W must already be a C-contiguous float64 array: it is NOT copied (6.2 GB at the paper's scale).
+    W must already be a float64 array whose rows are contiguous: it is NOT copied (6.2 GB at the paper's scale).
+    As in rmat_form, a row stride larger than n_poles (a column slice of a wider array) is passed on as the C
+    routine's leading dimension ldw.
     """
-    if not (isinstance(W, np.ndarray) and W.dtype == np.float64 and W.flags.c_contiguous and W.ndim == 2):
-        raise ValueError("W must be a C-contiguous float64 [n_chan, n_poles] array")
+    if not (isinstance(W, np.ndarray) and W.dtype == np.float64 and W.ndim == 2):
+        raise ValueError("W must be a float64 [n_chan, n_poles] array")
+    rows_ok = W.shape[1] <= 1 or W.strides[1] == W.itemsize
+    ld_ok = W.shape[0] <= 1 or (W.strides[0] % W.itemsize == 0 and W.strides[0] // W.itemsize >= W.shape[1])
+    if not (rows_ok and ld_ok):
+        raise ValueError("W must have unit stride along the poles and a row stride of at least n_poles elements (it is not copied)")
     E_k = np.ascontiguousarray(E_k, dtype=np.float64)
     energies = np.ascontiguousarray(energies, dtype=np.float64)
     if E_k.ndim != 1 or energies.ndim != 1 or W.shape[1] != E_k.shape[0]:
@@ -109,9 +115,10 @@ def rmat_entries(W, E_k, energies, a: float, e_idx, n_idx, m_idx, threads: int =
     if not (idx[0].ndim == 1 and idx[0].shape == idx[1].shape == idx[2].shape):
         raise ValueError("e_idx, n_idx, m_idx must be 1-D and of equal length")
     n_chan, n_poles = W.shape
+    ldw = max(W.strides[0] // W.itemsize, n_poles) if n_chan > 1 else n_poles
     out = np.zeros(idx[0].shape[0], dtype=np.float64)
     ip = ctypes.POINTER(ctypes.c_int)
-    rc = _load().oracle_rmat_entries(_dptr(W), n_poles, _dptr(E_k), _dptr(energies), n_chan, n_poles,
+    rc = _load().oracle_rmat_entries(_dptr(W), ldw, _dptr(E_k), _dptr(energies), n_chan, n_poles,
                                      energies.shape[0], float(a), out.shape[0],
                                      idx[0].ctypes.data_as(ip), idx[1].ctypes.data_as(ip), idx[2].ctypes.data_as(ip),
                                      _dptr(out), int(threads))

@@ -323,9 +323,12 @@ def test_leading_dimension_is_honoured(oracle):
         bound = (np.abs(Wc)[:, None, :] * np.abs(Wc)[None, :, :] / np.abs(E_k - E)).sum(-1) / (2 * 3.0)
         assert np.all(np.abs(R[e] - exact[e]) <= 4 * np.finfo(float).eps * bound)
     assert np.array_equal(R, oracle.rmat_form(np.ascontiguousarray(Wv), E_k, en, 3.0))
-    # the entry-by-entry routine needs a compact W and says so
+    # the entry-by-entry routine takes the same strided W (its own ldw argument): every entry, bitwise the dense
+    # result, with the NaN padding one element past every row; a W that is not contiguous along the poles is refused
+    ee, nn, mm = (x.ravel() for x in np.meshgrid(np.arange(N), np.arange(C), np.arange(C), indexing="ij"))
+    assert np.array_equal(oracle.rmat_entries(Wv, E_k, en, 3.0, ee, nn, mm).reshape(N, C, C), R)
     with pytest.raises(ValueError):
-        oracle.rmat_entries(Wv, E_k, en, 3.0, [0], [0], [0])
+        oracle.rmat_entries(np.ascontiguousarray(Wv.T).T, E_k, en, 3.0, [0], [0], [0])
 
 
 # ---- the diagonal addend (where a caller's Buttle correction goes) -------------------
