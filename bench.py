@@ -76,6 +76,9 @@ def parse_args():
                          "under context.int8_tensor_pops: the number behind DESIGN.md 11.6, not a path of the library")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
+    ap.add_argument("--no-all-configs", action="store_true",
+                    help="skip the `all_configs` entries (configs 1-4 and n_E = 1 / 32 on config 5's wave, 5 steps each) "
+                         "that the default config-5 run adds to its line")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
 
@@ -159,6 +162,20 @@ def job_workload(args, world: int):
         return inputs.make_config(args.config, n_E=args.n_E or None)
     base = inputs.config_shapes(args.config)
     return inputs.make_config(args.config, n_E=world * (args.n_E or base[0][2]))
+
+
+def rank_workload(wl_job, rank: int, world: int):
+    """This rank's share of the job: shard.plan's wave-rotated sets of energy blocks (Fig. 1),
+    waves in the rank's visiting order.  The whole job at world == 1."""
+    import numpy as np
+    from paper_1909_07321_b200 import inputs, shard
+    if world == 1:
+        return wl_job
+    wl = inputs.Workload(name=wl_job.name, seed=wl_job.seed)
+    for p, idx in shard.plan([w.n_E for w in wl_job.waves], rank, world):
+        w = wl_job.waves[p]
+        wl.waves.append(inputs.Wave(w.W, w.E_k, np.ascontiguousarray(w.energies[idx]), w.a))
+    return wl
 
 
 def workload_description(cfg: int, wl) -> dict:
@@ -305,14 +322,17 @@ def ncu_traffic(cfg: int):
 
 
 # ---- prior art on the same GPU (context) ---------------------------------------------------------
-def prior_art_leg(wl, n_sample: int = 16) -> dict:
+def prior_art_leg(wl, n_sample: int = 16, library_R=None) -> dict:
     """The scheme the paper describes for its CUDA-Fortran RINIT (Fig. 2), with a library DGEMM
     (cuBLAS through torch.matmul, float64) standing in for its matrix-multiply routine: per energy, form the scaled
     copy W diag(d), compute the 10 upper-triangle blocks of a 4 x 4 block grid one after another, symmetrise.
-    Timed on the first `n_sample` energies of every wave with CUDA events; every energy costs the same."""
+    Timed on the first `n_sample` energies of every wave with CUDA events; every energy costs the same.
+    library_R: per wave, this library's R for (at least) those energies (host or device tensors): the comparator's
+    result is checked against it, so that what is timed is known to be eq. 4 (reported as max_rel_err_vs_library,
+    the parity tests' per-energy measure)."""
     import torch
     total_ms, n_done, worst = 0.0, 0, 0.0
-    for w in wl.waves:
+    for wi, w in enumerate(wl.waves):
         W = torch.from_numpy(w.W).cuda()
         Ek = torch.from_numpy(w.E_k).cuda()
         en = torch.from_numpy(w.energies).cuda()
@@ -343,6 +363,11 @@ def prior_art_leg(wl, n_sample: int = 16) -> dict:
         torch.cuda.synchronize()
         total_ms += e0.elapsed_time(e1)
         n_done += k
+        if library_R is not None:
+            ref = library_R[wi][:k].to("cuda")
+            num = (R - ref).abs().reshape(k, -1).amax(1)
+            den = ref.abs().reshape(k, -1).amax(1)
+            worst = max(worst, float((num / den).max()))
     # a stronger library baseline: scaled copies of 8 energies at once and ONE batched DGEMM for the full squares
     b_ms, b_done = 0.0, 0
     for w in wl.waves:
@@ -375,7 +400,62 @@ def prior_art_leg(wl, n_sample: int = 16) -> dict:
             "value": n_done / (total_ms * 1e-3), "unit": UNIT, "kind": "paper's scheme (PAPER.md:164-166) with cuBLAS DGEMM via "
             "torch.matmul: scaled copy + 10 upper-triangle block multiplies + symmetrise, one energy at a time",
             "sample": f"first {n_sample} energies of each wave ({n_done} energies, {total_ms:.2f} ms)",
-            "tflops_counted": flop / (total_ms * 1e-3) / 1e12}
+            "tflops_counted": flop / (total_ms * 1e-3) / 1e12,
+            "max_rel_err_vs_library": worst if library_R is not None else None}
+
+
+# ---- the other configurations, in the same line ------------------------------------------------------
+def quick_config_line(cfg: int, n_E, peak_tflops: float, flush_buf, device_index: int, steps: int = 5, warmup: int = 3) -> dict:
+    """One configuration through the device-pointer calls, timed like the headline (L2 flushed between steps, CUDA
+    events on the launch stream, clocks sampled during its own timed region), as an entry of `all_configs`."""
+    import torch
+    from paper_1909_07321_b200 import inputs, rmat
+    wl = inputs.make_config(cfg, n_E=n_E)
+    dev, shared = [], {}
+    for w in wl.waves:
+        key = id(w.energies)
+        if key not in shared:
+            shared[key] = torch.from_numpy(w.energies).cuda()
+        R = torch.empty((w.n_E, w.n_chan, w.n_chan), dtype=torch.float64, device="cuda")
+        dev.append((torch.from_numpy(w.W).cuda(), torch.from_numpy(w.E_k).cuda(), shared[key], w.a, R))
+    if len(dev) > 1:
+        arr = rmat.make_wave_array(dev)
+        ws = torch.empty(rmat.pstgf_rmat_batch_workspace_bytes(arr), dtype=torch.uint8, device="cuda")
+
+    def step():
+        if len(dev) == 1:
+            W, E_k, en, a, R = dev[0]
+            rmat.pstgf_rmat_form(W, E_k, en, a, R_out=R)
+        else:
+            rmat.pstgf_rmat_form_batch(arr, ws)
+        return rmat.pstgf_last_launch_count()
+
+    for _ in range(warmup):
+        flush_buf.zero_()
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(device_index)
+    sampler.start()
+    time.sleep(0.12)
+    ms, launches = [], 0
+    t_end = time.perf_counter() + 0.25                     # at least a quarter of a second under load for the clock samples
+    while len(ms) < steps or time.perf_counter() < t_end:
+        flush_buf.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        n = step()
+        e1.record()
+        torch.cuda.synchronize()
+        if len(ms) < steps:
+            ms.append(e0.elapsed_time(e1))
+            launches += n
+    clocks = sampler.stop()
+    t = sum(ms) / len(ms)
+    tf = wl.counted_flop() / (t * 1e-3) / 1e12
+    return {"config": cfg, "n_E": n_E, "workload": workload_description(cfg, wl)["workload"] + (f", n_E overridden to {n_E}" if n_E else ""),
+            "steps": len(ms), "warmup": warmup, "ms_per_step": t, "step_ms_min_max": [min(ms), max(ms)],
+            "energies_per_s": wl.n_energies() / (t * 1e-3), "tflops_counted": tf, "frac": tf / peak_tflops,
+            "gpu_launches": launches, "clocks": clocks}
 
 
 # ---- CUDA arm ----------------------------------------------------------------------------------
@@ -408,14 +488,7 @@ def run_cuda(args):
     wl_job = job_workload(args, world)
     n_e_job = wl_job.n_energies()
     job_description = workload_description(args.config, wl_job)
-    if world == 1:
-        wl = wl_job
-    else:
-        from paper_1909_07321_b200 import shard
-        wl = inputs.Workload(name=wl_job.name, seed=wl_job.seed)
-        for p, idx in shard.plan([w.n_E for w in wl_job.waves], rank, world):
-            w = wl_job.waves[p]
-            wl.waves.append(inputs.Wave(w.W, w.E_k, np.ascontiguousarray(w.energies[idx]), w.a))
+    wl = rank_workload(wl_job, rank, world)
     hdat = args.w_layout == "channels"
     layout = rmat.PSTGF_W_CHANNEL_CONTIGUOUS if hdat else rmat.PSTGF_W_POLE_CONTIGUOUS
 
@@ -605,9 +678,26 @@ def run_cuda(args):
 
     prior = None
     if rank == 0 and world == 1 and args.prior_art:
+        lib_R = [d[4][:16].cpu() for d in dev_waves]       # the library's R of the energies the comparator forms
         del dev_waves
         torch.cuda.empty_cache()
-        prior = prior_art_leg(wl)
+        prior = prior_art_leg(wl, library_R=lib_R)
+        if not prior["max_rel_err_vs_library"] <= 1e-11:
+            raise RuntimeError(f"prior-art comparator disagrees with the library: {prior['max_rel_err_vs_library']:.3e}")
+
+    # the other BASELINE.json configurations and the few-energy shapes of config 5's wave, so that every fraction
+    # DESIGN.md quotes has a twin in the driver's record (default run only: config 5, one GPU, the DMMA path)
+    all_configs = None
+    if rank == 0 and world == 1 and args.config == 5 and not args.n_E and not sliced and not args.no_all_configs and probe:
+        try:
+            del dev_waves
+        except NameError:
+            pass
+        torch.cuda.empty_cache()
+        all_configs = []
+        for cfg, n_E in ((1, None), (2, None), (3, None), (4, None), (5, 1), (5, 32)):
+            all_configs.append(quick_config_line(cfg, n_E, roofline["peak"], flush_buf, local_rank))
+            torch.cuda.empty_cache()
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -629,6 +719,7 @@ def run_cuda(args):
                 "tflops_counted": wl_job.counted_flop() * args.steps / (total_ms_max * 1e-3) / 1e12,
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,
                 **({"prior_art": prior} if prior else {}), **({"context": context} if context else {}),
+                **({"all_configs": all_configs} if all_configs else {}),
                 "clocks": clocks, "wall_s_timed_region": wall, "step_ms_min_max": [min(step_ms), max(step_ms)]}
         print(json.dumps(line), flush=True)
     if world > 1:
