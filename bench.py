@@ -74,6 +74,9 @@ def parse_args():
     ap.add_argument("--probe-i8", action="store_true",
                     help="also run the INT8 tensor-pipe probe (tcgen05.mma kind::i8, measure/i8_probe.cu) and report its rate "
                          "under context.int8_tensor_pops: the number behind DESIGN.md 11.6, not a path of the library")
+    ap.add_argument("--probe-l2", action="store_true",
+                    help="run ONLY the L2 -> shared-memory load-rate probe (measure/l2_probe.cu: TMA boxes of several inner "
+                         "extents, 1-D bulk copies, issuing lanes, ring depths, multicast over 2 and 4 CTAs) and print its table")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--no-all-configs", action="store_true",
@@ -458,6 +461,38 @@ def quick_config_line(cfg: int, n_E, peak_tflops: float, flush_buf, device_index
             "gpu_launches": launches, "clocks": clocks}
 
 
+# ---- L2 -> SM load-rate probe ------------------------------------------------------
+def l2_probe_table(device_index: int, sm_mhz: float) -> list:
+    """Every row of probe.L2_PROBE_SWEEP on all SMs: best of 3 launches over a 32 MB array (L2-resident after the
+    first pass), CUDA events.  delivered = bytes that arrived in shared memory; from_l2 = delivered / cluster size."""
+    import torch
+    from paper_1909_07321_b200.measure import probe
+    sms = torch.cuda.get_device_properties(device_index).multi_processor_count
+    src = torch.zeros(400 * probe.L2_PROBE_PITCH, dtype=torch.uint8, device="cuda")
+    status = torch.zeros(1, dtype=torch.int32, device="cuda")
+    rows = []
+    for label, mode, inner, box_rows, bps, lanes, stages, cluster in probe.L2_PROBE_SWEEP:
+        stage_bytes = inner * box_rows * bps
+        iters = max(4 * stages, (64 << 20) // stage_bytes)
+        n_ctas = sms - sms % cluster
+        best = None
+        for rep in range(4):                                  # the first pass loads L2 and the kernel
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            delivered = probe.l2_probe(mode, inner, box_rows, bps, lanes, stages, cluster, iters, n_ctas, src, status)
+            e1.record()
+            torch.cuda.synchronize()
+            if rep:
+                best = e0.elapsed_time(e1) if best is None else min(best, e0.elapsed_time(e1))
+        if int(status.item()) != 0:
+            raise RuntimeError(f"l2 probe timed out in {label!r}")
+        tbs = delivered / (best * 1e-3) / 1e12
+        rows.append({"pattern": label, "cluster": cluster, "in_flight_kb_per_cta": stages * stage_bytes / 1024,
+                     "delivered_tb_s": tbs, "delivered_b_per_clk_per_sm": delivered / (best * 1e-3) / (sm_mhz * 1e6) / n_ctas,
+                     "from_l2_tb_s": tbs / cluster, "ms": best})
+    return rows
+
+
 # ---- CUDA arm ----------------------------------------------------------------------------------
 def run_cuda(args):
     import numpy as np
@@ -480,6 +515,17 @@ def run_cuda(args):
     rmat.pstgf_debug_set_slab_policy({"auto": rmat.PSTGF_SLAB_AUTO, "none": rmat.PSTGF_SLAB_NONE, "32": rmat.PSTGF_SLAB_T32,
                                       "64": rmat.PSTGF_SLAB_T64, "128": rmat.PSTGF_SLAB_T128}[args.slab_policy])
     peaks = measured_peaks()
+    if args.probe_l2:
+        if rank == 0:
+            sampler = ClockSampler(local_rank)
+            sampler.start()
+            table = l2_probe_table(local_rank, peaks["sm_max_mhz"])
+            print(json.dumps({"probe": "l2_to_shared_memory", "unit": "TB/s delivered into shared memory, all SMs",
+                              "source": "32 MB array, L2-resident; one issuing warp per CTA, one CTA per SM, best of 3",
+                              "sm_mhz_assumed": peaks["sm_max_mhz"], "rows": table, "clocks": sampler.stop()}), flush=True)
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
 
     # Weak scaling over ranks: at N ranks the job is the configuration with an N times
     # finer energy mesh; shard.plan gives each rank its wave-rotated share of the energy blocks (PAPER.md:116,

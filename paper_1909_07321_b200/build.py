@@ -18,7 +18,8 @@ HEADERS = [os.path.join(CSRC, "rmat_common.h"), os.path.join(CSRC, "rmat_kernel.
 UNITS = [(SOURCES[0], []), (SOURCES[1], ["-DPSTGF_FAM=0"]), (SOURCES[1], ["-DPSTGF_FAM=1"]), (SOURCES[1], ["-DPSTGF_FAM=2"]),
          (SOURCES[2], []), (SOURCES[3], [])]
 PROBE_LIB = os.path.join(_HERE, "libpstgf_probe.so")
-PROBE_SOURCES = [os.path.join(_HERE, "measure", "fp64_probe.cu"), os.path.join(_HERE, "measure", "i8_probe.cu")]
+PROBE_SOURCES = [os.path.join(_HERE, "measure", "fp64_probe.cu"), os.path.join(_HERE, "measure", "i8_probe.cu"),
+                 os.path.join(_HERE, "measure", "l2_probe.cu")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]
 

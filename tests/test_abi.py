@@ -132,6 +132,7 @@ def test_product_library_holds_no_measurement_code(lib):
     from paper_1909_07321_b200 import build
     assert hasattr(ctypes.CDLL(build.PROBE_LIB), "pstgf_fp64_probe")
     assert hasattr(ctypes.CDLL(build.PROBE_LIB), "pstgf_i8_probe") and not hasattr(lib, "pstgf_i8_probe")
+    assert hasattr(ctypes.CDLL(build.PROBE_LIB), "pstgf_l2_probe") and not hasattr(lib, "pstgf_l2_probe")
 
 
 def test_mesh_from_zscaled(lib):

@@ -1199,3 +1199,29 @@ def test_prior_art_comparator_matches_the_library(rmat):
     out = bench.prior_art_leg(wl, n_sample=16, library_R=lib_R)
     assert out["max_rel_err_vs_library"] is not None and out["max_rel_err_vs_library"] <= 1e-12
     assert out["value"] > 0 and out["cublas_batched"]["value"] > 0
+
+
+def test_l2_probe_runs_and_counts_its_bytes():
+    """The bench-side L2 -> shared-memory load-rate probe (measure/l2_probe.cu): a 2-D TMA pattern, a
+    1-D bulk pattern and a multicast pattern over 2 and 4 CTAs finish without a timed-out wait, report the bytes they
+    delivered, and move them at more than 1 TB/s over all SMs (an order-of-magnitude check that TMA, not a fallback,
+    did the moving)."""
+    from paper_1909_07321_b200.measure import probe
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    src = torch.zeros(400 * probe.L2_PROBE_PITCH, dtype=torch.uint8, device="cuda")
+    status = torch.zeros(1, dtype=torch.int32, device="cuda")
+    for mode, inner, rows, bps, lanes, stages, cluster in ((0, 160, 32, 8, 8, 4, 1), (1, 8192, 1, 5, 5, 4, 1),
+                                                            (0, 160, 32, 8, 4, 4, 2), (0, 160, 32, 8, 2, 4, 4)):
+        n_ctas = sms - sms % cluster
+        iters = 400
+        probe.l2_probe(mode, inner, rows, bps, lanes, stages, cluster, iters, n_ctas, src, status)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        b = probe.l2_probe(mode, inner, rows, bps, lanes, stages, cluster, iters, n_ctas, src, status)
+        e1.record()
+        torch.cuda.synchronize()
+        assert int(status.item()) == 0
+        assert b == float(n_ctas) * iters * inner * rows * bps
+        assert b / (e0.elapsed_time(e1) * 1e-3) > 1e12
+    with pytest.raises(RuntimeError):
+        probe.l2_probe(1, 8192, 1, 6, 6, 4, 2, 10, sms, src, status)      # multicast is a 2-D TMA mode only
