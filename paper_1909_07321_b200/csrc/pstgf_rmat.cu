@@ -390,17 +390,22 @@ double simulate_makespan(const std::vector<std::pair<double, int>> &runs, int gr
 //  - its busiest SM sub-partition's DMMAs: blocks per warp (SlabShape: nr x ncw) x warps per sub-partition x 5 k-steps
 //    x 16 clk, times a factor for the quality of the warp's inner loop (fewer DMMAs per fragment load and per scaling
 //    multiply in the small shapes; fitted to the B200 sweeps of bench.py --n-E), and
-//  - its panels coming out of L2: with every SM loading, L2 delivers 4.2 TB/s chip-wide, 15 B/clk per SM (measured:
-//    one energy at 512 x 10240 on tiles of edge 32 runs at 634 clk per k-tile for 10 KB of panels),
+//  - the rate at which a slab item is SEEN to take its panels in: 15 B/clk per SM, 4.2 TB/s chip-wide (measured: one
+//    energy at 512 x 10240 on tiles of edge 32 runs at 634 clk per k-tile for 10 KB of panels).  This is a fitted item
+//    rate, NOT the L2 -> SM fabric: the probe of measure/l2_probe.cu delivers 28-31 B/clk per SM (8-9 TB/s) on this
+//    chip (profiles/r03_l2_probe.md), and issuing the boxes of four stages in one TMA instruction -- the pattern
+//    that takes the probe from 2.6 to 8 TB/s -- left these items where they were (0.170 -> 0.169 ms):
+//    a k-tile of an edge-32 tile is 320 clk of DMMA issue on a sub-partition that holds ONE computing warp, and that
+//    warp's wait / fragment loads / scaling / dependent DMMAs / release run one after the other,
 // plus a fixed cost per item (epilogue, ring refill) of three k-tiles.
-constexpr double L2_BYTES_PER_CLK_PER_SM = 15.0;
+constexpr double SLAB_PANEL_BYTES_PER_CLK = 15.0;
 double slab_item_cost(int T, int g, int n_kt) {
   const pstgf::SlabShape sh = pstgf::slab_shape(T, g);
   const int blocks = sh.nr * sh.ncw;
   const double quality = blocks >= 32 ? 1.0 : blocks >= 16 ? 1.04 : blocks >= 8 ? 1.10 : 1.15;
   const double warps_per_smsp = (T == 32 && g == 1) ? 1.0 : 2.0;          // (edge 32 with one energy keeps four warps idle)
   const double compute = blocks * warps_per_smsp * 80.0 * quality;
-  const double l2 = pstgf::slab_panels(T) * (double)pstgf::BOX_BYTES / L2_BYTES_PER_CLK_PER_SM;
+  const double l2 = pstgf::slab_panels(T) * (double)pstgf::BOX_BYTES / SLAB_PANEL_BYTES_PER_CLK;
   return std::max(compute, l2) * ((double)n_kt + 3.0);
 }
 
