@@ -1225,3 +1225,57 @@ def test_l2_probe_runs_and_counts_its_bytes():
         assert b / (e0.elapsed_time(e1) * 1e-3) > 1e12
     with pytest.raises(RuntimeError):
         probe.l2_probe(1, 8192, 1, 6, 6, 4, 2, 10, sms, src, status)      # multicast is a 2-D TMA mode only
+
+
+def test_R_out_in_mapped_host_memory_more_kernels(rmat):
+    """The mapped-host-memory stress of test_R_out_in_mapped_host_memory (every store a PCIe write, the load/store unit
+    backed up for microseconds: the only race detector this pool allows) on the kernels it did not reach: slab tiles
+    of edge 64 and 128 (one energy of a 1100-channel wave), the one-launch kernel for tiny waves, and the sliced
+    variant's GEMM (a two-stage ring released by tcgen05.commit).  Each bitwise equal to its device-memory run."""
+    from paper_1909_07321_b200 import inputs
+    lib = rmat.load()
+    stream = lambda: torch.cuda.current_stream().cuda_stream
+
+    def both(w, call):
+        """call(R_ptr) enqueues the formation into R; returns (device-memory result, mapped-host result)."""
+        R_dev = torch.full((w.n_E, w.n_chan, w.n_chan), float("nan"), dtype=torch.float64, device="cuda")
+        assert call(R_dev.data_ptr()) == 0
+        torch.cuda.synchronize()
+        R_host = torch.full((w.n_E, w.n_chan, w.n_chan), float("nan"), dtype=torch.float64).pin_memory()
+        assert call(R_host.data_ptr()) == 0
+        torch.cuda.synchronize()
+        return R_dev.cpu(), R_host
+
+    # slab tiles of edge 64 and 128: one energy of a 1100-channel wave
+    w = inputs.make_wave(5160, 1100, 2200, 1)
+    Wd, Ek, en = _dev(w.W), _dev(w.E_k), _dev(w.energies)
+    try:
+        for policy in (rmat.PSTGF_SLAB_T64, rmat.PSTGF_SLAB_T128):
+            rmat.pstgf_debug_set_slab_policy(policy)
+            for trial in range(2):
+                a, b = both(w, lambda R: lib.pstgf_rmat_form(Wd.data_ptr(), Wd.stride(0), Ek.data_ptr(), en.data_ptr(), w.n_chan,
+                                                             w.n_poles, w.n_E, w.a, R, stream()))
+                assert bool(torch.isfinite(a).all()) and torch.equal(a, b), f"slab policy {policy}, trial {trial}"
+    finally:
+        rmat.pstgf_debug_set_slab_policy(rmat.PSTGF_SLAB_AUTO)
+    # the one-launch kernel for tiny waves (BASELINE.json configs[0]'s shape)
+    w1 = inputs.make_wave(5161, 8, 160, 1000)
+    W1, Ek1, en1 = _dev(w1.W), _dev(w1.E_k), _dev(w1.energies)
+    for trial in range(2):
+        a, b = both(w1, lambda R: lib.pstgf_rmat_form(W1.data_ptr(), W1.stride(0), Ek1.data_ptr(), en1.data_ptr(), w1.n_chan,
+                                                      w1.n_poles, w1.n_E, w1.a, R, stream()))
+        assert rmat.pstgf_last_launch_count() == 1               # rmat_small_kernel, nothing else
+        assert bool(torch.isfinite(a).all()) and torch.equal(a, b), f"small kernel, trial {trial}"
+    # the sliced variant's GEMM
+    w2 = inputs.make_wave(5162, 130, 300, 5)
+    W2, Ek2, en2 = _dev(w2.W), _dev(w2.E_k), _dev(w2.energies)
+    ws = torch.empty(rmat.pstgf_rmat_sliced_workspace_bytes(w2.n_chan, w2.n_poles, w2.n_E, 7), dtype=torch.uint8, device="cuda")
+
+    def sliced(R):
+        wave = rmat.pstgf_wave_t(w2.n_chan, w2.n_poles, w2.n_E, rmat.PSTGF_W_POLE_CONTIGUOUS, W2.stride(0), w2.a, W2.data_ptr(),
+                                 Ek2.data_ptr(), en2.data_ptr(), R, None)
+        return lib.pstgf_rmat_form_sliced(ctypes.byref(wave), 7, ws.data_ptr(), ws.numel(), stream())
+
+    for trial in range(2):
+        a, b = both(w2, sliced)
+        assert bool(torch.isfinite(a).all()) and torch.equal(a, b), f"sliced GEMM, trial {trial}"
